@@ -1,0 +1,149 @@
+/* pfc.h -- C ABI of libpfc: per-step energy, forces and velocity-Verlet update
+ * of an ANI-style machine-learned interatomic potential on one NVIDIA B200
+ * (sm_100a).
+ *
+ * What the calls are.  The paper (arxiv 2412.18271, "OpenMM-Python-Force")
+ * states the problem: an MD integrator calls a provider every step with the
+ * positions and receives the scalar energy, forces being -dE/dx by
+ * differentiation (section 2.1 / listing) or returned
+ * explicitly (section 3.2); tensors stay on the device
+ * (abstract); integration is NVE from 300 K velocities
+ * (section 3.1).  BASELINE.json:north_star names the four entry
+ * points (pfc_create, pfc_energy_forces, pfc_step, pfc_destroy); the
+ * potential itself is BASELINE.json:configs[0] completed by DESIGN.md
+ * "Readings" S1-S24.
+ *
+ * Conventions
+ *  - Units: Angstrom, eV, eV/Angstrom, amu, fs, Angstrom/fs.
+ *    (OpenMM side of the paper: 1 nm = 10 A, 1 eV = 96.485332 kJ/mol.)
+ *  - "DEVICE" pointers are CUDA device memory owned by the caller (PyTorch in
+ *    this repository); "HOST" pointers are ordinary host memory.  The library
+ *    never allocates device memory: everything it needs is carved out of the
+ *    caller's `workspace`.
+ *  - pos / vel / frc are arrays of 4 floats per atom (float4, 16-byte
+ *    aligned): pos = {x,y,z,ignored}, vel = {vx,vy,vz,ignored},
+ *    frc = {Fx,Fy,Fz,e_i} where e_i is the atom's energy contribution.
+ *    The .w lanes of caller-owned pos/vel are never written.
+ *  - Atoms of system s are the contiguous range sys_offsets[s]..sys_offsets[s+1];
+ *    there are no pairs across systems.
+ *  - Every call except create/destroy/status/run_host only ENQUEUES work on
+ *    the given stream and returns; it never synchronises.
+ *  - Return value: PFC_OK (0) or a negative PFC_ERR_* code.  Nothing throws or
+ *    aborts across this boundary.  Conditions detected on the device
+ *    (neighbour capacity overflow, angular row longer than PFC_MAX_ANGULAR,
+ *    non-finite energy) set sticky bits readable with pfc_status(); outputs
+ *    are then unspecified.
+ *  - One handle = one stream = one caller at a time.
+ */
+#ifndef PFC_H_
+#define PFC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PFC_OK 0
+#define PFC_ERR_ARG (-1)        /* NULL / out-of-range argument                  */
+#define PFC_ERR_SPECIES (-2)    /* species outside 0..3 or bad sys_offsets       */
+#define PFC_ERR_WORKSPACE (-3)  /* workspace missing, misaligned or too small    */
+#define PFC_ERR_CUDA (-4)       /* a CUDA runtime call failed                    */
+#define PFC_ERR_CAPTURE (-5)    /* graph capture / instantiate failed            */
+#define PFC_ERR_STATE (-6)      /* pfc_step before pfc_set_state                 */
+
+/* sticky device status bits (pfc_status) */
+#define PFC_STATUS_RADIAL_OVERFLOW 1u   /* total radial entries > capacity       */
+#define PFC_STATUS_ANGULAR_OVERFLOW 2u  /* total angular entries > capacity      */
+#define PFC_STATUS_ANGULAR_ROW 4u       /* one atom has > PFC_MAX_ANGULAR angular neighbours */
+#define PFC_STATUS_NONFINITE 8u         /* a system energy is NaN/Inf            */
+#define PFC_STATUS_CELL_OVERFLOW 16u    /* cell grid exceeded its capacity       */
+
+#define PFC_AEV_LEN 384                 /* 64 radial + 320 angular (configs[0])  */
+#define PFC_N_WEIGHTS 378756            /* 4 elements x 94,689 (O5)    */
+#define PFC_MAX_ANGULAR 96              /* angular neighbours one atom may have  */
+
+#define PFC_MLP_FP32 0                  /* FP32 FFMA grouped MLP                 */
+#define PFC_MLP_TF32X3 1                /* tcgen05 kind::tf32, 3-term split      */
+
+typedef struct pfc_ctx pfc_t;           /* opaque; owned by the library          */
+
+/* All pointers in the descriptor are HOST pointers except `workspace`;
+ * everything is copied during pfc_create and may be freed afterwards
+ * (the workspace must outlive the handle). */
+typedef struct {
+  int32_t n_atoms;               /* >= 1                                           */
+  int32_t n_systems;             /* >= 1                                           */
+  const int32_t *species;        /* HOST [n_atoms], 0=H 1=C 2=N 3=O               */
+  const int32_t *sys_offsets;    /* HOST [n_systems+1], ascending, [0]=0, last=n_atoms */
+  const float *weights;          /* HOST [PFC_N_WEIGHTS]; per element e=0..3:
+                                    W1[160][384] b1[160] W2[128][160] b2[128]
+                                    W3[96][128] b3[96] W4[1][96] b4[1], row-major [out][in] */
+  const float *masses_amu;       /* HOST [4] or NULL -> {1.008,12.011,14.007,15.999} */
+  void *workspace;               /* DEVICE, 256-byte aligned, >= pfc_workspace_bytes() */
+  size_t workspace_bytes;
+  int32_t mlp_path;              /* PFC_MLP_FP32 or PFC_MLP_TF32X3                 */
+} pfc_desc_t;
+
+/* Bytes of device workspace pfc_create needs for these sizes (0 on bad args). */
+size_t pfc_workspace_bytes(int32_t n_atoms, int32_t n_systems);
+
+/* Validates the descriptor, builds the static element grouping, uploads the
+ * weights (synchronous copies on the legacy stream) and returns a handle. */
+int pfc_create(const pfc_desc_t *desc, pfc_t **out);
+
+/* Energy and forces at the given positions (explicit-force
+ * return as in PAPER.md:121).  pos: DEVICE [n_atoms] float4 (read only).
+ * E: DEVICE [n_systems] floats, potential energy per system.  F: DEVICE
+ * [n_atoms] float4 = {-dE/dx, -dE/dy, -dE/dz, e_i}.  stream: a cudaStream_t
+ * (NULL = legacy default stream).  Enqueues: neighbour build (K1), AEV (K2),
+ * MLP forward/backward (K3), force chain rule + gather (K4), energy sum. */
+int pfc_energy_forces(pfc_t *ctx, const float *pos, float *E, float *F, void *stream);
+
+/* Binds (does not copy) the MD state advanced by pfc_step: pos, vel DEVICE
+ * [n_atoms] float4, updated in place; E DEVICE [n_systems]; F DEVICE [n_atoms]
+ * float4 (forces/energies of the last completed step).  Resets the internal
+ * position-compensation words and marks forces as stale so that the next
+ * pfc_step evaluates them at the bound positions first. */
+int pfc_set_state(pfc_t *ctx, float *pos, float *vel, float *E, float *F, void *stream);
+
+/* n_steps of velocity-Verlet (O8) with time step dt_fs
+ * on the bound state, on the bound stream, by replaying one captured CUDA
+ * graph per step with no host round trip.  On return (after the caller syncs
+ * the stream) pos, vel, F, E hold the synchronous (x_n, v_n, F(x_n), E(x_n)). */
+int pfc_step(pfc_t *ctx, int32_t n_steps, float dt_fs);
+
+/* Host-buffer convenience path (used for end-to-end timing): copies pos/vel
+ * HOST [n_atoms][4] to internal device buffers, runs n_steps, copies pos, vel,
+ * F (optional, may be NULL) and E HOST [n_systems] back, and synchronises. */
+int pfc_run_host(pfc_t *ctx, float *pos_host, float *vel_host, int32_t n_steps, float dt_fs,
+                 float *E_host, float *F_host, void *stream);
+
+/* Parity getters: DEVICE pointers into the workspace, valid until the next
+ * call that enqueues work.  Lists are int32 CSR, rows ascending by neighbour
+ * index (O2/S7). */
+int pfc_get_neighbors(pfc_t *ctx, const int32_t **r_off, const int32_t **r_idx,
+                      const int32_t **a_off, const int32_t **a_idx);
+/* aev, g: [n_rows][384] in element-sorted padded row order; row_of_atom
+ * DEVICE [n_atoms] gives each atom's row. */
+int pfc_get_intermediates(pfc_t *ctx, const float **aev, const float **g,
+                          const int32_t **row_of_atom, int32_t *n_rows);
+
+/* Parity helper: synchronous cudaMemcpy of `bytes` from a DEVICE pointer returned
+ * by the getters above into HOST memory. */
+int pfc_copy_to_host(const void *device_src, void *host_dst, size_t bytes);
+
+/* Synchronises the bound/last-used stream and returns the sticky status bits. */
+int pfc_status(pfc_t *ctx, uint32_t *bits);
+
+/* Number of kernel launches one energy_forces pass / one MD step enqueues. */
+int pfc_launch_counts(pfc_t *ctx, int32_t *per_energy_forces, int32_t *per_step);
+
+int pfc_destroy(pfc_t *ctx);
+const char *pfc_error_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PFC_H_ */

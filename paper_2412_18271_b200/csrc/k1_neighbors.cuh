@@ -1,0 +1,379 @@
+// k1_neighbors.cuh -- K1: gas-phase neighbour builder (O2, S6, S7, S22).
+//
+// Output: int32 CSR, rows by atom index, neighbours ascending:
+//   r_off[N+1], r_idx[]  all j != i of the same system with d2 <  RC2_R
+//   a_off[N+1], a_idx[]  the subset with                     d2 <  RC2_A
+// The predicate is the fp32, individually rounded expression dist2_rn().
+// Two passes (count -> exclusive scan -> fill) give exact-size pooled rows
+// inside a static CUDA graph; ordered compaction is ballot + popc, no sort.
+//
+//  * brute force: one warp per atom scans its own system 32 atoms at a time
+//    (systems <= BRUTE_MAX atoms)
+//  * cell list (systems > BRUTE_MAX atoms): per-step bounding box, cells of
+//    edge >= 5.2*(1+2^-10), atoms binned in ascending index order per cell,
+//    27-cell stencil walked in ascending cell order, rows ordered by index with
+//    a rank-by-count pass.  The same predicate decides membership.
+#pragma once
+#include "pfc_common.cuh"
+
+namespace pfc {
+
+constexpr int K1_WARPS = 8;
+constexpr int SCAN_THREADS = 256, SCAN_ITEMS = 8, SCAN_BLOCK = SCAN_THREADS * SCAN_ITEMS;  // 2048
+
+// ---- brute force -----------------------------------------------------------
+// FILL=false: counts -> cnt[i] = {radial, angular}; also writes the packed copy
+//             xs[i] = {x, y, z, bitcast(species)} every later kernel reads.
+// FILL=true : writes r_idx / a_idx rows at r_off[i] / a_off[i].
+template <bool FILL>
+__global__ void __launch_bounds__(K1_WARPS * 32)
+k1_brute_kernel(int n_atoms, const float4* __restrict__ pos, const int* __restrict__ species,
+                const int* __restrict__ sys_id, const int* __restrict__ sys_off,
+                const unsigned char* __restrict__ sys_is_cell,
+                float4* __restrict__ xs, int2* __restrict__ cnt,
+                const int* __restrict__ r_off, const int* __restrict__ a_off,
+                int* __restrict__ r_idx, int* __restrict__ a_idx, int cap_r, int cap_a) {
+  int i = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
+  if (i >= n_atoms) return;
+  const uint32_t lane = lane_id();
+  float4 pi = pos[i];
+  int sid = sys_id[i];
+  if (!FILL && lane == 0) {
+    float4 o = pi;
+    o.w = __int_as_float(species[i]);
+    xs[i] = o;
+  }
+  if (sys_is_cell[sid]) return;          // handled by the cell-list kernels
+  int b = sys_off[sid], e = sys_off[sid + 1];
+  int nr = 0, na = 0;
+  int ro = 0, ao = 0;
+  if (FILL) {
+    ro = r_off[i]; ao = a_off[i];
+    // capacity overflow was flagged by the scan; never write out of bounds
+    if (r_off[i + 1] > cap_r || a_off[i + 1] > cap_a) return;
+  }
+  for (int j0 = b; j0 < e; j0 += 32) {
+    int j = j0 + (int)lane;
+    bool valid = (j < e) && (j != i);
+    float d2 = 1e30f;
+    if (valid) {
+      float4 pj = pos[j];
+      d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+    }
+    uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
+    uint32_t ma = __ballot_sync(0xffffffffu, d2 < RC2_A);
+    if (FILL) {
+      uint32_t lt = lanemask_lt();
+      if (d2 < RC2_R) r_idx[ro + nr + __popc(mr & lt)] = j;
+      if (d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
+    }
+    nr += __popc(mr);
+    na += __popc(ma);
+  }
+  if (!FILL && lane == 0) cnt[i] = make_int2(nr, na);
+}
+
+// ---- exclusive scan of cnt -> r_off, a_off (reduce-then-scan, two tiny kernels)
+__global__ void __launch_bounds__(SCAN_THREADS)
+k1_scan_totals_kernel(int n, const int2* __restrict__ cnt, int2* __restrict__ block_tot) {
+  __shared__ int2 wsum[SCAN_THREADS / 32];
+  int base = blockIdx.x * SCAN_BLOCK;
+  int sr = 0, sa = 0;
+  for (int q = threadIdx.x; q < SCAN_BLOCK; q += SCAN_THREADS) {
+    int i = base + q;
+    if (i < n) { int2 c = cnt[i]; sr += c.x; sa += c.y; }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    sr += __shfl_xor_sync(0xffffffffu, sr, o);
+    sa += __shfl_xor_sync(0xffffffffu, sa, o);
+  }
+  if (lane_id() == 0) wsum[threadIdx.x >> 5] = make_int2(sr, sa);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int2 t = make_int2(0, 0);
+    for (int w = 0; w < SCAN_THREADS / 32; ++w) { t.x += wsum[w].x; t.y += wsum[w].y; }
+    block_tot[blockIdx.x] = t;
+  }
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS)
+k1_scan_kernel(int n, const int2* __restrict__ cnt, const int2* __restrict__ block_tot,
+               int* __restrict__ r_off, int* __restrict__ a_off, int cap_r, int cap_a,
+               uint32_t* __restrict__ status) {
+  __shared__ int2 wsum[SCAN_THREADS / 32];
+  __shared__ int2 sbase;
+  const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+  // base = sum of the totals of all earlier blocks (integer: order-free)
+  int br = 0, ba = 0;
+  for (int q = threadIdx.x; q < (int)blockIdx.x; q += SCAN_THREADS) {
+    int2 t = block_tot[q]; br += t.x; ba += t.y;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    br += __shfl_xor_sync(0xffffffffu, br, o);
+    ba += __shfl_xor_sync(0xffffffffu, ba, o);
+  }
+  if (lane == 0) wsum[warp] = make_int2(br, ba);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int2 t = make_int2(0, 0);
+    for (int w = 0; w < SCAN_THREADS / 32; ++w) { t.x += wsum[w].x; t.y += wsum[w].y; }
+    sbase = t;
+  }
+  __syncthreads();
+  int2 base = sbase;
+  __syncthreads();
+  // each thread owns SCAN_ITEMS consecutive atoms
+  int i0 = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_ITEMS;
+  int2 c[SCAN_ITEMS];
+  int tr = 0, ta = 0;
+#pragma unroll
+  for (int q = 0; q < SCAN_ITEMS; ++q) {
+    c[q] = (i0 + q < n) ? cnt[i0 + q] : make_int2(0, 0);
+    tr += c[q].x; ta += c[q].y;
+  }
+  int ir = tr, ia = ta;                      // inclusive warp scan of thread totals
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int xr = __shfl_up_sync(0xffffffffu, ir, o), xa = __shfl_up_sync(0xffffffffu, ia, o);
+    if ((int)lane >= o) { ir += xr; ia += xa; }
+  }
+  if (lane == 31) wsum[warp] = make_int2(ir, ia);
+  __syncthreads();
+  int wr = 0, wa = 0;
+  for (int w = 0; w < (int)warp; ++w) { wr += wsum[w].x; wa += wsum[w].y; }
+  int er = base.x + wr + ir - tr, ea = base.y + wa + ia - ta;   // exclusive prefix
+#pragma unroll
+  for (int q = 0; q < SCAN_ITEMS; ++q) {
+    if (i0 + q < n) { r_off[i0 + q] = er; a_off[i0 + q] = ea; }
+    er += c[q].x; ea += c[q].y;
+    if (i0 + q == n - 1) {
+      r_off[n] = er; a_off[n] = ea;
+      uint32_t bits = (er > cap_r ? ST_RADIAL_OVERFLOW : 0u) | (ea > cap_a ? ST_ANGULAR_OVERFLOW : 0u);
+      if (bits) atomicOr(status, bits);
+    }
+  }
+}
+
+// ---- cell list (systems > BRUTE_MAX atoms) ----------------------------------
+struct CellGrid {          // one per cell-list system, in device memory
+  float lo[3];             // bounding-box minimum
+  float inv_edge[3];       // 1 / cell edge per axis
+  int nc[3];               // cells per axis
+  int cell_base;           // first cell of this system in the pooled cell arrays
+  int n_cells;
+};
+
+constexpr int CELL_THREADS = 256;
+// 2^-10 of slack: binning round-off ((x-lo)*inv_edge carries ~nc*1.2e-7 of error) can never
+// put two atoms closer than the cutoff into non-adjacent cells; the predicate decides.
+constexpr float CELL_EDGE_MIN = 5.2f * (1.0f + 9.765625e-4f);
+
+// one CTA per cell-list system: bounding box -> grid; zero the cell counters
+__global__ void __launch_bounds__(CELL_THREADS)
+k1_cell_grid_kernel(const int* __restrict__ cell_sys, const int* __restrict__ sys_off,
+                    const int* __restrict__ cell_cap_base, const float4* __restrict__ pos,
+                    CellGrid* __restrict__ grids, int* __restrict__ cell_count,
+                    uint32_t* __restrict__ status) {
+  __shared__ float smin[3][CELL_THREADS / 32], smax[3][CELL_THREADS / 32];
+  __shared__ CellGrid g;
+  int cs = blockIdx.x, sid = cell_sys[cs];
+  int b = sys_off[sid], e = sys_off[sid + 1];
+  float lo[3] = {3e38f, 3e38f, 3e38f}, hi[3] = {-3e38f, -3e38f, -3e38f};
+  for (int i = b + threadIdx.x; i < e; i += CELL_THREADS) {
+    float4 p = pos[i];
+    lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+    lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+    lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+  }
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+      hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+    }
+    if (lane_id() == 0) { smin[d][threadIdx.x >> 5] = lo[d]; smax[d][threadIdx.x >> 5] = hi[d]; }
+  }
+  __syncthreads();
+  int cap_cells = cell_cap_base[cs + 1] - cell_cap_base[cs] - 1;   // one extra slot: cell_start[n_cells]
+  if (threadIdx.x == 0) {
+    float ext[3];
+    for (int d = 0; d < 3; ++d) {
+      float l = smin[d][0], h = smax[d][0];
+      for (int w = 1; w < CELL_THREADS / 32; ++w) { l = fminf(l, smin[d][w]); h = fmaxf(h, smax[d][w]); }
+      g.lo[d] = l; ext[d] = h - l;
+    }
+    // cells of edge >= CELL_EDGE_MIN; if the grid would exceed its capacity
+    // (an expanding cluster), grow the edge -- larger cells are still correct.
+    float edge = CELL_EDGE_MIN;
+    for (int it = 0; it < 64; ++it) {
+      long long tot = 1;
+      for (int d = 0; d < 3; ++d) { g.nc[d] = max(1, (int)floorf(ext[d] / edge)); tot *= g.nc[d]; }
+      if (tot <= cap_cells) break;
+      edge *= 1.25f;
+    }
+    if ((long long)g.nc[0] * g.nc[1] * g.nc[2] > cap_cells) {
+      g.nc[0] = g.nc[1] = g.nc[2] = 1;
+      atomicOr(status, ST_CELL_OVERFLOW);
+    }
+    for (int d = 0; d < 3; ++d) {
+      float ce = fmaxf(ext[d] / (float)g.nc[d], edge);   // actual edge >= CELL_EDGE_MIN
+      g.inv_edge[d] = 1.0f / ce;
+    }
+    g.cell_base = cell_cap_base[cs];
+    g.n_cells = g.nc[0] * g.nc[1] * g.nc[2];
+    grids[cs] = g;
+  }
+  __syncthreads();
+  for (int c = threadIdx.x; c < g.n_cells; c += CELL_THREADS) cell_count[g.cell_base + c] = 0;
+}
+
+__device__ __forceinline__ int cell_coord(float x, float lo, float inv_edge, int nc) {
+  int c = (int)floorf((x - lo) * inv_edge);
+  return min(max(c, 0), nc - 1);
+}
+
+// per atom of a cell-list system: cell id + histogram
+__global__ void k1_cell_assign_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
+                                      const int* __restrict__ atom_cell_sys,
+                                      const float4* __restrict__ pos, const CellGrid* __restrict__ grids,
+                                      int* __restrict__ atom_cell, int* __restrict__ cell_count) {
+  int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= n_cell_atoms) return;
+  int i = cell_atom_list[q];
+  const CellGrid& g = grids[atom_cell_sys[q]];
+  float4 p = pos[i];
+  int cx = cell_coord(p.x, g.lo[0], g.inv_edge[0], g.nc[0]);
+  int cy = cell_coord(p.y, g.lo[1], g.inv_edge[1], g.nc[1]);
+  int cz = cell_coord(p.z, g.lo[2], g.inv_edge[2], g.nc[2]);
+  int c = g.cell_base + (cz * g.nc[1] + cy) * g.nc[0] + cx;
+  atom_cell[q] = c;
+  atomicAdd(&cell_count[c], 1);          // integer histogram: result is order-free
+}
+
+// one CTA per cell-list system: exclusive scan of its cell histogram -> cell_start
+// (pooled, relative to the system's first slot), and reset the fill cursors.
+__global__ void __launch_bounds__(CELL_THREADS)
+k1_cell_scan_kernel(const int* __restrict__ cell_sys, const int* __restrict__ cell_slot_base,
+                    const CellGrid* __restrict__ grids, const int* __restrict__ cell_count,
+                    int* __restrict__ cell_start, int* __restrict__ cell_cursor) {
+  __shared__ int wsum[CELL_THREADS / 32];
+  __shared__ int carry;
+  const CellGrid g = grids[blockIdx.x];
+  if (threadIdx.x == 0) carry = cell_slot_base[blockIdx.x];
+  __syncthreads();
+  for (int c0 = 0; c0 < g.n_cells; c0 += CELL_THREADS) {
+    int c = c0 + threadIdx.x;
+    int v = (c < g.n_cells) ? cell_count[g.cell_base + c] : 0;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int x = __shfl_up_sync(0xffffffffu, inc, o);
+      if ((int)lane_id() >= o) inc += x;
+    }
+    if (lane_id() == 31) wsum[threadIdx.x >> 5] = inc;
+    __syncthreads();
+    int w = 0;
+    for (int q = 0; q < (int)(threadIdx.x >> 5); ++q) w += wsum[q];
+    int excl = carry + w + inc - v;
+    if (c < g.n_cells) { cell_start[g.cell_base + c] = excl; cell_cursor[g.cell_base + c] = excl; }
+    __syncthreads();
+    if (threadIdx.x == CELL_THREADS - 1) carry = excl + v;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) cell_start[g.cell_base + g.n_cells] = carry;
+}
+
+// scatter atoms into their cells (slot order inside a cell is arbitrary: rows are
+// ordered by index afterwards, so the final lists do not depend on it)
+__global__ void k1_cell_fill_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
+                                    const int* __restrict__ atom_cell, int* __restrict__ cell_cursor,
+                                    int* __restrict__ cell_atoms) {
+  int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= n_cell_atoms) return;
+  int slot = atomicAdd(&cell_cursor[atom_cell[q]], 1);
+  cell_atoms[slot] = cell_atom_list[q];
+}
+
+// neighbour rows through the cell list: one warp per atom.
+// FILL=false counts; FILL=true writes the row unsorted, then orders it by
+// rank-by-count (all indices are distinct) and derives the angular row.
+constexpr int CELL_ROW_MAX = 512;        // longest radial row the in-warp ordering supports
+template <bool FILL>
+__global__ void __launch_bounds__(K1_WARPS * 32)
+k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
+                    const int* __restrict__ atom_cell_sys, const int* __restrict__ atom_cell,
+                    const float4* __restrict__ pos, const CellGrid* __restrict__ grids,
+                    const int* __restrict__ cell_start, const int* __restrict__ cell_atoms,
+                    int2* __restrict__ cnt, const int* __restrict__ r_off, const int* __restrict__ a_off,
+                    int* __restrict__ r_idx, int* __restrict__ a_idx, int cap_r, int cap_a,
+                    uint32_t* __restrict__ status) {
+  __shared__ int srow[K1_WARPS][CELL_ROW_MAX];
+  int q = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
+  if (q >= n_cell_atoms) return;
+  const uint32_t lane = lane_id(), lt = lanemask_lt();
+  int* row = srow[threadIdx.x >> 5];
+  int i = cell_atom_list[q];
+  const CellGrid g = grids[atom_cell_sys[q]];
+  float4 pi = pos[i];
+  int c = atom_cell[q] - g.cell_base;
+  int cx = c % g.nc[0], cy = (c / g.nc[0]) % g.nc[1], cz = c / (g.nc[0] * g.nc[1]);
+  int nr = 0, na = 0;
+  if (FILL && (r_off[i + 1] > cap_r || a_off[i + 1] > cap_a)) return;
+  for (int z = max(cz - 1, 0); z <= min(cz + 1, g.nc[2] - 1); ++z)
+    for (int y = max(cy - 1, 0); y <= min(cy + 1, g.nc[1] - 1); ++y) {
+      // cells x-1..x+1 of one (y,z) line are contiguous in the pooled array
+      int c0 = g.cell_base + (z * g.nc[1] + y) * g.nc[0] + max(cx - 1, 0);
+      int c1 = g.cell_base + (z * g.nc[1] + y) * g.nc[0] + min(cx + 1, g.nc[0] - 1);
+      int s0 = cell_start[c0], s1 = cell_start[c1 + 1];
+      for (int p0 = s0; p0 < s1; p0 += 32) {
+        int p = p0 + (int)lane;
+        int j = (p < s1) ? cell_atoms[p] : i;
+        float d2 = 1e30f;
+        if (j != i) {
+          float4 pj = pos[j];
+          d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+        }
+        uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
+        if (FILL) {
+          int slot = nr + __popc(mr & lt);
+          if (d2 < RC2_R && slot < CELL_ROW_MAX) row[slot] = j;
+        } else {
+          na += __popc(__ballot_sync(0xffffffffu, d2 < RC2_A));
+        }
+        nr += __popc(mr);
+      }
+    }
+  if (!FILL) {
+    if (lane == 0) cnt[i] = make_int2(nr, na);
+    return;
+  }
+  if (nr > CELL_ROW_MAX) { if (lane == 0) atomicOr(status, ST_RADIAL_OVERFLOW); return; }
+  __syncwarp();
+  // order by index: rank = number of smaller entries (entries are distinct)
+  int ro = r_off[i], ao = a_off[i];
+  for (int s = lane; s < nr; s += 32) {
+    int v = row[s], rank = 0;
+    for (int t = 0; t < nr; ++t) rank += (row[t] < v);
+    r_idx[ro + rank] = v;
+  }
+  __syncwarp();
+  // angular row: ordered compaction of the ordered radial row
+  for (int s0 = 0; s0 < nr; s0 += 32) {
+    int s = s0 + (int)lane;
+    float d2 = 1e30f;
+    int j = 0;
+    if (s < nr) {
+      j = r_idx[ro + s];
+      float4 pj = pos[j];
+      d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+    }
+    uint32_t ma = __ballot_sync(0xffffffffu, d2 < RC2_A);
+    if (d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
+    na += __popc(ma);
+  }
+}
+
+}  // namespace pfc

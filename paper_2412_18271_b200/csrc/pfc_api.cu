@@ -1,0 +1,514 @@
+// pfc_api.cu -- the C ABI of include/pfc.h: workspace carving, static element
+// grouping, weight repacking, kernel sequencing and CUDA-graph capture/replay.
+// Device memory and streams come from the caller (PyTorch); the library calls
+// no allocator.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/pfc.h"
+#include "k1_neighbors.cuh"
+#include "k2_aev.cuh"
+#include "k3_mlp_fp32.cuh"
+#include "k4_forces.cuh"
+#include "k5_verlet.cuh"
+
+using namespace pfc;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+// per-element weight block on the device (floats), forward then backward copies
+constexpr int OFF_W1T = 0;
+constexpr int OFF_B1 = OFF_W1T + D0 * D1;
+constexpr int OFF_W2T = OFF_B1 + D1;
+constexpr int OFF_B2 = OFF_W2T + D1 * D2;
+constexpr int OFF_W3T = OFF_B2 + D2;
+constexpr int OFF_B3 = OFF_W3T + D2 * D3;
+constexpr int OFF_W4 = OFF_B3 + D3;
+constexpr int OFF_B4 = OFF_W4 + D3;
+constexpr int OFF_W1 = OFF_B4 + 4;
+constexpr int OFF_W2 = OFF_W1 + D1 * D0;
+constexpr int OFF_W3 = OFF_W2 + D2 * D1;
+constexpr int DEV_W_PER_ELEM = OFF_W3 + D3 * D2;
+static_assert(DEV_W_PER_ELEM % 4 == 0 && OFF_W1 % 4 == 0 && OFF_W2T % 4 == 0 && OFF_W3T % 4 == 0, "16-byte rows");
+
+struct Carver {                 // bump allocator over the caller's workspace (or a dry run)
+  char* base;
+  size_t off = 0;
+  explicit Carver(void* b) : base((char*)b) {}
+  template <typename T>
+  T* take(size_t n) {
+    off = align_up(off);
+    T* p = base ? (T*)(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+};
+
+struct Sizes {
+  int n_atoms, n_systems, n_rows;
+  int cap_r, cap_a;
+  int n_scan_blocks;
+  int n_cell_sys, n_cell_atoms, cell_slots;   // cell_slots: pooled cell arrays (incl. +1 per system)
+};
+
+struct Buffers {
+  int *species, *sys_id, *sys_off, *row_of_atom;
+  unsigned char* sys_is_cell;
+  float4* xs;
+  int2 *cnt, *block_tot;
+  int *r_off, *a_off, *r_idx, *a_idx;
+  float *aev, *g, *e_row;
+  float4 *edge, *self, *xlo;
+  uint32_t* status;
+  StepParams* sp;
+  float* weights;
+  // cell list
+  int *cell_sys, *cell_cap_base, *cell_slot_base, *cell_atom_list, *atom_cell_sys, *atom_cell;
+  int *cell_count, *cell_start, *cell_cursor, *cell_atoms;
+  CellGrid* grids;
+  // internal state for pfc_run_host
+  float4 *h_pos, *h_vel, *h_frc;
+  float* h_E;
+};
+
+size_t carve(const Sizes& s, void* base, Buffers* b) {
+  Carver c(base);
+  Buffers t;
+  const size_t N = (size_t)s.n_atoms;
+  t.species = c.take<int>(N);
+  t.sys_id = c.take<int>(N);
+  t.sys_off = c.take<int>((size_t)s.n_systems + 1);
+  t.row_of_atom = c.take<int>(N);
+  t.sys_is_cell = c.take<unsigned char>((size_t)s.n_systems);
+  t.xs = c.take<float4>(N);
+  t.cnt = c.take<int2>(N);
+  t.block_tot = c.take<int2>((size_t)s.n_scan_blocks);
+  t.r_off = c.take<int>(N + 1);
+  t.a_off = c.take<int>(N + 1);
+  t.r_idx = c.take<int>((size_t)s.cap_r);
+  t.a_idx = c.take<int>((size_t)s.cap_a);
+  t.aev = c.take<float>((size_t)s.n_rows * AEV_LEN);
+  t.g = c.take<float>((size_t)s.n_rows * AEV_LEN);
+  t.e_row = c.take<float>((size_t)s.n_rows);
+  t.edge = c.take<float4>((size_t)s.cap_r);
+  t.self = c.take<float4>(N);
+  t.xlo = c.take<float4>(N);
+  t.status = c.take<uint32_t>(64);
+  t.sp = c.take<StepParams>(1);
+  t.weights = c.take<float>((size_t)NSPEC * DEV_W_PER_ELEM);
+  t.cell_sys = c.take<int>((size_t)s.n_cell_sys + 1);
+  t.cell_cap_base = c.take<int>((size_t)s.n_cell_sys + 1);
+  t.cell_slot_base = c.take<int>((size_t)s.n_cell_sys + 1);
+  t.grids = c.take<CellGrid>((size_t)s.n_cell_sys + 1);
+  t.cell_atom_list = c.take<int>((size_t)s.n_cell_atoms + 1);
+  t.atom_cell_sys = c.take<int>((size_t)s.n_cell_atoms + 1);
+  t.atom_cell = c.take<int>((size_t)s.n_cell_atoms + 1);
+  t.cell_atoms = c.take<int>((size_t)s.n_cell_atoms + 1);
+  t.cell_count = c.take<int>((size_t)s.cell_slots + 1);
+  t.cell_start = c.take<int>((size_t)s.cell_slots + 1);
+  t.cell_cursor = c.take<int>((size_t)s.cell_slots + 1);
+  t.h_pos = c.take<float4>(N);
+  t.h_vel = c.take<float4>(N);
+  t.h_frc = c.take<float4>(N);
+  t.h_E = c.take<float>((size_t)s.n_systems);
+  if (b) *b = t;
+  return align_up(c.off);
+}
+
+inline int cells_for(int n_sys_atoms) { return n_sys_atoms + 64 + 1; }
+
+// worst case over all species / system layouts with these totals
+Sizes worst_case_sizes(int n_atoms, int n_systems) {
+  Sizes s{};
+  s.n_atoms = n_atoms; s.n_systems = n_systems;
+  s.n_rows = (n_atoms + ROW_PAD - 1) / ROW_PAD * ROW_PAD + NSPEC * ROW_PAD;
+  long long per_r = n_atoms - 1 < 128 ? n_atoms - 1 : 128;
+  long long per_a = n_atoms - 1 < 48 ? n_atoms - 1 : 48;
+  long long cr = (long long)n_atoms * (per_r > 1 ? per_r : 1), ca = (long long)n_atoms * (per_a > 1 ? per_a : 1);
+  s.cap_r = (int)(cr > 2000000000LL ? 2000000000LL : cr);
+  s.cap_a = (int)(ca > 2000000000LL ? 2000000000LL : ca);
+  s.n_scan_blocks = (n_atoms + SCAN_BLOCK - 1) / SCAN_BLOCK;
+  s.n_cell_sys = n_atoms / (BRUTE_MAX + 1) + 1;
+  if (s.n_cell_sys > n_systems) s.n_cell_sys = n_systems;
+  s.n_cell_atoms = n_atoms;
+  s.cell_slots = n_atoms + 65 * s.n_cell_sys;
+  return s;
+}
+
+}  // namespace
+
+struct pfc_ctx {
+  Sizes sz;
+  Buffers b;
+  MlpParams mlp;
+  int mlp_path;
+  int n_cell_sys, n_cell_atoms;
+  int launches_ef, launches_step;
+  // bound MD state
+  float4 *pos = nullptr, *vel = nullptr, *frc = nullptr;
+  float* E = nullptr;
+  cudaStream_t stream = nullptr, cap_stream = nullptr;
+  bool bound = false, forces_stale = true;
+  float cur_dt = -1.0f;
+  cudaGraphExec_t g_forces = nullptr, g_step = nullptr;
+  int launch_counter = 0;
+};
+
+namespace {
+
+#define LAUNCH(ctx, kernel, grid, block, smem, stream, ...)     \
+  do {                                                          \
+    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__); \
+    ++(ctx)->launch_counter;                                    \
+  } while (0)
+
+inline int cdiv(int a, int b) { return (a + b - 1) / b; }
+
+// K1..K4 + energy sum on `st`
+void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStream_t st) {
+  const Sizes& s = c->sz;
+  const Buffers& b = c->b;
+  const int N = s.n_atoms;
+  LAUNCH(c, k1_brute_kernel<false>, cdiv(N, K1_WARPS), K1_WARPS * 32, 0, st, N, pos, b.species, b.sys_id,
+         b.sys_off, b.sys_is_cell, b.xs, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
+  if (c->n_cell_sys > 0) {
+    const int nca = c->n_cell_atoms;
+    LAUNCH(c, k1_cell_grid_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.sys_off, b.cell_cap_base,
+           pos, b.grids, b.cell_count, b.status);
+    LAUNCH(c, k1_cell_assign_kernel, cdiv(nca, 256), 256, 0, st, nca, b.cell_atom_list, b.atom_cell_sys, pos,
+           b.grids, b.atom_cell, b.cell_count);
+    LAUNCH(c, k1_cell_scan_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.cell_slot_base, b.grids,
+           b.cell_count, b.cell_start, b.cell_cursor);
+    LAUNCH(c, k1_cell_fill_kernel, cdiv(nca, 256), 256, 0, st, nca, b.cell_atom_list, b.atom_cell,
+           b.cell_cursor, b.cell_atoms);
+    LAUNCH(c, k1_cell_rows_kernel<false>, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
+           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_atoms, b.cnt, b.r_off, b.a_off,
+           b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
+  }
+  if (s.n_scan_blocks > 1)
+    LAUNCH(c, k1_scan_totals_kernel, s.n_scan_blocks, SCAN_THREADS, 0, st, N, b.cnt, b.block_tot);
+  LAUNCH(c, k1_scan_kernel, s.n_scan_blocks, SCAN_THREADS, 0, st, N, b.cnt, b.block_tot, b.r_off, b.a_off,
+         s.cap_r, s.cap_a, b.status);
+  LAUNCH(c, k1_brute_kernel<true>, cdiv(N, K1_WARPS), K1_WARPS * 32, 0, st, N, pos, b.species, b.sys_id,
+         b.sys_off, b.sys_is_cell, b.xs, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
+  if (c->n_cell_sys > 0) {
+    const int nca = c->n_cell_atoms;
+    LAUNCH(c, k1_cell_rows_kernel<true>, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
+           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_atoms, b.cnt, b.r_off, b.a_off,
+           b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
+  }
+  LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.r_off, b.r_idx,
+         b.row_of_atom, b.aev, b.status);
+  LAUNCH(c, k3_mlp_fp32_kernel, s.n_rows / MLP_TM, MLP_THREADS, MLP_FP32_SMEM, st, c->mlp, b.aev, b.g, b.e_row);
+  LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.r_off, b.r_idx,
+         b.row_of_atom, b.g, b.edge, b.self);
+  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.r_off, b.r_idx, b.edge, b.self,
+         b.row_of_atom, b.e_row, F);
+  LAUNCH(c, k_energy_sum_kernel, s.n_systems, ESUM_THREADS, 0, st, b.sys_off, F, E, b.status);
+}
+
+template <int MODE>
+void enqueue_verlet(pfc_ctx* c, cudaStream_t st) {
+  LAUNCH(c, k5_verlet_kernel<MODE>, cdiv(c->sz.n_atoms, K5_THREADS), K5_THREADS, 0, st, c->sz.n_atoms, c->b.sp,
+         c->b.species, c->frc, c->pos, c->vel, c->b.xlo);
+}
+
+void drop_graphs(pfc_ctx* c) {
+  if (c->g_forces) cudaGraphExecDestroy(c->g_forces);
+  if (c->g_step) cudaGraphExecDestroy(c->g_step);
+  c->g_forces = c->g_step = nullptr;
+}
+
+// capture {optional fused Verlet kernel, forces} for the bound state
+int capture(pfc_ctx* c, bool with_verlet, cudaGraphExec_t* out, int* n_launches) {
+  // capture on a private stream (the caller's may be the legacy stream, which cannot
+  // capture); the instantiated graph is launched on the caller's stream.
+  cudaGraph_t graph = nullptr;
+  if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess)
+    return PFC_ERR_CAPTURE;
+  if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) return PFC_ERR_CAPTURE;
+  c->launch_counter = 0;
+  if (with_verlet) enqueue_verlet<2>(c, c->cap_stream);
+  enqueue_forces(c, c->pos, c->E, c->frc, c->cap_stream);
+  *n_launches = c->launch_counter;
+  cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+  if (e != cudaSuccess || !graph) { cudaGetLastError(); return PFC_ERR_CAPTURE; }
+  e = cudaGraphInstantiate(out, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) { cudaGetLastError(); return PFC_ERR_CAPTURE; }
+  return PFC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t pfc_workspace_bytes(int32_t n_atoms, int32_t n_systems) {
+  if (n_atoms < 1 || n_systems < 1 || n_systems > n_atoms) return 0;
+  Sizes s = worst_case_sizes(n_atoms, n_systems);
+  return carve(s, nullptr, nullptr);
+}
+
+int pfc_create(const pfc_desc_t* d, pfc_t** out) {
+  if (!d || !out || !d->species || !d->sys_offsets || !d->weights) return PFC_ERR_ARG;
+  if (d->n_atoms < 1 || d->n_systems < 1 || d->n_systems > d->n_atoms) return PFC_ERR_ARG;
+  if (d->mlp_path != PFC_MLP_FP32) return PFC_ERR_ARG;   // tensor-core path: see k3_mlp_tc (later)
+  const int N = d->n_atoms, NS = d->n_systems;
+  if (d->sys_offsets[0] != 0 || d->sys_offsets[NS] != N) return PFC_ERR_SPECIES;
+  for (int s = 0; s < NS; ++s)
+    if (d->sys_offsets[s + 1] <= d->sys_offsets[s]) return PFC_ERR_SPECIES;
+  int count[NSPEC] = {0, 0, 0, 0};
+  for (int i = 0; i < N; ++i) {
+    if (d->species[i] < 0 || d->species[i] >= NSPEC) return PFC_ERR_SPECIES;
+    ++count[d->species[i]];
+  }
+  if (!d->workspace || ((uintptr_t)d->workspace % ALIGN) != 0) return PFC_ERR_WORKSPACE;
+  if (d->workspace_bytes < pfc_workspace_bytes(N, NS)) return PFC_ERR_WORKSPACE;
+
+  pfc_ctx* c = new (std::nothrow) pfc_ctx();
+  if (!c) return PFC_ERR_ARG;
+  c->mlp_path = d->mlp_path;
+  c->sz = worst_case_sizes(N, NS);                      // capacities are the worst-case ones
+  // static element grouping: rows sorted by element, blocks padded to ROW_PAD
+  int row_start[NSPEC + 1];
+  row_start[0] = 0;
+  for (int e = 0; e < NSPEC; ++e) row_start[e + 1] = row_start[e] + (count[e] + ROW_PAD - 1) / ROW_PAD * ROW_PAD;
+  c->sz.n_rows = row_start[NSPEC];
+  std::vector<int> row_of_atom(N), sys_id(N);
+  {
+    int next[NSPEC];
+    for (int e = 0; e < NSPEC; ++e) next[e] = row_start[e];
+    for (int i = 0; i < N; ++i) row_of_atom[i] = next[d->species[i]]++;
+  }
+  // systems above BRUTE_MAX atoms go through the cell list
+  std::vector<unsigned char> is_cell(NS, 0);
+  std::vector<int> cell_sys, cell_cap_base(1, 0), cell_slot_base, cell_atom_list, atom_cell_sys;
+  for (int s = 0; s < NS; ++s) {
+    const int b0 = d->sys_offsets[s], e0 = d->sys_offsets[s + 1];
+    for (int i = b0; i < e0; ++i) sys_id[i] = s;
+    if (e0 - b0 > BRUTE_MAX) {
+      is_cell[s] = 1;
+      cell_slot_base.push_back((int)cell_atom_list.size());
+      for (int i = b0; i < e0; ++i) { cell_atom_list.push_back(i); atom_cell_sys.push_back((int)cell_sys.size()); }
+      cell_sys.push_back(s);
+      cell_cap_base.push_back(cell_cap_base.back() + cells_for(e0 - b0));
+    }
+  }
+  c->n_cell_sys = (int)cell_sys.size();
+  c->n_cell_atoms = (int)cell_atom_list.size();
+  carve(c->sz, d->workspace, &c->b);
+  Buffers& b = c->b;
+
+  // device weights: forward copies transposed to [k][n], backward copies as given
+  std::vector<float> w((size_t)NSPEC * DEV_W_PER_ELEM, 0.0f);
+  for (int e = 0; e < NSPEC; ++e) {
+    const float* src = d->weights + (size_t)e * W_PER_ELEM;
+    const float *W1 = src, *b1 = W1 + D1 * D0, *W2 = b1 + D1, *b2 = W2 + D2 * D1, *W3 = b2 + D2,
+                *b3 = W3 + D3 * D2, *W4 = b3 + D3, *b4 = W4 + D3;
+    float* dst = w.data() + (size_t)e * DEV_W_PER_ELEM;
+    for (int o = 0; o < D1; ++o) for (int k = 0; k < D0; ++k) dst[OFF_W1T + k * D1 + o] = W1[o * D0 + k];
+    for (int o = 0; o < D2; ++o) for (int k = 0; k < D1; ++k) dst[OFF_W2T + k * D2 + o] = W2[o * D1 + k];
+    for (int o = 0; o < D3; ++o) for (int k = 0; k < D2; ++k) dst[OFF_W3T + k * D3 + o] = W3[o * D2 + k];
+    memcpy(dst + OFF_B1, b1, sizeof(float) * D1);
+    memcpy(dst + OFF_B2, b2, sizeof(float) * D2);
+    memcpy(dst + OFF_B3, b3, sizeof(float) * D3);
+    memcpy(dst + OFF_W4, W4, sizeof(float) * D3);
+    dst[OFF_B4] = b4[0];
+    memcpy(dst + OFF_W1, W1, sizeof(float) * D1 * D0);
+    memcpy(dst + OFF_W2, W2, sizeof(float) * D2 * D1);
+    memcpy(dst + OFF_W3, W3, sizeof(float) * D3 * D2);
+    const float* dv = b.weights + (size_t)e * DEV_W_PER_ELEM;
+    c->mlp.w[e] = MlpWeights{dv + OFF_W1T, dv + OFF_B1, dv + OFF_W2T, dv + OFF_B2, dv + OFF_W3T, dv + OFF_B3,
+                             dv + OFF_W4,  dv + OFF_B4, dv + OFF_W1,  dv + OFF_W2, dv + OFF_W3};
+  }
+  for (int e = 0; e <= NSPEC; ++e) c->mlp.row_start[e] = row_start[e];
+
+  ModelTables tab;
+  {
+    // S2/S3: the constants are the fp32 roundings of the decimal values
+    const double shf_r[NSHF_R] = {0.9, 1.16875, 1.4375, 1.70625, 1.975, 2.24375, 2.5125, 2.78125,
+                                  3.05, 3.31875, 3.5875, 3.85625, 4.125, 4.39375, 4.6625, 4.93125};
+    const double shf_a[NSHF_A] = {0.9, 1.55, 2.2, 2.85};
+    const double shf_z[NSHF_Z] = {0.19634954, 0.58904862, 0.98174770, 1.37444679,
+                                  1.76714587, 2.15984495, 2.55254403, 2.94524311};
+    for (int k = 0; k < NSHF_R; ++k) tab.shf_r[k] = (float)shf_r[k];
+    for (int a = 0; a < NSHF_A; ++a) tab.shf_a[a] = (float)shf_a[a];
+    for (int z = 0; z < NSHF_Z; ++z) {
+      const double th = (double)(float)shf_z[z];
+      tab.cos_z[z] = (float)cos(th);
+      tab.sin_z[z] = (float)sin(th);
+    }
+    const double mass_default[NSPEC] = {1.008, 12.011, 14.007, 15.999};
+    for (int e = 0; e < NSPEC; ++e) {
+      const double m = d->masses_amu ? (double)d->masses_amu[e] : mass_default[e];
+      tab.inv_mass_acc[e] = (float)(9.648533216e-3 / m);
+    }
+  }
+  bool ok = true;
+  auto up = [&](void* dst, const void* src, size_t bytes) {
+    if (bytes && cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
+  };
+  if (cudaMemcpyToSymbol(c_tab, &tab, sizeof(tab)) != cudaSuccess) ok = false;
+  up(b.species, d->species, sizeof(int) * N);
+  up(b.sys_id, sys_id.data(), sizeof(int) * N);
+  up(b.sys_off, d->sys_offsets, sizeof(int) * (NS + 1));
+  up(b.row_of_atom, row_of_atom.data(), sizeof(int) * N);
+  up(b.sys_is_cell, is_cell.data(), NS);
+  up(b.weights, w.data(), sizeof(float) * w.size());
+  up(b.cell_sys, cell_sys.data(), sizeof(int) * cell_sys.size());
+  up(b.cell_cap_base, cell_cap_base.data(), sizeof(int) * cell_cap_base.size());
+  up(b.cell_slot_base, cell_slot_base.data(), sizeof(int) * cell_slot_base.size());
+  up(b.cell_atom_list, cell_atom_list.data(), sizeof(int) * cell_atom_list.size());
+  up(b.atom_cell_sys, atom_cell_sys.data(), sizeof(int) * atom_cell_sys.size());
+  // padded AEV rows are never written by K2: zero everything once
+  if (cudaMemset(b.aev, 0, sizeof(float) * (size_t)c->sz.n_rows * AEV_LEN) != cudaSuccess) ok = false;
+  if (cudaMemset(b.status, 0, 256) != cudaSuccess) ok = false;
+  if (cudaMemset(b.xlo, 0, sizeof(float4) * N) != cudaSuccess) ok = false;
+  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)MLP_FP32_SMEM) != cudaSuccess) ok = false;
+  if (cudaDeviceSynchronize() != cudaSuccess) ok = false;
+  if (!ok) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
+  // launch counts (static: depends only on the configuration)
+  c->launches_ef = 8 + (c->sz.n_scan_blocks > 1 ? 1 : 0) + (c->n_cell_sys > 0 ? 6 : 0);
+  c->launches_step = c->launches_ef + 1;
+  *out = c;
+  return PFC_OK;
+}
+
+int pfc_energy_forces(pfc_t* c, const float* pos, float* E, float* F, void* stream) {
+  if (!c || !pos || !E || !F) return PFC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  c->launch_counter = 0;
+  enqueue_forces(c, (const float4*)pos, E, (float4*)F, st);
+  if (!c->bound) c->stream = st;
+  return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_set_state(pfc_t* c, float* pos, float* vel, float* E, float* F, void* stream) {
+  if (!c || !pos || !vel || !E || !F) return PFC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const bool same = c->bound && c->pos == (float4*)pos && c->vel == (float4*)vel && c->E == E &&
+                    c->frc == (float4*)F;
+  if (!same) drop_graphs(c);                       // pointers are baked into the graphs
+  c->pos = (float4*)pos; c->vel = (float4*)vel; c->E = E; c->frc = (float4*)F;
+  c->stream = st;
+  c->bound = true;
+  c->forces_stale = true;
+  if (cudaMemsetAsync(c->b.xlo, 0, sizeof(float4) * c->sz.n_atoms, st) != cudaSuccess) return PFC_ERR_CUDA;
+  return PFC_OK;
+}
+
+int pfc_step(pfc_t* c, int32_t n_steps, float dt_fs) {
+  if (!c || n_steps < 0 || !(dt_fs > 0.0f)) return PFC_ERR_ARG;
+  if (!c->bound) return PFC_ERR_STATE;
+  cudaStream_t st = c->stream;
+  int rc;
+  if (!c->g_forces && (rc = capture(c, false, &c->g_forces, &c->launches_ef)) != PFC_OK) return rc;
+  if (!c->g_step && (rc = capture(c, true, &c->g_step, &c->launches_step)) != PFC_OK) return rc;
+  if (dt_fs != c->cur_dt) {
+    k5_set_params_kernel<<<1, 1, 0, st>>>(c->b.sp, dt_fs);
+    c->cur_dt = dt_fs;
+  }
+  if (c->forces_stale) {
+    if (cudaGraphLaunch(c->g_forces, st) != cudaSuccess) return PFC_ERR_CUDA;
+    c->forces_stale = false;
+  }
+  if (n_steps == 0) return PFC_OK;
+  // step 1: half kick + drift, forces.  steps 2..n: one graph each = fused
+  // (trailing half kick + leading half kick + drift), forces.  Then the last half kick.
+  enqueue_verlet<1>(c, st);
+  if (cudaGraphLaunch(c->g_forces, st) != cudaSuccess) return PFC_ERR_CUDA;
+  for (int s = 1; s < n_steps; ++s)
+    if (cudaGraphLaunch(c->g_step, st) != cudaSuccess) return PFC_ERR_CUDA;
+  enqueue_verlet<0>(c, st);
+  return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_run_host(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, float dt_fs, float* E_h, float* F_h,
+                 void* stream) {
+  if (!c || !pos_h || !vel_h || !E_h) return PFC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t nb = sizeof(float4) * (size_t)c->sz.n_atoms;
+  Buffers& b = c->b;
+  if (cudaMemcpyAsync(b.h_pos, pos_h, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if (cudaMemcpyAsync(b.h_vel, vel_h, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PFC_ERR_CUDA;
+  int rc = pfc_set_state(c, (float*)b.h_pos, (float*)b.h_vel, b.h_E, (float*)b.h_frc, stream);
+  if (rc != PFC_OK) return rc;
+  if ((rc = pfc_step(c, n_steps, dt_fs)) != PFC_OK) return rc;
+  if (cudaMemcpyAsync(pos_h, b.h_pos, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if (cudaMemcpyAsync(vel_h, b.h_vel, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if (F_h && cudaMemcpyAsync(F_h, b.h_frc, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if (cudaMemcpyAsync(E_h, b.h_E, sizeof(float) * c->sz.n_systems, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    return PFC_ERR_CUDA;
+  return cudaStreamSynchronize(st) == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_get_neighbors(pfc_t* c, const int32_t** r_off, const int32_t** r_idx, const int32_t** a_off,
+                      const int32_t** a_idx) {
+  if (!c) return PFC_ERR_ARG;
+  if (r_off) *r_off = c->b.r_off;
+  if (r_idx) *r_idx = c->b.r_idx;
+  if (a_off) *a_off = c->b.a_off;
+  if (a_idx) *a_idx = c->b.a_idx;
+  return PFC_OK;
+}
+
+int pfc_get_intermediates(pfc_t* c, const float** aev, const float** g, const int32_t** row_of_atom,
+                          int32_t* n_rows) {
+  if (!c) return PFC_ERR_ARG;
+  if (aev) *aev = c->b.aev;
+  if (g) *g = c->b.g;
+  if (row_of_atom) *row_of_atom = c->b.row_of_atom;
+  if (n_rows) *n_rows = c->sz.n_rows;
+  return PFC_OK;
+}
+
+int pfc_copy_to_host(const void* src, void* dst, size_t bytes) {
+  if (!src || !dst) return PFC_ERR_ARG;
+  return cudaMemcpy(dst, src, bytes, cudaMemcpyDeviceToHost) == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_status(pfc_t* c, uint32_t* bits) {
+  if (!c || !bits) return PFC_ERR_ARG;
+  if (cudaStreamSynchronize(c->stream) != cudaSuccess) return PFC_ERR_CUDA;
+  if (cudaMemcpy(bits, c->b.status, sizeof(uint32_t), cudaMemcpyDeviceToHost) != cudaSuccess) return PFC_ERR_CUDA;
+  return PFC_OK;
+}
+
+int pfc_launch_counts(pfc_t* c, int32_t* per_ef, int32_t* per_step) {
+  if (!c) return PFC_ERR_ARG;
+  if (per_ef) *per_ef = c->launches_ef;
+  if (per_step) *per_step = c->launches_step;
+  return PFC_OK;
+}
+
+int pfc_destroy(pfc_t* c) {
+  if (!c) return PFC_ERR_ARG;
+  drop_graphs(c);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  delete c;
+  return PFC_OK;
+}
+
+const char* pfc_error_string(int code) {
+  switch (code) {
+    case PFC_OK: return "ok";
+    case PFC_ERR_ARG: return "invalid argument";
+    case PFC_ERR_SPECIES: return "species outside 0..3 or malformed sys_offsets";
+    case PFC_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case PFC_ERR_CUDA: return "CUDA runtime error";
+    case PFC_ERR_CAPTURE: return "CUDA graph capture failed";
+    case PFC_ERR_STATE: return "pfc_step called before pfc_set_state";
+    default: return "unknown pfc error";
+  }
+}
+
+}  // extern "C"

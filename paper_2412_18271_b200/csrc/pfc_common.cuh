@@ -1,0 +1,86 @@
+// pfc_common.cuh -- model constants, device-side views and small helpers shared
+// by the pfc kernels (sm_100a).  Nothing here is shared with oracle/.
+//
+// Constants restate DESIGN.md "Model constants" (readings S2-S8): every model
+// constant is DEFINED as an fp32 value.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pfc {
+
+constexpr int NSPEC = 4;
+constexpr int NSHF_R = 16, NSHF_A = 4, NSHF_Z = 8, NPAIR = 10;
+constexpr int RAD_LEN = NSPEC * NSHF_R;            // 64
+constexpr int ANG_LEN = NPAIR * NSHF_A * NSHF_Z;   // 320
+constexpr int AEV_LEN = RAD_LEN + ANG_LEN;         // 384
+constexpr int D0 = AEV_LEN, D1 = 160, D2 = 128, D3 = 96;
+constexpr int W_PER_ELEM = D1 * D0 + D1 + D2 * D1 + D2 + D3 * D2 + D3 + D3 + 1;  // 94,689
+constexpr int ROW_PAD = 128;                       // element blocks padded to this many rows
+constexpr int MAX_ANG = 96;                        // PFC_MAX_ANGULAR
+constexpr int BRUTE_MAX = 2048;                    // systems above this use the cell list
+
+constexpr float RC2_R = 27.04f;                    // S6: 0x41d851ec (not 5.2f*5.2f)
+constexpr float RC2_A = 12.25f;
+constexpr float RC_R = 5.2f, RC_A = 3.5f;
+constexpr float ETA_R = 16.0f, ETA_A = 8.0f;
+constexpr float COS_SCALE = 0.95f;                 // S5
+constexpr float CELU_ALPHA = 0.1f;
+constexpr float PI_F = 3.14159265358979323846f;
+constexpr float LOG2E = 1.4426950408889634f;
+constexpr float ACC_F = 9.648533216e-3f;           // (A/fs^2) per (eV/A/amu)
+
+// device status bits (mirror include/pfc.h)
+constexpr uint32_t ST_RADIAL_OVERFLOW = 1u, ST_ANGULAR_OVERFLOW = 2u, ST_ANGULAR_ROW = 4u,
+                   ST_NONFINITE = 8u, ST_CELL_OVERFLOW = 16u;
+
+// Tables in constant memory, filled by pfc_create.
+struct ModelTables {
+  float shf_r[NSHF_R];   // 0.9 + k*0.26875           (S2)
+  float shf_a[NSHF_A];   // 0.9, 1.55, 2.2, 2.85      (S3)
+  float cos_z[NSHF_Z];   // cos(SHF_Z[b]),  SHF_Z[b] = (float)(pi/16 + b*pi/8)  (S3)
+  float sin_z[NSHF_Z];
+  float inv_mass_acc[NSPEC];  // ACC / m_s
+};
+__constant__ ModelTables c_tab;
+
+// Step parameters live in device memory so a captured graph is reusable for any dt.
+struct StepParams {
+  float dt;        // fs
+  float half_dt;   // dt/2
+};
+
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// O2 predicate: three subtractions, three products, two sums, each rounded to
+// nearest fp32, never contracted into FMAs (S6).
+__device__ __forceinline__ float dist2_rn(float ax, float ay, float az, float bx, float by, float bz) {
+  float dx = __fsub_rn(ax, bx), dy = __fsub_rn(ay, by), dz = __fsub_rn(az, bz);
+  float s = __fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy));
+  return __fadd_rn(s, __fmul_rn(dz, dz));
+}
+
+// species-pair block of the angular AEV: HH0 HC1 HN2 HO3 CC4 CN5 CO6 NN7 NO8 OO9
+__device__ __forceinline__ int pair_block(int za, int zb) {
+  int s1 = min(za, zb), s2 = max(za, zb);
+  return s1 * NSPEC - ((s1 * (s1 - 1)) >> 1) + (s2 - s1);
+}
+
+__device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
+__device__ __forceinline__ uint32_t lanemask_lt() {
+  uint32_t m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+__device__ __forceinline__ float warp_sum(float v) {   // fixed xor tree: deterministic
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+}  // namespace pfc

@@ -1,0 +1,248 @@
+"""ctypes binding of libpfc.so (include/pfc.h) -- argument marshalling only.
+
+Every step of the path (neighbour build, AEV, MLP, force chain rule,
+velocity-Verlet, graph replay) runs inside the library's CUDA kernels; this
+module owns no arithmetic.  PyTorch supplies device memory (the workspace and
+all state tensors) and the stream.  There is no CPU fallback: importing this
+module without a built libpfc.so, or creating a handle without a CUDA device,
+raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_float, c_int, c_int32, c_size_t, c_uint32, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpfc.so")
+
+AEV_LEN = 384
+N_WEIGHTS = 378756
+MLP_FP32 = 0
+MLP_TF32X3 = 1
+
+STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
+               4: "angular row longer than PFC_MAX_ANGULAR", 8: "non-finite energy",
+               16: "cell grid overflow"}
+
+EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_set_state", "pfc_step",
+           "pfc_run_host", "pfc_get_neighbors", "pfc_get_intermediates", "pfc_status",
+           "pfc_copy_to_host", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
+
+
+class PfcError(RuntimeError):
+    pass
+
+
+class _Desc(ctypes.Structure):
+    _fields_ = [("n_atoms", c_int32), ("n_systems", c_int32),
+                ("species", POINTER(c_int32)), ("sys_offsets", POINTER(c_int32)),
+                ("weights", POINTER(c_float)), ("masses_amu", POINTER(c_float)),
+                ("workspace", c_void_p), ("workspace_bytes", c_size_t),
+                ("mlp_path", c_int32)]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libpfc.so and declare the prototypes of include/pfc.h.  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise PfcError(f"{LIB_PATH} is missing: build it with `python -m paper_2412_18271_b200.build` "
+                       "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    pp_i32 = POINTER(POINTER(c_int32))
+    pp_f = POINTER(POINTER(c_float))
+    lib.pfc_workspace_bytes.argtypes = [c_int32, c_int32]
+    lib.pfc_workspace_bytes.restype = c_size_t
+    lib.pfc_create.argtypes = [POINTER(_Desc), POINTER(c_void_p)]
+    lib.pfc_energy_forces.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pfc_set_state.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pfc_step.argtypes = [c_void_p, c_int32, c_float]
+    lib.pfc_run_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p, c_void_p]
+    lib.pfc_get_neighbors.argtypes = [c_void_p, pp_i32, pp_i32, pp_i32, pp_i32]
+    lib.pfc_get_intermediates.argtypes = [c_void_p, pp_f, pp_f, pp_i32, POINTER(c_int32)]
+    lib.pfc_copy_to_host.argtypes = [c_void_p, c_void_p, c_size_t]
+    lib.pfc_status.argtypes = [c_void_p, POINTER(c_uint32)]
+    lib.pfc_launch_counts.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32)]
+    lib.pfc_destroy.argtypes = [c_void_p]
+    lib.pfc_error_string.argtypes = [c_int]
+    lib.pfc_error_string.restype = c_char_p
+    for name in EXPORTS:
+        if name not in ("pfc_workspace_bytes", "pfc_error_string"):
+            getattr(lib, name).restype = c_int
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise PfcError(f"{what}: {load_library().pfc_error_string(rc).decode()} ({rc})")
+
+
+def pfc_workspace_bytes(n_atoms: int, n_systems: int) -> int:
+    return int(load_library().pfc_workspace_bytes(int(n_atoms), int(n_systems)))
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+class Pfc:
+    """One handle = one set of systems + one potential (pfc_create .. pfc_destroy)."""
+
+    def __init__(self, species, sys_offsets, weights, masses_amu=None, mlp_path: int = MLP_FP32,
+                 device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise PfcError("pfc needs a CUDA device (sm_100a); there is no CPU fallback")
+        self._lib = load_library()
+        self.device = torch.device(device)
+        species = np.ascontiguousarray(species, dtype=np.int32)
+        sys_offsets = np.ascontiguousarray(sys_offsets, dtype=np.int32)
+        weights = np.ascontiguousarray(weights, dtype=np.float32)
+        if weights.shape != (N_WEIGHTS,):
+            raise PfcError(f"weights must have {N_WEIGHTS} floats")
+        self.n_atoms = int(species.shape[0])
+        self.n_systems = int(sys_offsets.shape[0] - 1)
+        nbytes = pfc_workspace_bytes(self.n_atoms, self.n_systems)
+        if nbytes == 0:
+            raise PfcError("bad sizes")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self.workspace.data_ptr() + 255) // 256 * 256
+            masses = None if masses_amu is None else np.ascontiguousarray(masses_amu, dtype=np.float32)
+            d = _Desc(self.n_atoms, self.n_systems,
+                      species.ctypes.data_as(POINTER(c_int32)), sys_offsets.ctypes.data_as(POINTER(c_int32)),
+                      weights.ctypes.data_as(POINTER(c_float)),
+                      None if masses is None else masses.ctypes.data_as(POINTER(c_float)),
+                      c_void_p(base), c_size_t(nbytes), int(mlp_path))
+            h = c_void_p()
+            _check(self._lib.pfc_create(byref(d), byref(h)), "pfc_create")
+        self._h = h
+        self._bound = None
+
+    # -- pfc_energy_forces ------------------------------------------------------
+    def energy_forces(self, pos, E=None, F=None, stream=None):
+        """pos: cuda float32 [N,4].  Returns (E [n_systems], F [N,4] = {Fx,Fy,Fz,e_i}); enqueues only."""
+        import torch
+        self._expect(pos, (self.n_atoms, 4))
+        if E is None:
+            E = torch.empty(self.n_systems, dtype=torch.float32, device=self.device)
+        if F is None:
+            F = torch.empty(self.n_atoms, 4, dtype=torch.float32, device=self.device)
+        self._expect(E, (self.n_systems,))
+        self._expect(F, (self.n_atoms, 4))
+        _check(self._lib.pfc_energy_forces(self._h, pos.data_ptr(), E.data_ptr(), F.data_ptr(),
+                                           _stream_ptr(stream)), "pfc_energy_forces")
+        return E, F
+
+    # -- pfc_set_state / pfc_step -------------------------------------------------
+    def set_state(self, pos, vel, E=None, F=None, stream=None):
+        import torch
+        self._expect(pos, (self.n_atoms, 4))
+        self._expect(vel, (self.n_atoms, 4))
+        if E is None:
+            E = torch.empty(self.n_systems, dtype=torch.float32, device=self.device)
+        if F is None:
+            F = torch.empty(self.n_atoms, 4, dtype=torch.float32, device=self.device)
+        self._expect(E, (self.n_systems,))
+        self._expect(F, (self.n_atoms, 4))
+        _check(self._lib.pfc_set_state(self._h, pos.data_ptr(), vel.data_ptr(), E.data_ptr(), F.data_ptr(),
+                                       _stream_ptr(stream)), "pfc_set_state")
+        self._bound = (pos, vel, E, F)          # keep the tensors alive while bound
+        return E, F
+
+    def step(self, n_steps: int, dt_fs: float = 0.5):
+        _check(self._lib.pfc_step(self._h, int(n_steps), float(dt_fs)), "pfc_step")
+
+    # -- pfc_run_host -------------------------------------------------------------
+    def run_host(self, pos_host, vel_host, n_steps: int, dt_fs: float, E_host, F_host=None, stream=None):
+        """Host tensors/arrays [N,4] float32 (pinned for async copies), updated in place."""
+        def ptr(a):
+            if a is None:
+                return None
+            return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+        _check(self._lib.pfc_run_host(self._h, ptr(pos_host), ptr(vel_host), int(n_steps), float(dt_fs),
+                                      ptr(E_host), ptr(F_host), _stream_ptr(stream)), "pfc_run_host")
+
+    # -- getters ------------------------------------------------------------------
+    def status(self) -> int:
+        bits = c_uint32()
+        _check(self._lib.pfc_status(self._h, byref(bits)), "pfc_status")
+        return int(bits.value)
+
+    def check_status(self) -> None:
+        bits = self.status()
+        if bits:
+            raise PfcError("device status: " + ", ".join(v for k, v in STATUS_BITS.items() if bits & k))
+
+    def launch_counts(self):
+        a, b = c_int32(), c_int32()
+        _check(self._lib.pfc_launch_counts(self._h, byref(a), byref(b)), "pfc_launch_counts")
+        return int(a.value), int(b.value)
+
+    def neighbors(self):
+        """Copies the CSR lists of the last evaluation to host numpy arrays (synchronises)."""
+        import torch
+        p = [POINTER(c_int32)() for _ in range(4)]
+        _check(self._lib.pfc_get_neighbors(self._h, *[byref(x) for x in p]), "pfc_get_neighbors")
+        torch.cuda.synchronize(self.device)
+        r_off = self._copy(p[0], self.n_atoms + 1, np.int32)
+        a_off = self._copy(p[2], self.n_atoms + 1, np.int32)
+        r_idx = self._copy(p[1], int(r_off[-1]), np.int32)
+        a_idx = self._copy(p[3], int(a_off[-1]), np.int32)
+        return r_off, r_idx, a_off, a_idx
+
+    def intermediates(self):
+        """(aev [N,384], g [N,384]) of the last evaluation in ATOM order (host copies)."""
+        import torch
+        pa, pg, pr, nr = POINTER(c_float)(), POINTER(c_float)(), POINTER(c_int32)(), c_int32()
+        _check(self._lib.pfc_get_intermediates(self._h, byref(pa), byref(pg), byref(pr), byref(nr)),
+               "pfc_get_intermediates")
+        torch.cuda.synchronize(self.device)
+        rows = self._copy(pr, self.n_atoms, np.int32)
+        aev = self._copy(pa, nr.value * AEV_LEN, np.float32).reshape(nr.value, AEV_LEN)
+        g = self._copy(pg, nr.value * AEV_LEN, np.float32).reshape(nr.value, AEV_LEN)
+        return aev[rows], g[rows]
+
+    def _copy(self, dev_ptr, n, dtype):
+        """device -> host copy of n items (marshalling only)."""
+        out = np.empty(n, dtype=dtype)
+        if n:
+            addr = ctypes.cast(dev_ptr, c_void_p).value
+            _check(self._lib.pfc_copy_to_host(addr, out.ctypes.data, n * out.itemsize), "pfc_copy_to_host")
+        return out
+
+    def _expect(self, t, shape):
+        import torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32
+                and tuple(t.shape) == tuple(shape) and t.is_contiguous()):
+            raise PfcError(f"expected a contiguous cuda float32 tensor of shape {shape}")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.pfc_destroy(self._h)
+            self._h = c_void_p()
+        self._bound = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def pack4(a3) -> np.ndarray:
+    """[N,3] -> [N,4] float32 with a zero .w lane (layout helper, no arithmetic)."""
+    a3 = np.asarray(a3, dtype=np.float32)
+    out = np.zeros((a3.shape[0], 4), dtype=np.float32)
+    out[:, :3] = a3
+    return out
