@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py -- atom-steps/s of the graph-captured MD step (energy + forces + velocity-Verlet)
+on seeded synthetic gas-phase workloads (BASELINE.json:configs), one B200 per rank.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl reference]
+
+A "step" is one MD step = one pass of the whole hot path (K1 neighbour build, K2 AEV,
+K3 MLP fwd+bwd, K4 force chain rule + gather, energy sum, K5 velocity-Verlet) over the
+whole batch, replayed from one CUDA graph.  Prints ONE JSON line (rank 0).
+Multi-GPU: replicas only -- every rank runs the same workload on its own
+GPU, no data-path collective; value = atoms * steps * N / max-over-ranks time ("weak").
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same
+workload; it is a deliberately slow baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2412_18271_b200 import workloads as W  # noqa: E402
+
+METRIC = "atom_steps_per_s"
+UNIT = "atom-steps/s"
+DT_FS = 0.5
+MLP_FLOPS_PER_ATOM = 4.0 * 94304                     # fwd + bwd, 94,304 MAC each, 2 flop per MAC = 377,216
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.5: SMs x FP32 lanes x 2 x max SM clock
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt, self.proc = index, [], threading.Event(), None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([c.strip() for c in line.split(",")])
+                if self._stop_evt.is_set():
+                    break
+        except Exception:
+            pass
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.proc:
+            self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _oracle_steps_per_s(wl, weights, n_steps):
+    import oracle
+    t = time.perf_counter()
+    oracle.step(wl.pos, wl.vel, wl.species, wl.sys_offsets, weights, DT_FS, n_steps, cell=wl.n_atoms > 4096)
+    dt = time.perf_counter() - t
+    # oracle.step evaluates forces n_steps + 1 times (once at step 0)
+    return wl.n_atoms * (n_steps + 1) / dt, dt
+
+
+def _sample_workload(k, budget_atoms):
+    """A bounded sample of config k for the CPU legs: whole replicas / a smaller droplet."""
+    if k == 0:
+        return W.config0(), "config 0 whole (22 atoms)"
+    if k == 1:
+        n = max(1, min(256, budget_atoms // 22))
+        return W.config1(n_replicas=n), f"first {n} of 256 replicas of config 1"
+    if k == 2:
+        n = max(10, min(500, budget_atoms // 3))
+        return W.config2(n_mol=n), f"{n}-molecule droplet built by config 2's recipe"
+    if k == 3:
+        n = max(100, min(20000, budget_atoms))
+        return W.config3(n_atoms=n), f"{n}-atom droplet built by config 3's recipe"
+    n = max(1, min(4096, budget_atoms // 56))
+    return W.config4(n_replicas=n), f"first {n} of 4096 replicas of config 4"
+
+
+def run_reference(args):
+    """The oracle as it stands on the host cores; each step = one oracle MD step on a bounded sample."""
+    import oracle
+    weights = W.make_weights()
+    cores = oracle.num_threads()
+    probe, _ = _sample_workload(args.config, 2000)
+    rate, _ = _oracle_steps_per_s(probe, weights, 2)               # atom-evals/s, calibration
+    budget_s = 90.0
+    atoms = int(rate * budget_s / max(1, args.steps + args.warmup + 1))
+    wl, what = _sample_workload(args.config, max(22, atoms))
+    if args.warmup:
+        _oracle_steps_per_s(wl, weights, args.warmup)
+    value, dt = _oracle_steps_per_s(wl, weights, args.steps)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / (args.steps + 1) * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {args.config}", "sample": what, "atoms_in_sample": wl.n_atoms,
+                   "dt_fs": DT_FS},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def _time_steps(torch, p, stream, n_steps):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        p.step(n_steps, DT_FS)
+        e1.record(stream)
+    stream.synchronize()
+    return e0.elapsed_time(e1) * 1e-3
+
+
+def run_pfc(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2412_18271_b200 import pfc
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device; there is no CPU fallback (use --impl reference)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    pfc.load_library()
+    weights = W.make_weights()
+    wl = W.make_config(args.config)
+    N = wl.n_atoms
+    stream = torch.cuda.Stream(device=dev)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=args.mlp, device=dev)
+    pos0, vel0 = pfc.pack4(wl.pos), pfc.pack4(wl.vel)
+    pos, vel = torch.from_numpy(pos0).to(dev), torch.from_numpy(vel0).to(dev)
+    with torch.cuda.stream(stream):
+        E, F = p.set_state(pos, vel, stream=stream)
+        p.step(args.warmup, DT_FS)                               # W untimed steps (includes graph capture)
+    stream.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.3)
+    barrier()
+    t = _time_steps(torch, p, stream, args.steps)                # EXACTLY K steps, device time
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    if world > 1:
+        tt = torch.tensor([t], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t = float(tt.item())
+    status = p.status()
+    _, launches_step = p.launch_counts()
+    value = world * N * args.steps / t
+
+    line = None
+    if rank == 0:
+        peaks, peak_src = _peaks()
+        # ---- per-stage device times (CUDA events on the launching stream), averaged ----
+        stage_ms = np.zeros(pfc.N_STAGES)
+        reps = 10
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                p.profile_stages(pos, E, F, stream=stream)
+            for _ in range(reps):
+                stage_ms += np.array(p.profile_stages(pos, E, F, stream=stream))
+        stage_ms /= reps
+        k3_s = stage_ms[2] * 1e-3
+        flops = MLP_FLOPS_PER_ATOM * N
+        if args.mlp == pfc.MLP_FP32:
+            roof = {"bound": "alu", "achieved": flops / k3_s / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and max SM clock)"}
+        else:
+            roof = {"bound": "tensor", "achieved": flops / k3_s / 1e12,
+                    "peak": 0.5 * peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                    "peak_source": f"{peak_src} bf16 sustained x 0.5 (tf32:bf16 nominal ratio); "
+                                   "achieved counts algorithmic flops once, the 3-term split issues 3x"}
+        roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": None, "kernel": "K3 MLP fwd+bwd",
+                     "kernel_ms": float(stage_ms[2]),
+                     "stage_ms": {n: float(v) for n, v in zip(pfc.STAGE_NAMES, stage_ms)},
+                     "stage_share": {n: float(v / stage_ms.sum()) for n, v in zip(pfc.STAGE_NAMES, stage_ms)}})
+
+        # ---- end to end through the C ABI with HOST buffers: H2D + 1 step + D2H per step ----
+        ph, vh = torch.from_numpy(pos0.copy()).pin_memory(), torch.from_numpy(vel0.copy()).pin_memory()
+        Eh = torch.empty(wl.n_systems, dtype=torch.float32).pin_memory()
+        p2 = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=args.mlp, device=dev)
+        e2e_steps = max(3, min(args.steps, 50))
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                p2.run_host(ph, vh, 1, DT_FS, Eh, stream=stream)
+            t0 = time.perf_counter()
+            for _ in range(e2e_steps):
+                p2.run_host(ph, vh, 1, DT_FS, Eh, stream=stream)     # synchronises inside
+            t_e2e = time.perf_counter() - t0
+        p2.close()
+        e2e = {"value": world * N * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": 2 * N * 16,
+               "d2h_bytes_per_step": 2 * N * 16 + 4 * wl.n_systems, "steps": e2e_steps,
+               "call": "pfc_run_host(n_steps=1) per step, pinned host pos/vel in, pos/vel/E out"}
+
+        # ---- the oracle on the host cores, bounded sample ----
+        import oracle
+        swl, what = _sample_workload(args.config, 14000)
+        n_cpu_steps = 4 if swl.n_atoms > 5000 else 20
+        cpu_v, cpu_t = _oracle_steps_per_s(swl, weights, n_cpu_steps)
+        cpu = {"value": cpu_v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{what}, {n_cpu_steps} steps ({cpu_t:.1f} s)"}
+
+        steps_per_s = args.steps / t
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "config_index": args.config, "atoms": N, "systems": wl.n_systems,
+                       "dt_fs": DT_FS, "mlp_path": "fp32_ffma" if args.mlp == 0 else "tf32x3_tcgen05",
+                       "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "l2": "per-step working set (aev + g + lists + edge) exceeds the 126 MB L2"
+                             if N * 3072 > 126e6 else "working set fits L2: neighbour/AEV/MLP buffers are "
+                             "rewritten every step, no flush"},
+            "ns_per_day_per_replica": steps_per_s * DT_FS * 1e-6 * 86400,
+            "ns_per_day_aggregate": steps_per_s * DT_FS * 1e-6 * 86400 * wl.n_systems * world,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches_step * args.steps,
+            "launches_per_step": launches_step, "device_status": status,
+            "roofline": roof, "cpu_baseline": cpu,
+        }
+        if args.all_configs:
+            others = {}
+            for k in range(5):
+                if k == args.config:
+                    continue
+                w2 = W.make_config(k)
+                q = pfc.Pfc(w2.species, w2.sys_offsets, weights, mlp_path=args.mlp, device=dev)
+                x2, v2 = torch.from_numpy(pfc.pack4(w2.pos)).to(dev), torch.from_numpy(pfc.pack4(w2.vel)).to(dev)
+                with torch.cuda.stream(stream):
+                    q.set_state(x2, v2, stream=stream)
+                    q.step(10, DT_FS)
+                stream.synchronize()
+                n2 = 100
+                t2 = _time_steps(torch, q, stream, n2)
+                others[w2.name] = {"atoms": w2.n_atoms, "ms_per_step": t2 / n2 * 1e3,
+                                   "atom_steps_per_s": w2.n_atoms * n2 / t2,
+                                   "ns_per_day_per_replica": n2 / t2 * DT_FS * 1e-6 * 86400,
+                                   "device_status": q.status()}
+                q.close()
+            line["other_configs"] = others
+    p.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=4, choices=range(5))
+    ap.add_argument("--impl", default="pfc", choices=["pfc", "reference"])
+    ap.add_argument("--mlp", type=int, default=0, help="0 = FP32 FFMA, 1 = tcgen05 TF32x3")
+    ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (100 steps each)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "pfc":
+        args.warmup = 3
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_reference(args)
+        return
+    run_pfc(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -101,6 +101,14 @@ int pfc_create(const pfc_desc_t *desc, pfc_t **out);
  * MLP forward/backward (K3), force chain rule + gather (K4), energy sum. */
 int pfc_energy_forces(pfc_t *ctx, const float *pos, float *E, float *F, void *stream);
 
+/* Measurement helper: the same kernel sequence as pfc_energy_forces with a CUDA
+ * event recorded on `stream` at every stage boundary; synchronises and returns
+ * the device time of each stage in milliseconds, ms HOST [PFC_N_STAGES]:
+ * 0 = K1 neighbour build, 1 = K2 AEV forward, 2 = K3 MLP forward+backward,
+ * 3 = K4a AEV backward, 4 = K4b force gather, 5 = per-system energy sum. */
+#define PFC_N_STAGES 6
+int pfc_profile_stages(pfc_t *ctx, const float *pos, float *E, float *F, void *stream, float *ms);
+
 /* Binds (does not copy) the MD state advanced by pfc_step: pos, vel DEVICE
  * [n_atoms] float4, updated in place; E DEVICE [n_systems]; F DEVICE [n_atoms]
  * float4 (forces/energies of the last completed step).  Resets the internal

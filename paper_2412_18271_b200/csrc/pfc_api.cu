@@ -173,7 +173,11 @@ namespace {
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 // K1..K4 + energy sum on `st`
-void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStream_t st) {
+// `ev` (optional): PFC_N_STAGES+1 events recorded at the stage boundaries K1|K2|K3|K4a|K4b|E-sum
+void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStream_t st,
+                    cudaEvent_t* ev = nullptr) {
+  auto mark = [&](int k) { if (ev) cudaEventRecord(ev[k], st); };
+  mark(0);
   const Sizes& s = c->sz;
   const Buffers& b = c->b;
   const int N = s.n_atoms;
@@ -205,14 +209,20 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
            b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_atoms, b.cnt, b.r_off, b.a_off,
            b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
   }
+  mark(1);
   LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.r_off, b.r_idx,
          b.row_of_atom, b.aev, b.status);
+  mark(2);
   LAUNCH(c, k3_mlp_fp32_kernel, s.n_rows / MLP_TM, MLP_THREADS, MLP_FP32_SMEM, st, c->mlp, b.aev, b.g, b.e_row);
+  mark(3);
   LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.r_off, b.r_idx,
          b.row_of_atom, b.g, b.edge, b.self);
+  mark(4);
   LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.r_off, b.r_idx, b.edge, b.self,
          b.row_of_atom, b.e_row, F);
+  mark(5);
   LAUNCH(c, k_energy_sum_kernel, s.n_systems, ESUM_THREADS, 0, st, b.sys_off, F, E, b.status);
+  mark(6);
 }
 
 template <int MODE>
@@ -390,6 +400,20 @@ int pfc_energy_forces(pfc_t* c, const float* pos, float* E, float* F, void* stre
   enqueue_forces(c, (const float4*)pos, E, (float4*)F, st);
   if (!c->bound) c->stream = st;
   return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_profile_stages(pfc_t* c, const float* pos, float* E, float* F, void* stream, float* ms) {
+  if (!c || !pos || !E || !F || !ms) return PFC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t ev[PFC_N_STAGES + 1];
+  for (int k = 0; k <= PFC_N_STAGES; ++k)
+    if (cudaEventCreate(&ev[k]) != cudaSuccess) return PFC_ERR_CUDA;
+  enqueue_forces(c, (const float4*)pos, E, (float4*)F, st, ev);
+  int rc = cudaStreamSynchronize(st) == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+  for (int k = 0; k < PFC_N_STAGES && rc == PFC_OK; ++k)
+    if (cudaEventElapsedTime(&ms[k], ev[k], ev[k + 1]) != cudaSuccess) rc = PFC_ERR_CUDA;
+  for (int k = 0; k <= PFC_N_STAGES; ++k) cudaEventDestroy(ev[k]);
+  return rc;
 }
 
 int pfc_set_state(pfc_t* c, float* pos, float* vel, float* E, float* F, void* stream) {

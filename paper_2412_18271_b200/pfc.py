@@ -27,7 +27,10 @@ STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
                4: "angular row longer than PFC_MAX_ANGULAR", 8: "non-finite energy",
                16: "cell grid overflow"}
 
-EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_set_state", "pfc_step",
+N_STAGES = 6
+STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum")
+
+EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_profile_stages", "pfc_set_state", "pfc_step",
            "pfc_run_host", "pfc_get_neighbors", "pfc_get_intermediates", "pfc_status",
            "pfc_copy_to_host", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
 
@@ -62,6 +65,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_workspace_bytes.restype = c_size_t
     lib.pfc_create.argtypes = [POINTER(_Desc), POINTER(c_void_p)]
     lib.pfc_energy_forces.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pfc_profile_stages.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_float)]
     lib.pfc_set_state.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.pfc_step.argtypes = [c_void_p, c_int32, c_float]
     lib.pfc_run_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p, c_void_p]
@@ -143,6 +147,13 @@ class Pfc:
         _check(self._lib.pfc_energy_forces(self._h, pos.data_ptr(), E.data_ptr(), F.data_ptr(),
                                            _stream_ptr(stream)), "pfc_energy_forces")
         return E, F
+
+    def profile_stages(self, pos, E, F, stream=None):
+        """Per-stage device times (ms) of one energy_forces pass; synchronises."""
+        ms = (c_float * N_STAGES)()
+        _check(self._lib.pfc_profile_stages(self._h, pos.data_ptr(), E.data_ptr(), F.data_ptr(),
+                                            _stream_ptr(stream), ms), "pfc_profile_stages")
+        return [float(x) for x in ms]
 
     # -- pfc_set_state / pfc_step -------------------------------------------------
     def set_state(self, pos, vel, E=None, F=None, stream=None):

@@ -1,0 +1,355 @@
+"""GPU parity: the CUDA path (through the C ABI, libpfc.so) against the fp64 oracle on
+the same seeded inputs.  Bars (BASELINE.json:north_star):
+  * neighbour lists bit-exact (int32 CSR arrays equal);
+  * per-system energy |dE| <= 1e-5 * max(|E_ref|, 1 eV)          (S14);
+  * forces max|dF| <= 1e-3 eV/A (FP32 path; we also hold a 5e-5 internal target);
+  * trajectories: RMSD <= 1e-4 A per system after 100 steps of 0.5 fs.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle                                                    # noqa: E402
+from paper_2412_18271_b200 import workloads as W                 # noqa: E402
+
+E_RTOL = 1e-5
+F_ATOL = 1e-3
+F_ATOL_INTERNAL = 5e-5
+RMSD_TOL = 1e-4
+VEL_TOL = 2e-5
+
+
+@pytest.fixture(scope="module")
+def pfc():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2412_18271_b200 import pfc as m
+    m.load_library()
+    return m
+
+
+def _cfg(k):
+    if k == 4:
+        return W.config4()
+    return W.make_config(k)
+
+
+_cache = {}
+
+
+def cfg(k):
+    if k not in _cache:
+        _cache[k] = _cfg(k)
+    return _cache[k]
+
+
+def _dev(pfc, a3):
+    return torch.from_numpy(pfc.pack4(a3)).cuda()
+
+
+def _rmsd_per_system(x, xref, off):
+    d2 = ((x - xref) ** 2).sum(1)
+    return np.array([np.sqrt(d2[off[s]:off[s + 1]].mean()) for s in range(len(off) - 1)])
+
+
+def _assert_lists_equal(got, ref):
+    for name, a, b in zip(("r_off", "r_idx", "a_off", "a_idx"), got, ref):
+        assert a.dtype == np.int32 and a.shape == b.shape, name
+        assert np.array_equal(a, b), f"{name} differs"
+
+
+def _check_energy_forces(E, F, ref, tight=True):
+    Eh = E.cpu().numpy().astype(np.float64)
+    Fh = F.cpu().numpy().astype(np.float64)
+    tol_e = E_RTOL * np.maximum(np.abs(ref["E"]), 1.0)
+    assert (np.abs(Eh - ref["E"]) <= tol_e).all(), float((np.abs(Eh - ref["E"]) / tol_e).max())
+    dF = np.abs(Fh[:, :3] - ref["F"]).max()
+    assert dF <= F_ATOL, dF
+    if tight:
+        assert dF <= F_ATOL_INTERNAL, dF
+    assert np.abs(Fh[:, 3] - ref["e"]).max() <= 1e-5
+    return dF
+
+
+# ---- step 0 on every config at full size: lists, E, F --------------------------------
+@pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
+def test_step0_lists_energy_forces_full_size(pfc, weights, k):
+    wl = cfg(k)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    E, F = p.energy_forces(_dev(pfc, wl.pos))
+    assert p.status() == 0
+    # the definition is the O(N^2) enumeration; config 3 (20,000 atoms) goes through the
+    # oracle's cell list, which test_oracle_pins pins to the enumeration (P7)
+    _assert_lists_equal(p.neighbors(), oracle.neighbors(wl.pos, wl.sys_offsets, cell=(k == 3)))
+    ref = oracle.energy_forces(wl.pos.astype(np.float64), wl.species, wl.sys_offsets, weights,
+                               cell=(k == 3), want_intermediates=True)
+    _check_energy_forces(E, F, ref)
+    aev, g = p.intermediates()
+    assert np.abs(aev - ref["aev"]).max() <= 1e-5
+    assert np.abs(g - ref["g"]).max() <= 2e-6
+    p.close()
+
+
+def test_config3_brute_force_enumeration_matches_cell_path(pfc, weights):
+    """K1's cell list against the O(N^2) definition directly, on a cut of config 3 that is
+    still above BRUTE_MAX (so the GPU uses cells) -- independent of the oracle's cell list."""
+    wl = W.config3(n_atoms=5000)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    p.energy_forces(_dev(pfc, wl.pos))
+    _assert_lists_equal(p.neighbors(), oracle.neighbors(wl.pos, wl.sys_offsets, cell=False))
+    p.close()
+
+
+# ---- 100-step trajectories -----------------------------------------------------------
+def _trajectory(pfc, weights, wl, n_steps, cell=False):
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+    E, F = p.set_state(pos, vel)
+    p.step(n_steps, wl.dt_fs)
+    torch.cuda.synchronize()
+    assert p.status() == 0
+    ref = oracle.step(wl.pos, wl.vel, wl.species, wl.sys_offsets, weights, wl.dt_fs, n_steps, cell=cell)
+    x = pos.cpu().numpy()[:, :3].astype(np.float64)
+    v = vel.cpu().numpy()[:, :3].astype(np.float64)
+    rmsd = _rmsd_per_system(x, ref["pos"], wl.sys_offsets)
+    assert rmsd.max() <= RMSD_TOL, rmsd.max()
+    # velocities: north_star states no bound; DESIGN.md "Tolerances" derives 2e-5 A/fs from the
+    # position bound (an error that reaches 1e-4 A within the 50 fs window with the observed
+    # e-folding time of >= 5 fs moves at <= 1e-4/5 A/fs); thermal H speed is 1.6e-2 A/fs.
+    assert np.abs(v - ref["vel"]).max() <= VEL_TOL, np.abs(v - ref["vel"]).max()
+    # synchronous state: F and E belong to the final positions
+    Fh = F.cpu().numpy().astype(np.float64)
+    assert np.abs(Fh[:, :3] - ref["F"]).max() <= F_ATOL
+    Eh = E.cpu().numpy().astype(np.float64)
+    assert (np.abs(Eh - ref["pe"][-1]) <= 10 * E_RTOL * np.maximum(np.abs(ref["pe"][-1]), 1.0)).all()
+    assert (pos.cpu().numpy()[:, 3] == 0).all() and (vel.cpu().numpy()[:, 3] == 0).all()   # .w untouched
+    p.close()
+    return rmsd.max()
+
+
+def test_trajectory_config0(pfc, weights):
+    _trajectory(pfc, weights, cfg(0), 100)
+
+
+def test_trajectory_config1_all_256_replicas(pfc, weights):
+    _trajectory(pfc, weights, cfg(1), 100)
+
+
+def test_trajectory_config2(pfc, weights):
+    _trajectory(pfc, weights, cfg(2), 100)
+
+
+def test_trajectory_config3_full_size(pfc, weights):
+    _trajectory(pfc, weights, cfg(3), 100, cell=True)
+
+
+def test_trajectory_config4_subset_of_64_replicas(pfc, weights):
+    """100 steps on the first 64 replicas of config 4 (the full 4,096 are covered at step 0)."""
+    _trajectory(pfc, weights, W.config4(n_replicas=64), 100)
+
+
+# ---- frame replay (Fig. 4): oracle frames through pfc_energy_forces -------
+@pytest.mark.parametrize("k", [0, 2])
+def test_frame_replay(pfc, weights, k):
+    wl = cfg(k)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    x, v = wl.pos.astype(np.float64), wl.vel.astype(np.float64)
+    done = 0
+    for frame in (10, 50, 100):
+        out = oracle.step(x, v, wl.species, wl.sys_offsets, weights, wl.dt_fs, frame - done)
+        x, v, done = out["pos"], out["vel"], frame
+        xf = x.astype(np.float32)                                # the frame as a PDB-like fp32 record
+        E, F = p.energy_forces(_dev(pfc, xf))
+        _assert_lists_equal(p.neighbors(), oracle.neighbors(xf, wl.sys_offsets))
+        ref = oracle.energy_forces(xf.astype(np.float64), wl.species, wl.sys_offsets, weights)
+        _check_energy_forces(E, F, ref)
+    assert p.status() == 0
+    p.close()
+
+
+# ---- determinism ------------------------------------------------------------------------
+def test_bitwise_determinism(pfc, weights):
+    wl = W.config4(n_replicas=48)
+    outs = []
+    for _ in range(2):
+        p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+        pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+        E, F = p.set_state(pos, vel)
+        p.step(25, 0.5)
+        torch.cuda.synchronize()
+        outs.append((pos.cpu().numpy().copy(), vel.cpu().numpy().copy(), E.cpu().numpy().copy(),
+                     F.cpu().numpy().copy()))
+        p.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
+def test_step_splits_are_equivalent(pfc, weights):
+    """pfc_step(60) == pfc_step(25) + pfc_step(35) bit for bit (the state at exit is synchronous)."""
+    wl = W.config1(n_replicas=8)
+    res = []
+    for parts in ((60,), (25, 35)):
+        p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+        pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+        p.set_state(pos, vel)
+        for n in parts:
+            p.step(n, 0.5)
+        torch.cuda.synchronize()
+        res.append(pos.cpu().numpy().copy())
+        p.close()
+    # the fused kick (dt*a) and two half kicks round differently: equal to fp32 rounding, not bitwise
+    assert np.abs(res[0] - res[1]).max() <= 2e-6
+
+
+# ---- host-buffer entry point ----------------------------------------------------------------
+def test_run_host_matches_device_path(pfc, weights):
+    wl = W.config1(n_replicas=4)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+    E, F = p.set_state(pos, vel)
+    p.step(10, 0.5)
+    torch.cuda.synchronize()
+    ph = torch.from_numpy(pfc.pack4(wl.pos)).pin_memory()
+    vh = torch.from_numpy(pfc.pack4(wl.vel)).pin_memory()
+    Eh = torch.empty(wl.n_systems, dtype=torch.float32).pin_memory()
+    Fh = torch.empty(wl.n_atoms, 4, dtype=torch.float32).pin_memory()
+    p2 = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    p2.run_host(ph, vh, 10, 0.5, Eh, Fh)
+    assert np.array_equal(ph.numpy(), pos.cpu().numpy())
+    assert np.array_equal(Eh.numpy(), E.cpu().numpy())
+    assert np.array_equal(Fh.numpy(), F.cpu().numpy())
+    p.close(); p2.close()
+
+
+# ---- edge and degenerate cases ------------------------------------------------------------
+def _eval(pfc, weights, pos, species, off):
+    p = pfc.Pfc(species, off, weights)
+    E, F = p.energy_forces(_dev(pfc, pos))
+    lists = p.neighbors()
+    st = p.status()
+    ref = oracle.energy_forces(np.asarray(pos, np.float64), species, off, weights)
+    p.close()
+    return E, F, lists, st, ref
+
+
+def test_isolated_atoms_and_pairs(pfc, weights):
+    """Systems of one atom (empty rows, AEV = 0, E = MLP(0), F = 0), pairs beyond and inside the
+    cutoffs, and a pair straddling each cutoff by one fp32 ulp of d2."""
+    pos = np.zeros((10, 3), np.float32)
+    species = np.array([0, 1, 2, 3, 0, 0, 1, 3, 0, 0], np.int32)
+    off = np.array([0, 1, 2, 3, 4, 6, 8, 10], np.int32)
+    pos[5] = [6.0, 0, 0]                      # H-H beyond both cutoffs
+    pos[7] = [0, 3.0, 0]                      # C-O inside both
+    pos[9] = [0, 0, 4.0]                      # H-H radial only
+    E, F, lists, st, ref = _eval(pfc, weights, pos, species, off)
+    assert st == 0
+    _assert_lists_equal(lists, oracle.neighbors(pos, off))
+    assert list(np.diff(lists[0])) == [0, 0, 0, 0, 0, 0, 1, 1, 1, 1]
+    assert list(np.diff(lists[2])) == [0, 0, 0, 0, 0, 0, 1, 1, 0, 0]
+    _check_energy_forces(E, F, ref)
+    assert np.abs(F.cpu().numpy()[:6, :3]).max() == 0.0
+
+
+def test_cutoff_boundary_is_the_fp32_predicate(pfc, weights):
+    """d2 == RC2 exactly is excluded, one ulp below is included (S6), for both cutoffs."""
+    rc2 = {"r": np.float32(27.04), "a": np.float32(12.25)}
+    rows = []
+    pos, off = [], [0]
+    for key in ("r", "a"):
+        for ulps in (-1, 0, 1):
+            target = np.nextafter(rc2[key], np.float32(np.inf if ulps > 0 else -np.inf)) if ulps else rc2[key]
+            # find an x whose fp32 square is exactly `target` if one exists, else nearest below/above
+            x = np.float32(np.sqrt(np.float64(target)))
+            pos += [[0, 0, 0], [float(x), 0, 0]]
+            off.append(off[-1] + 2)
+            rows.append((key, float(np.float32(x) * np.float32(x))))
+    pos = np.array(pos, np.float32)
+    species = np.zeros(len(pos), np.int32)
+    E, F, lists, st, ref = _eval(pfc, weights, pos, species, np.array(off, np.int32))
+    _assert_lists_equal(lists, oracle.neighbors(pos, np.array(off, np.int32)))
+    nr, na = np.diff(lists[0])[::2], np.diff(lists[2])[::2]
+    for (key, d2), r, a in zip(rows, nr, na):
+        assert r == int(np.float32(d2) < np.float32(27.04))
+        assert a == int(np.float32(d2) < np.float32(12.25))
+    _check_energy_forces(E, F, ref)
+
+
+def test_brute_force_to_cell_list_switch(pfc, weights):
+    """2,048 atoms -> brute force, 2,049 -> cell list; both bit-exact against the enumeration."""
+    for n in (2048, 2049):
+        wl = W.config3(n_atoms=n)
+        p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+        E, F = p.energy_forces(_dev(pfc, wl.pos))
+        n_launch, _ = p.launch_counts()
+        _assert_lists_equal(p.neighbors(), oracle.neighbors(wl.pos, wl.sys_offsets))
+        _check_energy_forces(E, F, oracle.energy_forces(wl.pos.astype(np.float64), wl.species,
+                                                        wl.sys_offsets, weights))
+        assert (n_launch > 10) == (n > 2048)
+        p.close()
+
+
+def test_mixed_batch_of_cell_and_brute_systems(pfc, weights):
+    """One handle holding a 2,500-atom cluster (cell list), small molecules and a 1-atom system."""
+    big = W.config3(n_atoms=2500)
+    small = W.config4(n_replicas=5)
+    pos = np.concatenate([small.pos[:40], big.pos, small.pos[40:], [[0, 0, 0]]]).astype(np.float32)
+    species = np.concatenate([small.species[:40], big.species, small.species[40:], [2]]).astype(np.int32)
+    # four systems: 40 small-molecule atoms | the cluster | the remaining small atoms | one atom
+    off = np.array([0, 40, 40 + 2500, 40 + 2500 + (small.n_atoms - 40), len(pos)], np.int32)
+    E, F, lists, st, ref = _eval(pfc, weights, pos, species, off)
+    assert st == 0
+    _assert_lists_equal(lists, oracle.neighbors(pos, off))
+    _check_energy_forces(E, F, ref, tight=False)
+
+
+def test_dense_cluster_sets_the_angular_row_status_bit(pfc, weights):
+    """More than PFC_MAX_ANGULAR atoms within 3.5 A of one atom: reported, not silently wrong."""
+    rng = np.random.Generator(np.random.PCG64(5))
+    pos = (rng.random((130, 3)) * 1.6).astype(np.float32)
+    species = np.zeros(130, np.int32)
+    p = pfc.Pfc(species, np.array([0, 130], np.int32), weights)
+    p.energy_forces(_dev(pfc, pos))
+    assert p.status() & 4
+    _assert_lists_equal(p.neighbors(), oracle.neighbors(pos, np.array([0, 130], np.int32)))
+    p.close()
+
+
+def test_bad_arguments_are_rejected(pfc, weights):
+    with pytest.raises(pfc.PfcError):
+        pfc.Pfc(np.array([0, 4], np.int32), np.array([0, 2], np.int32), weights)       # species 4
+    with pytest.raises(pfc.PfcError):
+        pfc.Pfc(np.array([0, 1], np.int32), np.array([0, 1, 1, 2], np.int32), weights)  # empty system
+    with pytest.raises(pfc.PfcError):
+        pfc.Pfc(np.array([0, 1], np.int32), np.array([0, 2], np.int32), weights[:-1])
+    p = pfc.Pfc(np.array([0, 1], np.int32), np.array([0, 2], np.int32), weights)
+    with pytest.raises(pfc.PfcError):
+        p.step(1, 0.5)                                                                    # not bound
+    with pytest.raises(pfc.PfcError):
+        p.energy_forces(torch.zeros(3, 4, device="cuda"))
+    p.close()
+
+
+def test_nve_energy_conservation_on_gpu(pfc, weights):
+    """PAPER.md:75 (Fig. 2): the Hamiltonian is flat over 100 NVE steps.  Here: |H(t)-H(0)| stays
+    within 5e-4 eV for config 0 at dt = 0.5 fs, and the GPU H(t) tracks the oracle's."""
+    wl = cfg(0)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+    E, F = p.set_state(pos, vel)
+    m = W.MASSES_AMU[wl.species]
+    H = []
+    for _ in range(101):
+        p.step(1 if H else 0, 0.5)             # step(0) only evaluates E, F at the bound state
+        torch.cuda.synchronize()
+        v = vel.cpu().numpy()[:, :3].astype(np.float64)
+        ke = (0.5 * m[:, None] * v * v).sum() / W.ACC
+        H.append(float(E.cpu().numpy()[0]) + ke)
+    ref = oracle.step(wl.pos, wl.vel, wl.species, wl.sys_offsets, weights, 0.5, 100)
+    Href = ref["pe"][:, 0] + ref["ke"][:, 0]
+    H = np.array(H)
+    assert np.abs(H - H[0]).max() < 5e-4
+    assert np.abs(H - Href).max() < 2e-5
+    p.close()
