@@ -133,6 +133,9 @@ int pfc_run_host(pfc_t *ctx, float *pos_host, float *vel_host, int32_t n_steps, 
  * index (O2/S7). */
 int pfc_get_neighbors(pfc_t *ctx, const int32_t **r_off, const int32_t **r_idx,
                       const int32_t **a_off, const int32_t **a_idx);
+/* Entries r_idx / a_idx can hold; when r_off[n_atoms] (a_off[n_atoms]) exceeds it the overflow
+ * status bit is set and the rows past the capacity are not written. */
+int pfc_get_capacities(pfc_t *ctx, int32_t *cap_r, int32_t *cap_a);
 /* aev, g: [n_rows][384] in element-sorted padded row order; row_of_atom
  * DEVICE [n_atoms] gives each atom's row. */
 int pfc_get_intermediates(pfc_t *ctx, const float **aev, const float **g,

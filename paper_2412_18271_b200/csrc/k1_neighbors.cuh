@@ -23,14 +23,17 @@ constexpr int SCAN_THREADS = 256, SCAN_ITEMS = 8, SCAN_BLOCK = SCAN_THREADS * SC
 
 // ---- brute force -----------------------------------------------------------
 // FILL=false: counts -> cnt[i] = {radial, angular}; also writes the packed copy
-//             xs[i] = {x, y, z, bitcast(species)} every later kernel reads.
+//             xs[i] = {x, y, z, bitcast(species)} every later kernel reads, and xsl[i], the low
+//             words of the positions (S15): the list predicate sees only the fp32 positions,
+//             the AEV geometry sees the two-float difference.
 // FILL=true : writes r_idx / a_idx rows at r_off[i] / a_off[i].
 template <bool FILL>
 __global__ void __launch_bounds__(K1_WARPS * 32)
 k1_brute_kernel(int n_atoms, const float4* __restrict__ pos, const int* __restrict__ species,
                 const int* __restrict__ sys_id, const int* __restrict__ sys_off,
                 const unsigned char* __restrict__ sys_is_cell,
-                float4* __restrict__ xs, int2* __restrict__ cnt,
+                const float4* __restrict__ xlo, float4* __restrict__ xs, float4* __restrict__ xsl,
+                int2* __restrict__ cnt,
                 const int* __restrict__ r_off, const int* __restrict__ a_off,
                 int* __restrict__ r_idx, int* __restrict__ a_idx, int cap_r, int cap_a) {
   int i = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
@@ -42,15 +45,19 @@ k1_brute_kernel(int n_atoms, const float4* __restrict__ pos, const int* __restri
     float4 o = pi;
     o.w = __int_as_float(species[i]);
     xs[i] = o;
+    // low words of the two-float positions (pfc_step state); zero for a plain pfc_energy_forces call
+    xsl[i] = xlo ? xlo[i] : make_float4(0.f, 0.f, 0.f, 0.f);
   }
   if (sys_is_cell[sid]) return;          // handled by the cell-list kernels
   int b = sys_off[sid], e = sys_off[sid + 1];
   int nr = 0, na = 0;
   int ro = 0, ao = 0;
+  bool fit_r = true, fit_a = true;
   if (FILL) {
     ro = r_off[i]; ao = a_off[i];
     // capacity overflow was flagged by the scan; never write out of bounds
-    if (r_off[i + 1] > cap_r || a_off[i + 1] > cap_a) return;
+    fit_r = r_off[i + 1] <= cap_r; fit_a = a_off[i + 1] <= cap_a;
+    if (!fit_r && !fit_a) return;
   }
   for (int j0 = b; j0 < e; j0 += 32) {
     int j = j0 + (int)lane;
@@ -64,8 +71,8 @@ k1_brute_kernel(int n_atoms, const float4* __restrict__ pos, const int* __restri
     uint32_t ma = __ballot_sync(0xffffffffu, d2 < RC2_A);
     if (FILL) {
       uint32_t lt = lanemask_lt();
-      if (d2 < RC2_R) r_idx[ro + nr + __popc(mr & lt)] = j;
-      if (d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
+      if (fit_r && d2 < RC2_R) r_idx[ro + nr + __popc(mr & lt)] = j;
+      if (fit_a && d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
     }
     nr += __popc(mr);
     na += __popc(ma);
@@ -321,7 +328,8 @@ k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
   int c = atom_cell[q] - g.cell_base;
   int cx = c % g.nc[0], cy = (c / g.nc[0]) % g.nc[1], cz = c / (g.nc[0] * g.nc[1]);
   int nr = 0, na = 0;
-  if (FILL && (r_off[i + 1] > cap_r || a_off[i + 1] > cap_a)) return;
+  if (FILL && r_off[i + 1] > cap_r) return;
+  const bool fit_a = !FILL || a_off[i + 1] <= cap_a;
   for (int z = max(cz - 1, 0); z <= min(cz + 1, g.nc[2] - 1); ++z)
     for (int y = max(cy - 1, 0); y <= min(cy + 1, g.nc[1] - 1); ++y) {
       // cells x-1..x+1 of one (y,z) line are contiguous in the pooled array
@@ -371,7 +379,7 @@ k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
       d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
     }
     uint32_t ma = __ballot_sync(0xffffffffu, d2 < RC2_A);
-    if (d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
+    if (fit_a && d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
     na += __popc(ma);
   }
 }

@@ -46,8 +46,9 @@ __device__ __forceinline__ void tri_decode(int t, int m, int& j, int& k) {
 }
 
 __global__ void __launch_bounds__(AEV_WARPS * 32)
-k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const int* __restrict__ r_off,
-                  const int* __restrict__ r_idx, const int* __restrict__ row_of_atom,
+k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __restrict__ xsl,
+                  const int* __restrict__ r_off,
+                  const int* __restrict__ r_idx, int cap_r, const int* __restrict__ row_of_atom,
                   float* __restrict__ aev, uint32_t* __restrict__ status) {
   __shared__ AevFwdSmem sm[AEV_WARPS];
   const int warp = threadIdx.x >> 5;
@@ -56,8 +57,9 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const int* __restr
   AevFwdSmem& S = sm[warp];
   const uint32_t lane = lane_id(), lt = lanemask_lt();
   for (int c = lane; c < AEV_LEN; c += 32) S.out[c] = 0.0f;
-  const float4 xi = xs[i];
-  const int rb = r_off[i], re = r_off[i + 1];
+  const float4 xi = xs[i], li = xsl[i];
+  const int rb = r_off[i];
+  const int re = r_off[i + 1] <= cap_r ? r_off[i + 1] : rb;   // capacity overflow (flagged by K1): row unwritten
   int m = 0;
   float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
   const int half = lane >> 4;
@@ -73,7 +75,10 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const int* __restr
       dx = __fsub_rn(xj.x, xi.x); dy = __fsub_rn(xj.y, xi.y); dz = __fsub_rn(xj.z, xi.z);
       // identical value to K1's predicate (squares do not see the sign)
       const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
-      r = sqrtf(d2);
+      // geometry from the two-float positions (zero low words outside pfc_step)
+      const float4 lj = xsl[j];
+      dx += lj.x - li.x; dy += lj.y - li.y; dz += lj.z - li.z;
+      r = sqrtf(fmaf(dx, dx, fmaf(dy, dy, dz * dz)));
       fcr = 0.5f * __cosf((PI_F / RC_R) * r) + 0.5f;
       sp = __float_as_int(xj.w);
       isang = d2 < RC2_A;

@@ -33,8 +33,9 @@ struct AevBwdSmem {
 };
 
 __global__ void __launch_bounds__(AEV_WARPS * 32)
-k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const int* __restrict__ r_off,
-                   const int* __restrict__ r_idx, const int* __restrict__ row_of_atom,
+k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __restrict__ xsl,
+                   const int* __restrict__ r_off,
+                   const int* __restrict__ r_idx, int cap_r, const int* __restrict__ row_of_atom,
                    const float* __restrict__ g, float4* __restrict__ edge, float4* __restrict__ self) {
   __shared__ AevBwdSmem sm[AEV_WARPS];
   const int warp = threadIdx.x >> 5;
@@ -51,8 +52,9 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const int* __rest
     }
   }
   __syncwarp();
-  const float4 xi = xs[i];
-  const int rb = r_off[i], re = r_off[i + 1];
+  const float4 xi = xs[i], li = xsl[i];
+  const int rb = r_off[i];
+  const int re = r_off[i + 1] <= cap_r ? r_off[i + 1] : rb;   // capacity overflow (flagged by K1): row unwritten
   int m = 0;
   float sx = 0.f, sy = 0.f, sz = 0.f;            // this lane's share of self[i]
   for (int c0 = rb; c0 < re; c0 += 32) {
@@ -63,9 +65,11 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const int* __rest
     if (e < re) {
       const int j = r_idx[e];
       const float4 xj = xs[j];
-      const float dx = __fsub_rn(xj.x, xi.x), dy = __fsub_rn(xj.y, xi.y), dz = __fsub_rn(xj.z, xi.z);
+      float dx = __fsub_rn(xj.x, xi.x), dy = __fsub_rn(xj.y, xi.y), dz = __fsub_rn(xj.z, xi.z);
       const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
-      r = sqrtf(d2);
+      const float4 lj = xsl[j];                  // same two-float geometry as K2
+      dx += lj.x - li.x; dy += lj.y - li.y; dz += lj.z - li.z;
+      r = sqrtf(fmaf(dx, dx, fmaf(dy, dy, dz * dz)));
       const float rinv = 1.0f / r;
       ux = dx * rinv; uy = dy * rinv; uz = dz * rinv;
       sp = __float_as_int(xj.w);
@@ -195,14 +199,16 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const int* __rest
 // K4b: gather.  frc[a] = {F_a, e_a}.
 constexpr int K4B_WARPS = 8;
 __global__ void __launch_bounds__(K4B_WARPS * 32)
-k4b_gather_kernel(int n_atoms, const int* __restrict__ r_off, const int* __restrict__ r_idx,
+k4b_gather_kernel(int n_atoms, const int* __restrict__ r_off, const int* __restrict__ r_idx, int cap_r,
                   const float4* __restrict__ edge, const float4* __restrict__ self,
                   const int* __restrict__ row_of_atom, const float* __restrict__ e_row,
                   float4* __restrict__ frc) {
   const int a = blockIdx.x * K4B_WARPS + (threadIdx.x >> 5);
   if (a >= n_atoms) return;
   const uint32_t lane = lane_id();
-  const int rb = r_off[a], re = r_off[a + 1];
+  const int rb = r_off[a];
+  // on capacity overflow (flagged by K1) rows at the end are unwritten: outputs unspecified, no wild reads
+  const int re = r_off[n_atoms] <= cap_r ? r_off[a + 1] : rb;
   float gx = 0.f, gy = 0.f, gz = 0.f;
   for (int e = rb + (int)lane; e < re; e += 32) {
     const int j = r_idx[e];

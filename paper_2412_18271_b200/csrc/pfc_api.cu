@@ -62,7 +62,7 @@ struct Sizes {
 struct Buffers {
   int *species, *sys_id, *sys_off, *row_of_atom;
   unsigned char* sys_is_cell;
-  float4* xs;
+  float4 *xs, *xsl;
   int2 *cnt, *block_tot;
   int *r_off, *a_off, *r_idx, *a_idx;
   float *aev, *g, *e_row;
@@ -89,6 +89,7 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.row_of_atom = c.take<int>(N);
   t.sys_is_cell = c.take<unsigned char>((size_t)s.n_systems);
   t.xs = c.take<float4>(N);
+  t.xsl = c.take<float4>(N);
   t.cnt = c.take<int2>(N);
   t.block_tot = c.take<int2>((size_t)s.n_scan_blocks);
   t.r_off = c.take<int>(N + 1);
@@ -181,8 +182,10 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
   const Sizes& s = c->sz;
   const Buffers& b = c->b;
   const int N = s.n_atoms;
+  // the low position words belong to the bound MD state only
+  const float4* xlo = (c->bound && pos == c->pos) ? b.xlo : nullptr;
   LAUNCH(c, k1_brute_kernel<false>, cdiv(N, K1_WARPS), K1_WARPS * 32, 0, st, N, pos, b.species, b.sys_id,
-         b.sys_off, b.sys_is_cell, b.xs, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
+         b.sys_off, b.sys_is_cell, xlo, b.xs, b.xsl, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
   if (c->n_cell_sys > 0) {
     const int nca = c->n_cell_atoms;
     LAUNCH(c, k1_cell_grid_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.sys_off, b.cell_cap_base,
@@ -202,7 +205,7 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
   LAUNCH(c, k1_scan_kernel, s.n_scan_blocks, SCAN_THREADS, 0, st, N, b.cnt, b.block_tot, b.r_off, b.a_off,
          s.cap_r, s.cap_a, b.status);
   LAUNCH(c, k1_brute_kernel<true>, cdiv(N, K1_WARPS), K1_WARPS * 32, 0, st, N, pos, b.species, b.sys_id,
-         b.sys_off, b.sys_is_cell, b.xs, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
+         b.sys_off, b.sys_is_cell, xlo, b.xs, b.xsl, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
   if (c->n_cell_sys > 0) {
     const int nca = c->n_cell_atoms;
     LAUNCH(c, k1_cell_rows_kernel<true>, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
@@ -210,15 +213,15 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
            b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
   }
   mark(1);
-  LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.r_off, b.r_idx,
+  LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.r_off, b.r_idx, s.cap_r,
          b.row_of_atom, b.aev, b.status);
   mark(2);
   LAUNCH(c, k3_mlp_fp32_kernel, s.n_rows / MLP_TM, MLP_THREADS, MLP_FP32_SMEM, st, c->mlp, b.aev, b.g, b.e_row);
   mark(3);
-  LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.r_off, b.r_idx,
+  LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.r_off, b.r_idx, s.cap_r,
          b.row_of_atom, b.g, b.edge, b.self);
   mark(4);
-  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.r_off, b.r_idx, b.edge, b.self,
+  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.r_off, b.r_idx, s.cap_r, b.edge, b.self,
          b.row_of_atom, b.e_row, F);
   mark(5);
   LAUNCH(c, k_energy_sum_kernel, s.n_systems, ESUM_THREADS, 0, st, b.sys_off, F, E, b.status);
@@ -492,6 +495,13 @@ int pfc_get_intermediates(pfc_t* c, const float** aev, const float** g, const in
   if (g) *g = c->b.g;
   if (row_of_atom) *row_of_atom = c->b.row_of_atom;
   if (n_rows) *n_rows = c->sz.n_rows;
+  return PFC_OK;
+}
+
+int pfc_get_capacities(pfc_t* c, int32_t* cap_r, int32_t* cap_a) {
+  if (!c) return PFC_ERR_ARG;
+  if (cap_r) *cap_r = c->sz.cap_r;
+  if (cap_a) *cap_a = c->sz.cap_a;
   return PFC_OK;
 }
 

@@ -31,7 +31,7 @@ N_STAGES = 6
 STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum")
 
 EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_profile_stages", "pfc_set_state", "pfc_step",
-           "pfc_run_host", "pfc_get_neighbors", "pfc_get_intermediates", "pfc_status",
+           "pfc_run_host", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
            "pfc_copy_to_host", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
 
 
@@ -70,6 +70,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_step.argtypes = [c_void_p, c_int32, c_float]
     lib.pfc_run_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p, c_void_p]
     lib.pfc_get_neighbors.argtypes = [c_void_p, pp_i32, pp_i32, pp_i32, pp_i32]
+    lib.pfc_get_capacities.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32)]
     lib.pfc_get_intermediates.argtypes = [c_void_p, pp_f, pp_f, pp_i32, POINTER(c_int32)]
     lib.pfc_copy_to_host.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.pfc_status.argtypes = [c_void_p, POINTER(c_uint32)]
@@ -208,8 +209,10 @@ class Pfc:
         torch.cuda.synchronize(self.device)
         r_off = self._copy(p[0], self.n_atoms + 1, np.int32)
         a_off = self._copy(p[2], self.n_atoms + 1, np.int32)
-        r_idx = self._copy(p[1], int(r_off[-1]), np.int32)
-        a_idx = self._copy(p[3], int(a_off[-1]), np.int32)
+        cr, ca = c_int32(), c_int32()
+        _check(self._lib.pfc_get_capacities(self._h, byref(cr), byref(ca)), "pfc_get_capacities")
+        r_idx = self._copy(p[1], min(int(r_off[-1]), cr.value), np.int32)   # rows past the capacity
+        a_idx = self._copy(p[3], min(int(a_off[-1]), ca.value), np.int32)   # were never written
         return r_off, r_idx, a_off, a_idx
 
     def intermediates(self):
