@@ -66,6 +66,7 @@ extern "C" {
 
 #define PFC_MLP_FP32 0                  /* FP32 FFMA grouped MLP                 */
 #define PFC_MLP_TF32X3 1                /* tcgen05 kind::tf32, 3-term split      */
+#define PFC_MLP_TF32X1 2                /* tcgen05 plain TF32: tolerance evidence only (fails it) */
 
 typedef struct pfc_ctx pfc_t;           /* opaque; owned by the library          */
 
@@ -83,7 +84,7 @@ typedef struct {
   const float *masses_amu;       /* HOST [4] or NULL -> {1.008,12.011,14.007,15.999} */
   void *workspace;               /* DEVICE, 256-byte aligned, >= pfc_workspace_bytes() */
   size_t workspace_bytes;
-  int32_t mlp_path;              /* PFC_MLP_FP32 or PFC_MLP_TF32X3                 */
+  int32_t mlp_path;              /* PFC_MLP_FP32, PFC_MLP_TF32X3 (or PFC_MLP_TF32X1) */
 } pfc_desc_t;
 
 /* Bytes of device workspace pfc_create needs for these sizes (0 on bad args). */

@@ -14,6 +14,7 @@
 #include "k1_neighbors.cuh"
 #include "k2_aev.cuh"
 #include "k3_mlp_fp32.cuh"
+#include "k3_mlp_tc.cuh"
 #include "k4_forces.cuh"
 #include "k5_verlet.cuh"
 
@@ -70,6 +71,8 @@ struct Buffers {
   uint32_t* status;
   StepParams* sp;
   float* weights;
+  uint8_t* wtc;                 // tensor-core path: packed hi|lo swizzled weight chunks
+  float* bias_tc;
   // cell list
   int *cell_sys, *cell_cap_base, *cell_slot_base, *cell_atom_list, *atom_cell_sys, *atom_cell;
   int *cell_count, *cell_start, *cell_cursor, *cell_atoms;
@@ -105,6 +108,8 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.status = c.take<uint32_t>(64);
   t.sp = c.take<StepParams>(1);
   t.weights = c.take<float>((size_t)NSPEC * DEV_W_PER_ELEM);
+  t.wtc = c.take<uint8_t>((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
+  t.bias_tc = c.take<float>((size_t)NSPEC * TC_BIAS_LEN);
   t.cell_sys = c.take<int>((size_t)s.n_cell_sys + 1);
   t.cell_cap_base = c.take<int>((size_t)s.n_cell_sys + 1);
   t.cell_slot_base = c.take<int>((size_t)s.n_cell_sys + 1);
@@ -150,7 +155,9 @@ struct pfc_ctx {
   Sizes sz;
   Buffers b;
   MlpParams mlp;
+  TcParams tcp;
   int mlp_path;
+  int n_sms = 148;
   int n_cell_sys, n_cell_atoms;
   int launches_ef, launches_step;
   // bound MD state
@@ -216,7 +223,15 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
   LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.r_off, b.r_idx, s.cap_r,
          b.row_of_atom, b.aev, b.status);
   mark(2);
-  LAUNCH(c, k3_mlp_fp32_kernel, s.n_rows / MLP_TM, MLP_THREADS, MLP_FP32_SMEM, st, c->mlp, b.aev, b.g, b.e_row);
+  if (c->mlp_path == PFC_MLP_FP32) {
+    LAUNCH(c, k3_mlp_fp32_kernel, s.n_rows / MLP_TM, MLP_THREADS, MLP_FP32_SMEM, st, c->mlp, b.aev, b.g, b.e_row);
+  } else {
+    const int grid = c->tcp.n_tiles < c->n_sms ? c->tcp.n_tiles : c->n_sms;   // persistent: one CTA per SM
+    if (c->mlp_path == PFC_MLP_TF32X3)
+      LAUNCH(c, k3_mlp_tc_kernel<3>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, b.aev, b.g, b.e_row);
+    else
+      LAUNCH(c, k3_mlp_tc_kernel<1>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, b.aev, b.g, b.e_row);
+  }
   mark(3);
   LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.r_off, b.r_idx, s.cap_r,
          b.row_of_atom, b.g, b.edge, b.self);
@@ -273,7 +288,8 @@ size_t pfc_workspace_bytes(int32_t n_atoms, int32_t n_systems) {
 int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (!d || !out || !d->species || !d->sys_offsets || !d->weights) return PFC_ERR_ARG;
   if (d->n_atoms < 1 || d->n_systems < 1 || d->n_systems > d->n_atoms) return PFC_ERR_ARG;
-  if (d->mlp_path != PFC_MLP_FP32) return PFC_ERR_ARG;   // tensor-core path: see k3_mlp_tc (later)
+  if (d->mlp_path != PFC_MLP_FP32 && d->mlp_path != PFC_MLP_TF32X3 && d->mlp_path != PFC_MLP_TF32X1)
+    return PFC_ERR_ARG;
   const int N = d->n_atoms, NS = d->n_systems;
   if (d->sys_offsets[0] != 0 || d->sys_offsets[NS] != N) return PFC_ERR_SPECIES;
   for (int s = 0; s < NS; ++s)
@@ -344,6 +360,56 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   }
   for (int e = 0; e <= NSPEC; ++e) c->mlp.row_start[e] = row_start[e];
 
+  // tensor-core path: per element, the B operand of every phase chunk exactly as it sits in
+  // shared memory -- [N rows x 32 k] fp32, K-major, SWIZZLE_128B, hi block then lo block
+  std::vector<uint8_t> wtc((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
+  std::vector<float> bias_tc((size_t)NSPEC * TC_BIAS_LEN, 0.0f);
+  for (int e = 0; e < NSPEC; ++e) {
+    const float* src = d->weights + (size_t)e * W_PER_ELEM;
+    const float *W1 = src, *b1 = W1 + D1 * D0, *W2 = b1 + D1, *b2 = W2 + D2 * D1, *W3 = b2 + D2,
+                *b3 = W3 + D3 * D2, *W4 = b3 + D3, *b4 = W4 + D3;
+    // B[n][k] of phase p (see k3_mlp_tc.cuh): forward W[n][k]; backward W[k][n]
+    auto bval = [&](int p, int n, int k) -> float {
+      switch (p) {
+        case 0: return W1[n * D0 + k];
+        case 1: return W2[n * D1 + k];
+        case 2: return W3[n * D2 + k];
+        case 3: return W3[k * D2 + n];
+        case 4: return W2[k * D1 + n];
+        default: return W1[k * D0 + (p - 5) * TC_GN + n];
+      }
+    };
+    uint8_t* img = wtc.data() + (size_t)e * TC_W_BYTES_PER_ELEM;
+    for (int p = 0; p < TC_NPHASE; ++p) {
+      const int N = tc_phase_n(p), nk = tc_phase_nk(p);
+      for (int ch = 0; ch < nk; ++ch) {
+        uint8_t* chunk = img + tc_phase_off(p) + (size_t)ch * tc_chunk_bytes(p);
+        for (int n = 0; n < N; ++n)
+          for (int kk = 0; kk < 32; ++kk) {
+            const float v = bval(p, n, 32 * ch + kk);
+            uint32_t u;
+            memcpy(&u, &v, 4);
+            u = (u + 0x1000u) & 0xFFFFE000u;               // hi: rounded to tf32 precision
+            float hi;
+            memcpy(&hi, &u, 4);
+            const float lo = v - hi;                        // exact
+            memcpy(chunk + tc::sw128_off(n, kk), &hi, 4);
+            memcpy(chunk + (size_t)N * 128 + tc::sw128_off(n, kk), &lo, 4);
+          }
+      }
+    }
+    float* bt = bias_tc.data() + (size_t)e * TC_BIAS_LEN;
+    memcpy(bt + TC_BIAS_B1, b1, sizeof(float) * D1);
+    memcpy(bt + TC_BIAS_B2, b2, sizeof(float) * D2);
+    memcpy(bt + TC_BIAS_B3, b3, sizeof(float) * D3);
+    memcpy(bt + TC_BIAS_W4, W4, sizeof(float) * D3);
+    bt[TC_BIAS_B4] = b4[0];
+    c->tcp.bias[e] = c->b.bias_tc + (size_t)e * TC_BIAS_LEN;
+  }
+  c->tcp.wpack = c->b.wtc;
+  for (int e = 0; e <= NSPEC; ++e) c->tcp.row_start[e] = row_start[e];
+  c->tcp.n_tiles = c->sz.n_rows / TC_TM;
+
   ModelTables tab;
   {
     // S2/S3: the constants are the fp32 roundings of the decimal values
@@ -376,6 +442,8 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   up(b.row_of_atom, row_of_atom.data(), sizeof(int) * N);
   up(b.sys_is_cell, is_cell.data(), NS);
   up(b.weights, w.data(), sizeof(float) * w.size());
+  up(b.wtc, wtc.data(), wtc.size());
+  up(b.bias_tc, bias_tc.data(), sizeof(float) * bias_tc.size());
   up(b.cell_sys, cell_sys.data(), sizeof(int) * cell_sys.size());
   up(b.cell_cap_base, cell_cap_base.data(), sizeof(int) * cell_cap_base.size());
   up(b.cell_slot_base, cell_slot_base.data(), sizeof(int) * cell_slot_base.size());
@@ -387,6 +455,16 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (cudaMemset(b.xlo, 0, sizeof(float4) * N) != cudaSuccess) ok = false;
   if (cudaFuncSetAttribute(k3_mlp_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)MLP_FP32_SMEM) != cudaSuccess) ok = false;
+  if (cudaFuncSetAttribute(k3_mlp_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)TC_SMEM_BYTES) != cudaSuccess) ok = false;
+  if (cudaFuncSetAttribute(k3_mlp_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)TC_SMEM_BYTES) != cudaSuccess) ok = false;
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      c->n_sms = sms;
+  }
   if (cudaDeviceSynchronize() != cudaSuccess) ok = false;
   if (!ok) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
   // launch counts (static: depends only on the configuration)
