@@ -18,6 +18,11 @@
 //   warp 9     one elected thread issues tcgen05.mma and commits to the ring / phase barriers.
 // TMEM (512 columns) keeps the forward pre-activations z1,z2,z3 for the backward pass:
 //   z1 [0,160)  z2 [160,288)  z3 [288,384)  d2pre [384,512)  d1pre [160,320)  g-pass [384,512)
+// The accumulate step of the tensor core rounds toward zero (measured: the energy error of a
+// single-accumulator split correlates at -0.7 with the energy), one truncation per MMA, so the
+// small terms A_lo*B_hi + A_hi*B_lo of phases 0 and 2 go to an accumulator of their own
+// (S0 [352,512), S2 [384,480): free at that time) and are added on the CUDA cores; z1 is written
+// back (bias included) for the backward pass.
 #pragma once
 #include "pfc_common.cuh"
 #include "tc_ptx.cuh"
@@ -32,6 +37,7 @@ constexpr int TC_A_SLOT = 2 * TC_TM * 128;       // 32,768 B: hi | lo
 constexpr int TC_B_SLOT = 2 * D1 * 128;          // 40,960 B: widest N (160) hi | lo
 constexpr int TC_NPHASE = 8;
 constexpr int TC_GN = 128;                       // g is produced in 3 passes of 128 columns
+constexpr int TC_S0_COL = 352, TC_S2_COL = 384;  // small-term accumulators of phases 0 and 2
 
 // phase schedule: N, K chunks, D column, packed-weight byte offset (per element)
 __host__ __device__ constexpr int tc_phase_n(int p) {
@@ -70,10 +76,15 @@ struct TcParams {
 constexpr int TC_BIAS_B1 = 0, TC_BIAS_B2 = D1, TC_BIAS_B3 = D1 + D2, TC_BIAS_W4 = D1 + D2 + D3,
               TC_BIAS_B4 = D1 + D2 + D3 + D3, TC_BIAS_LEN = 484;
 
-// x -> (hi, lo): hi = x rounded to tf32 precision (10 mantissa bits), lo = x - hi (exact)
+// x -> (hi, lo): hi = x rounded to tf32 precision (10 mantissa bits); lo = x - hi (exact in fp32)
+// rounded to tf32 as well -- the tensor core would otherwise TRUNCATE it, a one-sided 2^-21 error
+// that adds up linearly over K and over the atoms of a system; rounded, it is 2^-22 and unbiased.
+__device__ __forceinline__ float tf32_round(float x) {
+  return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
+}
 __device__ __forceinline__ void tf32_split(float x, float& hi, float& lo) {
-  hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
-  lo = x - hi;
+  hi = tf32_round(x);
+  lo = tf32_round(x - hi);
 }
 
 // CELU(x) and CELU'(x), alpha = 0.1:  e = exp(min(x,0)/alpha)
@@ -134,6 +145,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
       return ringA + s * TC_A_SLOT;
     };
     auto publish = [&]() {
+      tc::tc_fence_before();                                   // this thread's tcgen05.ld precede the MMAs that overwrite
       tc::fence_proxy_async_smem();
       tc::mbar_arrive(&S.a_full[ia % TC_NA]);
       ++ia;
@@ -186,10 +198,22 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
       for (int c = 0; c < D1 / 32; ++c) {
         float z[16], h[16], d;
         tc::tmem_ld16(tlane + 0 + 32 * c + 16 * hf, z);
-        tc::tmem_ld_wait();
         const float* b = bias + TC_BIAS_B1 + 32 * c + 16 * hf;
+        if (N_TERMS == 3) {
+          float sm[16];
+          tc::tmem_ld16(tlane + TC_S0_COL + 32 * c + 16 * hf, sm);
+          tc::tmem_ld_wait();
 #pragma unroll
-        for (int k = 0; k < 16; ++k) celu_both(z[k] + __ldg(b + k), h[k], d);
+          for (int k = 0; k < 16; ++k) z[k] = (z[k] + sm[k]) + __ldg(b + k);
+        } else {
+          tc::tmem_ld_wait();
+#pragma unroll
+          for (int k = 0; k < 16; ++k) z[k] += __ldg(b + k);
+        }
+        tc::tmem_st16(tlane + 0 + 32 * c + 16 * hf, z);          // z1 + b1, kept for delta1
+#pragma unroll
+        for (int k = 0; k < 16; ++k) celu_both(z[k], h[k], d);
+        tc::tmem_st_wait();
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish();
@@ -214,7 +238,15 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
         for (int c = 0; c < D3 / 32; ++c) {
           float z[16], dl[16];
           tc::tmem_ld16(tlane + 288 + 32 * c + 16 * hf, z);
-          tc::tmem_ld_wait();
+          if (N_TERMS == 3) {
+            float sm[16];
+            tc::tmem_ld16(tlane + TC_S2_COL + 32 * c + 16 * hf, sm);
+            tc::tmem_ld_wait();
+#pragma unroll
+            for (int k = 0; k < 16; ++k) z[k] += sm[k];
+          } else {
+            tc::tmem_ld_wait();
+          }
           const float* b = bias + TC_BIAS_B3 + 32 * c + 16 * hf;
           const float* w4 = bias + TC_BIAS_W4 + 32 * c + 16 * hf;
 #pragma unroll
@@ -259,11 +291,10 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           tc::tmem_ld16(tlane + 0 + 32 * c + 16 * hf, z);
           tc::tmem_ld16(tlane + 160 + 32 * c + 16 * hf, p);
           tc::tmem_ld_wait();
-          const float* b = bias + TC_BIAS_B1 + 32 * c + 16 * hf;
 #pragma unroll
           for (int k = 0; k < 16; ++k) {
             float h, d;
-            celu_both(z[k] + __ldg(b + k), h, d);
+            celu_both(z[k], h, d);                             // z1 already holds the bias
             p[k] *= d;
           }
           uint8_t* slot = acquire();
@@ -325,9 +356,12 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           const int N = tc_phase_n(p), nk = tc_phase_nk(p);
           const uint32_t dcol = tbase + (uint32_t)tc_phase_dcol(p);
           const uint32_t idesc = tc::idesc_tf32(TC_TM, N);
-          if (p == 4) {
-            // d1pre overwrites z2 / z3 / d2pre: every delta2 chunk must exist first (the last
-            // chunk's barrier completes after the earlier ones: producers arrive in order)
+          const bool split_acc = N_TERMS == 3 && (p == 0 || p == 2);
+          const uint32_t scol = tbase + (uint32_t)(p == 0 ? TC_S0_COL : TC_S2_COL);
+          if (p == 3 || p == 4) {
+            // p4: d1pre overwrites z2 / z3 / d2pre: every delta2 chunk must exist first (the last
+            // chunk's barrier completes after the earlier ones: producers arrive in order);
+            // p3: d2pre overwrites S2, which the delta3 producers still read
             const uint32_t il = ia + (uint32_t)nk - 1;
             tc::mbar_wait(&S.a_full[il % TC_NA], (il / TC_NA) & 1u);
           }
@@ -346,7 +380,11 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
             for (int ks = 0; ks < 4; ++ks) {
               const uint64_t dah = tc::smem_desc_sw128(a_hi + 32 * ks), dal = tc::smem_desc_sw128(a_lo + 32 * ks);
               const uint64_t dbh = tc::smem_desc_sw128(b_hi + 32 * ks), dbl = tc::smem_desc_sw128(b_lo + 32 * ks);
-              if (N_TERMS == 3) {
+              if (split_acc) {
+                tc::mma_tf32_ss(scol, dal, dbh, idesc, (c | ks) ? 1u : 0u);
+                tc::mma_tf32_ss(scol, dah, dbl, idesc, 1u);
+                tc::mma_tf32_ss(dcol, dah, dbh, idesc, (c | ks) ? 1u : 0u);
+              } else if (N_TERMS == 3) {
                 tc::mma_tf32_ss(dcol, dal, dbh, idesc, (c | ks) ? 1u : 0u);
                 tc::mma_tf32_ss(dcol, dah, dbl, idesc, 1u);
                 tc::mma_tf32_ss(dcol, dah, dbh, idesc, 1u);

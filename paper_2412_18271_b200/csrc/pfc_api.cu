@@ -392,7 +392,10 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
             u = (u + 0x1000u) & 0xFFFFE000u;               // hi: rounded to tf32 precision
             float hi;
             memcpy(&hi, &u, 4);
-            const float lo = v - hi;                        // exact
+            float lo = v - hi;                              // exact; then rounded to tf32 like hi
+            memcpy(&u, &lo, 4);
+            u = (u + 0x1000u) & 0xFFFFE000u;
+            memcpy(&lo, &u, 4);
             memcpy(chunk + tc::sw128_off(n, kk), &hi, 4);
             memcpy(chunk + (size_t)N * 128 + tc::sw128_off(n, kk), &lo, 4);
           }

@@ -22,6 +22,7 @@ AEV_LEN = 384
 N_WEIGHTS = 378756
 MLP_FP32 = 0
 MLP_TF32X3 = 1
+MLP_TF32X1 = 2            # plain TF32: tolerance evidence only
 
 STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
                4: "angular row longer than PFC_MAX_ANGULAR", 8: "non-finite energy",
