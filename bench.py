@@ -136,6 +136,22 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(seconds, device=None):
+    """Whole-job time = the slowest rank's device time (no data-path collective: replicas only)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(seconds)
+    tt = torch.tensor([seconds], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def job_value(atoms_per_rank, steps, world, seconds):
+    """atom-steps/s of the whole job: every rank advances its own copy of the batch (weak scaling)."""
+    return world * atoms_per_rank * steps / seconds
+
+
 def _time_steps(torch, p, stream, n_steps):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(stream):
@@ -187,13 +203,10 @@ def run_pfc(args):
     t = _time_steps(torch, p, stream, args.steps)                # EXACTLY K steps, device time
     barrier()
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        tt = torch.tensor([t], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t = float(tt.item())
+    t = max_over_ranks(t, dev)
     status = p.status()
     _, launches_step = p.launch_counts()
-    value = world * N * args.steps / t
+    value = job_value(N, args.steps, world, t)
 
     line = None
     if rank == 0:
