@@ -1,36 +1,59 @@
-// k3_mlp_fp32.cuh -- K3 (FP32 FFMA path): per-element MLP 384->160->128->96->1 with
-// CELU(0.1), forward and input-gradient backward, fused per 64-row tile
+// k3_mlp_fp32.cuh -- K3 (FP32 FFMA path, the default): per-element MLP 384->160->128->96->1
+// with CELU(0.1), forward and input-gradient backward, fused per row tile
 // (O5; backward = PAPER.md:67 "forces by backprop", weight gradients
 // are never needed).
 //
-// Rows are atoms of ONE element (element blocks are padded to ROW_PAD rows), so
-// a tile is a dense [64 x K] x [K x N] contraction chain -- a grouped GEMM over
-// the four element blocks.  Activations stay in shared memory, k-major
-// (XT[k][m], stride 68 floats) so a warp's 8-row A fragment is two broadcast
-// LDS.128; weights stream from L2 through a cp.async double buffer, laid out
-// [k][n] for every GEMM (forward uses transposed copies made by pfc_create).
-// Thread tile: 8 rows (warp w -> rows 8w..8w+7) x N/32 columns (lane + 32c).
-// This path is kept as the in-tolerance FP32 reference for the tensor-core path.
+// Rows are atoms of ONE element (element blocks are padded to ROW_PAD = 128 rows), so a
+// tile is a dense [128 x K] x [K x N] contraction chain -- a grouped GEMM over the four
+// element blocks.  Tile height TM is a template parameter (16, 32, 64, 128; pfc_create picks 32,
+// or 16 for small batches -- measurements in pfc_api.cu); 8 warps per (up to) 64 rows.
+// A warp owns min(TM,64) rows x N/8 columns: lane = (row group rg = lane/4,
+// column group cg = lane%4), thread rows 64*half + rg + 8r (r < 8), thread columns 4q..4q+3
+// (+ 128+q for N = 160; 2q, 2q+1, 64+q for N = 96) with q = 4*(warp%8) + cg.  Per k that is
+// 2 + (1 or 2) shared-memory wavefronts for 8*N/32 FFMA per thread (0.1 per FFMA), which keeps
+// the LSU pipe clear of the FMA pipe.
+//   * activations h1/h2/h3 (later delta1/2/3) stay in shared memory, row-major with row stride
+//     = 4 mod 32 floats, so the eight row groups of a warp read eight different bank groups;
+//   * the AEV tile is NOT held: phase 0 streams it in 16-wide K chunks with cp.async
+//     (into the h2 region, idle at that time) next to the weight chunks;
+//   * weights are laid out by pfc_create per phase as B[k][n], so a chunk of 16 k is one
+//     contiguous block fetched from L2 by ONE cp.async.bulk (TMA) on an mbarrier, double buffered;
+//   * warps whose 64 rows are all padding skip the arithmetic.
 #pragma once
 #include "pfc_common.cuh"
+#include "tc_ptx.cuh"
 
 namespace pfc {
 
-constexpr int MLP_TM = 64;
-constexpr int MLP_THREADS = 256;
-constexpr int MLP_KC = 16;
-constexpr int MLP_LDT = MLP_TM + 4;      // 68: k-major activation stride
-constexpr int MLP_BS_FLOATS = MLP_KC * D1;   // one staging buffer (widest N = 160)
-constexpr size_t MLP_FP32_SMEM =
-    sizeof(float) * ((size_t)(D0 + D1 + D2 + D3) * MLP_LDT + 2 * MLP_BS_FLOATS);   // 229,376 B
-
-struct MlpWeights {          // device pointers, one set per element
-  const float *W1t, *b1, *W2t, *b2, *W3t, *b3, *W4, *b4;   // forward: [k][n]
-  const float *W1, *W2, *W3;                               // backward: original [out][in]
+constexpr int MLP_LD1 = D1 + 4, MLP_LD2 = D2 + 4, MLP_LD3 = D3 + 4;   // row strides (floats): 4 mod 32
+template <int TM> struct MlpCfg {                                     // TM = 16, 32, 64 or 128 rows per tile
+  static constexpr int THREADS = TM >= 64 ? 4 * TM : 256;             // 8 warps per (up to) 64 rows
+  static constexpr int R = TM >= 64 ? 8 : TM / 8;                     // rows per thread
+  static constexpr int KC = TM == 64 ? 8 : 16;                        // k per staged chunk (64: two CTAs per SM)
+  static constexpr int AS_LD = KC + 4;                                // AEV chunk row stride: 4 mod 8 floats
+  static constexpr int AS_FLOATS = TM * AS_LD;                        // one AEV chunk [TM][KC+4]
+  static constexpr int BS_FLOATS = KC * D1;                           // one weight buffer (widest N = 160)
+  static constexpr size_t SMEM = sizeof(float) * ((size_t)TM * (MLP_LD1 + MLP_LD2 + MLP_LD3) +
+                                                  2 * BS_FLOATS + (size_t)TM * 8) + 64;
+  static_assert(2 * AS_FLOATS <= TM * MLP_LD2, "AEV chunks live in the h2 region during phase 0");
 };
+
+// weight image per element (floats): phases 0..5, each B[K][N] row-major
+constexpr int MLP_P_OFF0 = 0;                          // W1^T  K=384 N=160
+constexpr int MLP_P_OFF1 = MLP_P_OFF0 + D0 * D1;       // W2^T  K=160 N=128
+constexpr int MLP_P_OFF2 = MLP_P_OFF1 + D1 * D2;       // W3^T  K=128 N=96
+constexpr int MLP_P_OFF3 = MLP_P_OFF2 + D2 * D3;       // W3    K=96  N=128
+constexpr int MLP_P_OFF4 = MLP_P_OFF3 + D3 * D2;       // W2    K=128 N=160
+constexpr int MLP_P_OFF5 = MLP_P_OFF4 + D2 * D1;       // W1    K=160 N=3x128 (pass-major)
+constexpr int MLP_P_FLOATS = MLP_P_OFF5 + D1 * D0;     // 188,416
+constexpr int MLP_V_B1 = 0, MLP_V_B2 = D1, MLP_V_B3 = D1 + D2, MLP_V_W4 = D1 + D2 + D3,
+              MLP_V_B4 = D1 + D2 + 2 * D3, MLP_V_FLOATS = 484;
+
 struct MlpParams {
-  MlpWeights w[NSPEC];
-  int row_start[NSPEC + 1];  // element block boundaries in padded row order
+  const float* wpack[NSPEC];   // MLP_P_FLOATS per element
+  const float* vec[NSPEC];     // b1 b2 b3 w4 b4
+  int row_start[NSPEC + 1];    // element block boundaries in padded row order
+  int row_end[NSPEC];          // row_start[e] + number of atoms of element e
 };
 
 __device__ __forceinline__ float celu_f(float x) {
@@ -49,163 +72,231 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
 
-// acc[r][c] = sum_k AT[k][8w + r] * B[k][n0 + lane + 32c],  k < K
-template <int K, int N>
-__device__ __forceinline__ void mlp_gemm(const float* __restrict__ AT, const float* __restrict__ Bg,
-                                         int ldb, float* __restrict__ Bs, float (&acc)[8][N / 32]) {
+struct MlpPipe {               // shared-memory staging state, uniform across the CTA
+  float* Bs;                   // [2][MLP_BS_FLOATS]
+  float* As;                   // [2][AS_FLOATS]  (phase 0 only)
+  uint64_t* full;              // [2] mbarriers: weight chunk landed
+  uint32_t gc;                 // chunks consumed so far (buffer = gc & 1, parity = (gc >> 1) & 1)
+};
+
+// column c (< NT) of the thread with column slot q, N = 32*NT
+template <int NT>
+__device__ __forceinline__ int mlp_col(int q, int c) {
+  return NT == 5 ? (c < 4 ? 4 * q + c : 128 + q) : NT == 4 ? 4 * q + c : (c < 2 ? 2 * q + c : 64 + q);
+}
+
+// acc[r][c] = sum_k A[rowbase + 8r][k] * B[k][mlp_col(q, c)],  k < K, r < R,  rowbase = 64*half + rg.
+// A_GLOBAL: A is the AEV tile in global memory (row stride AEV_LEN), streamed; else A is a
+// row-major shared-memory activation with row stride lda.
+template <int TM, int K, int N, bool A_GLOBAL>
+__device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A, int lda,
+                                         const float* __restrict__ Bg, bool active,
+                                         float (&acc)[MlpCfg<TM>::R][N / 32]) {
   constexpr int NT = N / 32;
+  constexpr int R = MlpCfg<TM>::R;
+  constexpr int MLP_KC = MlpCfg<TM>::KC, MLP_AS_LD = MlpCfg<TM>::AS_LD, MLP_BS_FLOATS = MlpCfg<TM>::BS_FLOATS;
   constexpr int NCH = K / MLP_KC;
-  constexpr int V4 = MLP_KC * N / 4;                     // float4s per chunk
+  constexpr int GR = MLP_KC / 4;                         // 16-byte granules per AEV chunk row
+  constexpr uint32_t CH_BYTES = MLP_KC * N * sizeof(float);
+  constexpr int AS_FLOATS = MlpCfg<TM>::AS_FLOATS;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const int rowbase = 64 * (w >> 3) + (lane >> 2), q = 4 * (w & 7) + (lane & 3);
 #pragma unroll
-  for (int r = 0; r < 8; ++r)
+  for (int r = 0; r < R; ++r)
 #pragma unroll
     for (int c = 0; c < NT; ++c) acc[r][c] = 0.0f;
-  auto stage = [&](int ch, int buf) {
-    const float* src = Bg + (size_t)ch * MLP_KC * ldb;
-    float* dst = Bs + buf * MLP_BS_FLOATS;
-    for (int q = tid; q < V4; q += MLP_THREADS) {
-      const int kk = q / (N / 4), n4 = q - kk * (N / 4);
-      cp_async16(dst + kk * N + 4 * n4, src + (size_t)kk * ldb + 4 * n4);
+  auto issue = [&](int ch, uint32_t buf) {
+    if (tid == 0) {
+      tc::mbar_arrive_expect_tx(&P.full[buf], CH_BYTES);
+      tc::bulk_g2s(P.Bs + buf * MLP_BS_FLOATS, Bg + (size_t)ch * MLP_KC * N, CH_BYTES, &P.full[buf]);
     }
-    cp_async_commit();
+    if (A_GLOBAL) {                                      // TM rows x 4 granules
+      if (tid < GR * TM)
+        cp_async16(P.As + buf * AS_FLOATS + (tid / GR) * MLP_AS_LD + 4 * (tid % GR),
+                   A + (size_t)(tid / GR) * AEV_LEN + ch * MLP_KC + 4 * (tid % GR));
+      cp_async_commit();
+    }
   };
-  __syncthreads();                                       // previous users of Bs / writers of AT done
-  stage(0, 0);
+  __syncthreads();                  // previous phase: activation stores visible, staging buffers free
+  issue(0, P.gc & 1u);
   for (int ch = 0; ch < NCH; ++ch) {
-    if (ch + 1 < NCH) { stage(ch + 1, (ch + 1) & 1); cp_async_wait<1>(); }
-    else cp_async_wait<0>();
-    __syncthreads();
-    const float* bs = Bs + (ch & 1) * MLP_BS_FLOATS + lane;
-    const float* at = AT + (size_t)ch * MLP_KC * MLP_LDT + 8 * w;
+    const uint32_t buf = P.gc & 1u;
+    if (A_GLOBAL) cp_async_wait<0>();
+    tc::mbar_wait(&P.full[buf], (P.gc >> 1) & 1u);
+    __syncthreads();                // all A granules visible; the other buffer is no longer read
+    if (ch + 1 < NCH) issue(ch + 1, buf ^ 1u);
+    ++P.gc;
+    if (!active) continue;
+    const float* bs = P.Bs + buf * MLP_BS_FLOATS;
+    const float* at = A_GLOBAL ? P.As + buf * AS_FLOATS + rowbase * MLP_AS_LD
+                               : A + (size_t)rowbase * lda + ch * MLP_KC;
+    const int astr = 8 * (A_GLOBAL ? MLP_AS_LD : lda);
 #pragma unroll
-    for (int kk = 0; kk < MLP_KC; ++kk) {
-      const float4 a0 = *reinterpret_cast<const float4*>(at + kk * MLP_LDT);
-      const float4 a1 = *reinterpret_cast<const float4*>(at + kk * MLP_LDT + 4);
-      const float a[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-      float b[NT];
+    for (int k4 = 0; k4 < MLP_KC / 4; ++k4) {
+      float4 a[R];
 #pragma unroll
-      for (int c = 0; c < NT; ++c) b[c] = bs[kk * N + 32 * c];
+      for (int r = 0; r < R; ++r) a[r] = *reinterpret_cast<const float4*>(at + r * astr + 4 * k4);
 #pragma unroll
-      for (int r = 0; r < 8; ++r)
+      for (int j = 0; j < 4; ++j) {
+        const float* brow = bs + (4 * k4 + j) * N;
+        float b[NT];
+        if (NT == 5) {
+          const float4 v = *reinterpret_cast<const float4*>(brow + 4 * q);
+          b[0] = v.x; b[1] = v.y; b[2] = v.z; b[3] = v.w;
+          b[NT - 1] = brow[128 + q];
+        } else if (NT == 4) {
+          const float4 v = *reinterpret_cast<const float4*>(brow + 4 * q);
+          b[0] = v.x; b[1] = v.y; b[2] = v.z; b[3] = v.w;
+        } else {
+          const float2 v = *reinterpret_cast<const float2*>(brow + 2 * q);
+          b[0] = v.x; b[1] = v.y;
+          b[NT - 1] = brow[64 + q];
+        }
 #pragma unroll
-        for (int c = 0; c < NT; ++c) acc[r][c] = fmaf(a[r], b[c], acc[r][c]);
+        for (int r = 0; r < R; ++r) {
+          const float av = j == 0 ? a[r].x : j == 1 ? a[r].y : j == 2 ? a[r].z : a[r].w;
+#pragma unroll
+          for (int c = 0; c < NT; ++c) acc[r][c] = fmaf(av, b[c], acc[r][c]);
+        }
+      }
     }
-    __syncthreads();
   }
 }
 
-// store an [8 x NT] thread tile k-major: HT[n][8w + r]
-template <int NT>
-__device__ __forceinline__ void store_tile_T(float* __restrict__ HT, const float (&v)[8][NT]) {
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-#pragma unroll
-  for (int c = 0; c < NT; ++c) {
-    float* p = HT + (size_t)(lane + 32 * c) * MLP_LDT + 8 * w;
-    *reinterpret_cast<float4*>(p) = make_float4(v[0][c], v[1][c], v[2][c], v[3][c]);
-    *reinterpret_cast<float4*>(p + 4) = make_float4(v[4][c], v[5][c], v[6][c], v[7][c]);
-  }
-}
-
-__global__ void __launch_bounds__(MLP_THREADS, 1)
+template <int TM>
+__global__ void __launch_bounds__(MlpCfg<TM>::THREADS, TM == 64 ? 2 : 1)
 k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict__ aev,
                    float* __restrict__ g, float* __restrict__ e_row) {
   extern __shared__ __align__(16) float smem[];
-  float* XT = smem;
-  float* H1T = XT + D0 * MLP_LDT;
-  float* H2T = H1T + D1 * MLP_LDT;
-  float* H3T = H2T + D2 * MLP_LDT;
-  float* Bs = H3T + D3 * MLP_LDT;
+  float* H1 = smem;                                   // [TM][LD1]  h1, later delta1
+  float* H2 = H1 + TM * MLP_LD1;                      // [TM][LD2]  h2, later delta2 (phase 0: AEV chunks)
+  float* H3 = H2 + TM * MLP_LD2;                      // [TM][LD3]  delta3
+  MlpPipe pipe;
+  pipe.Bs = H3 + TM * MLP_LD3;
+  pipe.As = H2;
+  float* esum = pipe.Bs + 2 * MlpCfg<TM>::BS_FLOATS;          // [TM][8] partial energies per column group
+  pipe.full = reinterpret_cast<uint64_t*>(esum + TM * 8);
+  pipe.gc = 0;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  const int row0 = blockIdx.x * MLP_TM;
+  constexpr int R = MlpCfg<TM>::R;
+  const int rowbase = 64 * (w >> 3) + (lane >> 2), q = 4 * (w & 7) + (lane & 3);
+  const int row0 = blockIdx.x * TM;
   int el = 0;
 #pragma unroll
-  for (int q = 1; q < NSPEC; ++q) el += (row0 >= P.row_start[q]);
-  const MlpWeights W = P.w[el];
-
-  // AEV tile -> XT (transposed): warp w loads rows 8w..8w+7, lanes along k
-  for (int r = 0; r < 8; ++r) {
-    const float* src = aev + (size_t)(row0 + 8 * w + r) * AEV_LEN;
-#pragma unroll
-    for (int q = 0; q < AEV_LEN / 32; ++q) XT[(size_t)(lane + 32 * q) * MLP_LDT + 8 * w + r] = src[lane + 32 * q];
+  for (int k = 1; k < NSPEC; ++k) el += (row0 >= P.row_start[k]);
+  const float* __restrict__ Wp = P.wpack[el];
+  const float* __restrict__ V = P.vec[el];
+  if (row0 >= P.row_end[el]) return;                  // a tile of padding only (CTA-uniform)
+  const bool active = row0 + 64 * (w >> 3) < P.row_end[el];   // warp-uniform: my 64 rows hold an atom
+  if (tid == 0) {
+    tc::mbar_init(&pipe.full[0], 1);
+    tc::mbar_init(&pipe.full[1], 1);
+    tc::mbar_fence_init();
   }
+  // (the first __syncthreads of mlp_gemm orders the init before any use)
+
   // ---- forward ----
   {
-    float acc[8][D1 / 32];
-    mlp_gemm<D0, D1>(XT, W.W1t, D1, Bs, acc);
+    constexpr int NT = D1 / 32;
+    float acc[R][NT];
+    mlp_gemm<TM, D0, D1, true>(pipe, aev + (size_t)row0 * AEV_LEN, 0, Wp + MLP_P_OFF0, active, acc);
+    if (active) {
 #pragma unroll
-    for (int c = 0; c < D1 / 32; ++c) {
-      const float bias = W.b1[lane + 32 * c];
+      for (int c = 0; c < NT; ++c) {
+        const int n = mlp_col<NT>(q, c);
+        const float bias = __ldg(V + MLP_V_B1 + n);
 #pragma unroll
-      for (int r = 0; r < 8; ++r) acc[r][c] = celu_f(acc[r][c] + bias);
-    }
-    store_tile_T<D1 / 32>(H1T, acc);
-  }
-  {
-    float acc[8][D2 / 32];
-    mlp_gemm<D1, D2>(H1T, W.W2t, D2, Bs, acc);
-#pragma unroll
-    for (int c = 0; c < D2 / 32; ++c) {
-      const float bias = W.b2[lane + 32 * c];
-#pragma unroll
-      for (int r = 0; r < 8; ++r) acc[r][c] = celu_f(acc[r][c] + bias);
-    }
-    store_tile_T<D2 / 32>(H2T, acc);
-  }
-  {
-    float acc[8][D3 / 32];
-    mlp_gemm<D2, D3>(H2T, W.W3t, D3, Bs, acc);
-    float part[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-    for (int c = 0; c < D3 / 32; ++c) {
-      const float bias = W.b3[lane + 32 * c], w4 = W.W4[lane + 32 * c];
-#pragma unroll
-      for (int r = 0; r < 8; ++r) {
-        const float h = celu_f(acc[r][c] + bias);
-        part[r] = fmaf(w4, h, part[r]);
-        acc[r][c] = w4 * dcelu_from_h(h);               // delta3 = dE/dz3
+        for (int r = 0; r < R; ++r) H1[(rowbase + 8 * r) * MLP_LD1 + n] = celu_f(acc[r][c] + bias);
       }
     }
-    store_tile_T<D3 / 32>(H3T, acc);
-    const float b4 = W.b4[0];
+  }
+  {
+    constexpr int NT = D2 / 32;
+    float acc[R][NT];
+    mlp_gemm<TM, D1, D2, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF1, active, acc);
+    if (active) {
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-      const float s = warp_sum(part[r]);
-      if (lane == 0) e_row[row0 + 8 * w + r] = s + b4;
+      for (int c = 0; c < NT; ++c) {
+        const int n = mlp_col<NT>(q, c);
+        const float bias = __ldg(V + MLP_V_B2 + n);
+#pragma unroll
+        for (int r = 0; r < R; ++r) H2[(rowbase + 8 * r) * MLP_LD2 + n] = celu_f(acc[r][c] + bias);
+      }
+    }
+  }
+  {
+    constexpr int NT = D3 / 32;
+    float acc[R][NT];
+    mlp_gemm<TM, D2, D3, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF2, active, acc);
+    float part[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) part[r] = 0.0f;
+    if (active) {
+#pragma unroll
+      for (int c = 0; c < NT; ++c) {
+        const int n = mlp_col<NT>(q, c);
+        const float bias = __ldg(V + MLP_V_B3 + n), w4 = __ldg(V + MLP_V_W4 + n);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+          const float h = celu_f(acc[r][c] + bias);
+          part[r] = fmaf(w4, h, part[r]);
+          H3[(rowbase + 8 * r) * MLP_LD3 + n] = w4 * dcelu_from_h(h);   // delta3 = dE/dz3
+        }
+      }
+    }
+    // e_i = b4 + sum over the 96 columns: 4 lanes (xor tree), then the 8 column groups in order
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      float s = part[r];
+      s += __shfl_xor_sync(0xffffffffu, s, 1);
+      s += __shfl_xor_sync(0xffffffffu, s, 2);
+      if ((lane & 3) == 0) esum[(rowbase + 8 * r) * 8 + (w & 7)] = s;
+    }
+    __syncthreads();
+    if (tid < TM && row0 + tid < P.row_end[el]) {
+      const float* p = esum + tid * 8;
+      e_row[row0 + tid] = (((p[0] + p[1]) + (p[2] + p[3])) + ((p[4] + p[5]) + (p[6] + p[7]))) + __ldg(V + MLP_V_B4);
     }
   }
   // ---- backward (input gradient only) ----
   {
-    float acc[8][D2 / 32];
-    mlp_gemm<D3, D2>(H3T, W.W3, D2, Bs, acc);
+    constexpr int NT = D2 / 32;
+    float acc[R][NT];
+    mlp_gemm<TM, D3, D2, false>(pipe, H3, MLP_LD3, Wp + MLP_P_OFF3, active, acc);
+    if (active) {
 #pragma unroll
-    for (int c = 0; c < D2 / 32; ++c) {
-      const float* hp = H2T + (size_t)(lane + 32 * c) * MLP_LDT + 8 * w;
+      for (int c = 0; c < NT; ++c)
 #pragma unroll
-      for (int r = 0; r < 8; ++r) acc[r][c] *= dcelu_from_h(hp[r]);
+        for (int r = 0; r < R; ++r) {
+          float* hp = H2 + (rowbase + 8 * r) * MLP_LD2 + mlp_col<NT>(q, c);
+          *hp = acc[r][c] * dcelu_from_h(*hp);          // delta2 over h2 (own elements only)
+        }
     }
-    store_tile_T<D2 / 32>(H2T, acc);                    // delta2 over h2 (own elements only)
   }
   {
-    float acc[8][D1 / 32];
-    mlp_gemm<D2, D1>(H2T, W.W2, D1, Bs, acc);
+    constexpr int NT = D1 / 32;
+    float acc[R][NT];
+    mlp_gemm<TM, D2, D1, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF4, active, acc);
+    if (active) {
 #pragma unroll
-    for (int c = 0; c < D1 / 32; ++c) {
-      const float* hp = H1T + (size_t)(lane + 32 * c) * MLP_LDT + 8 * w;
+      for (int c = 0; c < NT; ++c)
 #pragma unroll
-      for (int r = 0; r < 8; ++r) acc[r][c] *= dcelu_from_h(hp[r]);
+        for (int r = 0; r < R; ++r) {
+          float* hp = H1 + (rowbase + 8 * r) * MLP_LD1 + mlp_col<NT>(q, c);
+          *hp = acc[r][c] * dcelu_from_h(*hp);          // delta1
+        }
     }
-    store_tile_T<D1 / 32>(H1T, acc);                    // delta1
   }
 #pragma unroll 1
-  for (int n0 = 0; n0 < D0; n0 += 128) {
-    float acc[8][4];
-    mlp_gemm<D1, 128>(H1T, W.W1 + n0, D0, Bs, acc);
+  for (int pass = 0; pass < D0 / 128; ++pass) {
+    float acc[R][4];
+    mlp_gemm<TM, D1, 128, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF5 + pass * D1 * 128, active, acc);
+    if (active) {
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-      float* dst = g + (size_t)(row0 + 8 * w + r) * AEV_LEN + n0 + lane;
-#pragma unroll
-      for (int c = 0; c < 4; ++c) dst[32 * c] = acc[r][c];
+      for (int r = 0; r < R; ++r) {
+        float* dst = g + (size_t)(row0 + rowbase + 8 * r) * AEV_LEN + pass * 128 + 4 * q;
+        *reinterpret_cast<float4*>(dst) = make_float4(acc[r][0], acc[r][1], acc[r][2], acc[r][3]);
+      }
     }
   }
 }

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -25,20 +26,9 @@ namespace {
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-// per-element weight block on the device (floats), forward then backward copies
-constexpr int OFF_W1T = 0;
-constexpr int OFF_B1 = OFF_W1T + D0 * D1;
-constexpr int OFF_W2T = OFF_B1 + D1;
-constexpr int OFF_B2 = OFF_W2T + D1 * D2;
-constexpr int OFF_W3T = OFF_B2 + D2;
-constexpr int OFF_B3 = OFF_W3T + D2 * D3;
-constexpr int OFF_W4 = OFF_B3 + D3;
-constexpr int OFF_B4 = OFF_W4 + D3;
-constexpr int OFF_W1 = OFF_B4 + 4;
-constexpr int OFF_W2 = OFF_W1 + D1 * D0;
-constexpr int OFF_W3 = OFF_W2 + D2 * D1;
-constexpr int DEV_W_PER_ELEM = OFF_W3 + D3 * D2;
-static_assert(DEV_W_PER_ELEM % 4 == 0 && OFF_W1 % 4 == 0 && OFF_W2T % 4 == 0 && OFF_W3T % 4 == 0, "16-byte rows");
+// per-element FFMA weight block on the device (floats): packed phase images, then b1 b2 b3 w4 b4
+constexpr int DEV_W_PER_ELEM = MLP_P_FLOATS + MLP_V_FLOATS;
+static_assert(MLP_P_FLOATS % 4 == 0 && DEV_W_PER_ELEM % 4 == 0, "16-byte aligned blocks");
 
 struct Carver {                 // bump allocator over the caller's workspace (or a dry run)
   char* base;
@@ -157,6 +147,7 @@ struct pfc_ctx {
   MlpParams mlp;
   TcParams tcp;
   int mlp_path;
+  int mlp_tm = 128;             // FFMA K3 tile height
   int n_sms = 148;
   int n_cell_sys, n_cell_atoms;
   int launches_ef, launches_step;
@@ -224,7 +215,16 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
          b.row_of_atom, b.aev, b.status);
   mark(2);
   if (c->mlp_path == PFC_MLP_FP32) {
-    LAUNCH(c, k3_mlp_fp32_kernel, s.n_rows / MLP_TM, MLP_THREADS, MLP_FP32_SMEM, st, c->mlp, b.aev, b.g, b.e_row);
+    switch (c->mlp_tm) {                                 // tile height chosen by pfc_create
+      case 128: LAUNCH(c, k3_mlp_fp32_kernel<128>, s.n_rows / 128, MlpCfg<128>::THREADS, MlpCfg<128>::SMEM, st,
+                       c->mlp, b.aev, b.g, b.e_row); break;
+      case 64:  LAUNCH(c, k3_mlp_fp32_kernel<64>, s.n_rows / 64, MlpCfg<64>::THREADS, MlpCfg<64>::SMEM, st,
+                       c->mlp, b.aev, b.g, b.e_row); break;
+      case 32:  LAUNCH(c, k3_mlp_fp32_kernel<32>, s.n_rows / 32, MlpCfg<32>::THREADS, MlpCfg<32>::SMEM, st,
+                       c->mlp, b.aev, b.g, b.e_row); break;
+      default:  LAUNCH(c, k3_mlp_fp32_kernel<16>, s.n_rows / 16, MlpCfg<16>::THREADS, MlpCfg<16>::SMEM, st,
+                       c->mlp, b.aev, b.g, b.e_row); break;
+    }
   } else {
     const int grid = c->tcp.n_tiles < c->n_sms ? c->tcp.n_tiles : c->n_sms;   // persistent: one CTA per SM
     if (c->mlp_path == PFC_MLP_TF32X3)
@@ -336,27 +336,35 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   carve(c->sz, d->workspace, &c->b);
   Buffers& b = c->b;
 
-  // device weights: forward copies transposed to [k][n], backward copies as given
+  // FFMA path: per element, every GEMM phase as a row-major B[k][n] (forward: W^T, backward: W,
+  // the last one in three 128-column passes), so a 16-k chunk is one contiguous bulk copy
   std::vector<float> w((size_t)NSPEC * DEV_W_PER_ELEM, 0.0f);
   for (int e = 0; e < NSPEC; ++e) {
     const float* src = d->weights + (size_t)e * W_PER_ELEM;
     const float *W1 = src, *b1 = W1 + D1 * D0, *W2 = b1 + D1, *b2 = W2 + D2 * D1, *W3 = b2 + D2,
                 *b3 = W3 + D3 * D2, *W4 = b3 + D3, *b4 = W4 + D3;
     float* dst = w.data() + (size_t)e * DEV_W_PER_ELEM;
-    for (int o = 0; o < D1; ++o) for (int k = 0; k < D0; ++k) dst[OFF_W1T + k * D1 + o] = W1[o * D0 + k];
-    for (int o = 0; o < D2; ++o) for (int k = 0; k < D1; ++k) dst[OFF_W2T + k * D2 + o] = W2[o * D1 + k];
-    for (int o = 0; o < D3; ++o) for (int k = 0; k < D2; ++k) dst[OFF_W3T + k * D3 + o] = W3[o * D2 + k];
-    memcpy(dst + OFF_B1, b1, sizeof(float) * D1);
-    memcpy(dst + OFF_B2, b2, sizeof(float) * D2);
-    memcpy(dst + OFF_B3, b3, sizeof(float) * D3);
-    memcpy(dst + OFF_W4, W4, sizeof(float) * D3);
-    dst[OFF_B4] = b4[0];
-    memcpy(dst + OFF_W1, W1, sizeof(float) * D1 * D0);
-    memcpy(dst + OFF_W2, W2, sizeof(float) * D2 * D1);
-    memcpy(dst + OFF_W3, W3, sizeof(float) * D3 * D2);
+    auto pack = [&](float* out, int K, int N, auto bval) {        // out[k][n] = B[k][n]
+      for (int k = 0; k < K; ++k)
+        for (int n = 0; n < N; ++n) out[(size_t)k * N + n] = bval(k, n);
+    };
+    pack(dst + MLP_P_OFF0, D0, D1, [&](int k, int n) { return W1[n * D0 + k]; });
+    pack(dst + MLP_P_OFF1, D1, D2, [&](int k, int n) { return W2[n * D1 + k]; });
+    pack(dst + MLP_P_OFF2, D2, D3, [&](int k, int n) { return W3[n * D2 + k]; });
+    pack(dst + MLP_P_OFF3, D3, D2, [&](int k, int n) { return W3[k * D2 + n]; });
+    pack(dst + MLP_P_OFF4, D2, D1, [&](int k, int n) { return W2[k * D1 + n]; });
+    for (int pass = 0; pass < D0 / 128; ++pass)
+      pack(dst + MLP_P_OFF5 + pass * D1 * 128, D1, 128, [&](int k, int n) { return W1[k * D0 + pass * 128 + n]; });
+    float* v = dst + MLP_P_FLOATS;
+    memcpy(v + MLP_V_B1, b1, sizeof(float) * D1);
+    memcpy(v + MLP_V_B2, b2, sizeof(float) * D2);
+    memcpy(v + MLP_V_B3, b3, sizeof(float) * D3);
+    memcpy(v + MLP_V_W4, W4, sizeof(float) * D3);
+    v[MLP_V_B4] = b4[0];
     const float* dv = b.weights + (size_t)e * DEV_W_PER_ELEM;
-    c->mlp.w[e] = MlpWeights{dv + OFF_W1T, dv + OFF_B1, dv + OFF_W2T, dv + OFF_B2, dv + OFF_W3T, dv + OFF_B3,
-                             dv + OFF_W4,  dv + OFF_B4, dv + OFF_W1,  dv + OFF_W2, dv + OFF_W3};
+    c->mlp.wpack[e] = dv;
+    c->mlp.vec[e] = dv + MLP_P_FLOATS;
+    c->mlp.row_end[e] = row_start[e] + count[e];
   }
   for (int e = 0; e <= NSPEC; ++e) c->mlp.row_start[e] = row_start[e];
 
@@ -456,8 +464,14 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (cudaMemset(b.aev, 0, sizeof(float) * (size_t)c->sz.n_rows * AEV_LEN) != cudaSuccess) ok = false;
   if (cudaMemset(b.status, 0, 256) != cudaSuccess) ok = false;
   if (cudaMemset(b.xlo, 0, sizeof(float4) * N) != cudaSuccess) ok = false;
-  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)MLP_FP32_SMEM) != cudaSuccess) ok = false;
+  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)MlpCfg<128>::SMEM) != cudaSuccess) ok = false;
+  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)MlpCfg<64>::SMEM) != cudaSuccess) ok = false;
+  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)MlpCfg<32>::SMEM) != cudaSuccess) ok = false;
+  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)MlpCfg<16>::SMEM) != cudaSuccess) ok = false;
   if (cudaFuncSetAttribute(k3_mlp_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)TC_SMEM_BYTES) != cudaSuccess) ok = false;
   if (cudaFuncSetAttribute(k3_mlp_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -467,6 +481,19 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
     if (cudaGetDevice(&dev) == cudaSuccess &&
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
       c->n_sms = sms;
+  }
+  {
+    // FFMA K3 tile height.  Measured on B200 (config 4, K3 alone): 32-row tiles, three CTAs per SM,
+    // 2.14 ms; 64 rows, two CTAs per SM, 2.16 ms; 128 rows, one CTA, 2.22 ms -- and on config 3
+    // 0.23 / 0.28 / 0.35 ms: co-resident small tiles hide the per-chunk latency best and quantise
+    // the grid finest.  A batch that cannot give every SM a 32-row tile uses 16-row tiles (a lone
+    // 16-row tile takes 50 us, a 64-row one 99 us).  PFC_K3_TM overrides (tuning only).
+    auto tiles = [&](int tm) { int n = 0; for (int e = 0; e < NSPEC; ++e) n += (count[e] + tm - 1) / tm; return n; };
+    c->mlp_tm = tiles(32) >= c->n_sms ? 32 : 16;
+    if (const char* ov = getenv("PFC_K3_TM")) {
+      const int v = atoi(ov);
+      if (v == 16 || v == 32 || v == 64 || v == 128) c->mlp_tm = v;
+    }
   }
   if (cudaDeviceSynchronize() != cudaSuccess) ok = false;
   if (!ok) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
