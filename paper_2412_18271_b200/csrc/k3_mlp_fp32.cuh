@@ -5,19 +5,25 @@
 //
 // Rows are atoms of ONE element (element blocks are padded to ROW_PAD = 128 rows), so a
 // tile is a dense [128 x K] x [K x N] contraction chain -- a grouped GEMM over the four
-// element blocks.  Tile height TM is a template parameter (16, 32, 64, 128; pfc_create picks 32,
-// or 16 for small batches -- measurements in pfc_api.cu); 8 warps per (up to) 64 rows.
-// A warp owns min(TM,64) rows x N/8 columns: lane = (row group rg = lane/4,
-// column group cg = lane%4), thread rows 64*half + rg + 8r (r < 8), thread columns 4q..4q+3
-// (+ 128+q for N = 160; 2q, 2q+1, 64+q for N = 96) with q = 4*(warp%8) + cg.  Per k that is
-// 2 + (1 or 2) shared-memory wavefronts for 8*N/32 FFMA per thread (0.1 per FFMA), which keeps
-// the LSU pipe clear of the FMA pipe.
+// element blocks.  Tile height TM is a template parameter (16, 32, 64, 128; pfc_create picks it,
+// measurements in pfc_api.cu); 8 warps per (up to) 64 rows.
+// A warp owns min(TM,64) rows x N/8 columns: lane = (row group rg = lane/2, column group
+// cg = lane%2), thread rows 64*half + rg + 16r (r < R = min(TM,64)/16), thread columns: float4s at
+// 4*cgi + 64*f (f < N/64) plus, for N = 160 / 96, a float2 at 64*(N/64) + 2*cgi, cgi = 2*(warp%8) + cg.
+// The lane mapping is chosen for the shared-memory pipe, which is what bounds this kernel (ncu:
+// 84 % of the LSU wavefront peak with the earlier rg = lane/4, cg = lane%4 mapping).  Measured on
+// B200: an LDS.128 costs 2 cycles of the SM's shared-memory pipe when lanes with equal addresses are
+// adjacent (or there are only two addresses, alternating), 4 cycles otherwise; with 16 row groups
+// of two adjacent lanes BOTH operand loads are 2-cycle: per 4 k a warp spends 2R + 2N/16 pipe
+// cycles for R*N/16 FFMA issue cycles (TM = 64, N = 128: 24 vs 32).
 //   * activations h1/h2/h3 (later delta1/2/3) stay in shared memory, row-major with row stride
-//     = 4 mod 32 floats, so the eight row groups of a warp read eight different bank groups;
+//     = 4 mod 32 floats, so the eight row groups of a half warp read eight different bank groups;
 //   * the AEV tile is NOT held: phase 0 streams it in 16-wide K chunks with cp.async
 //     (into the h2 region, idle at that time) next to the weight chunks;
 //   * weights are laid out by pfc_create per phase as B[k][n], so a chunk of 16 k is one
-//     contiguous block fetched from L2 by ONE cp.async.bulk (TMA) on an mbarrier, double buffered;
+//     contiguous block fetched from L2 by ONE cp.async.bulk (TMA) on an mbarrier, double buffered
+//     (a 4-stage full/empty mbarrier ring with no CTA barrier inside a phase was measured slower:
+//     2.30 vs 2.18 ms at 128 rows, 2.37 vs 2.12 ms at 32 rows, config 4);
 //   * warps whose 64 rows are all padding skip the arithmetic.
 #pragma once
 #include "pfc_common.cuh"
@@ -28,7 +34,7 @@ namespace pfc {
 constexpr int MLP_LD1 = D1 + 4, MLP_LD2 = D2 + 4, MLP_LD3 = D3 + 4;   // row strides (floats): 4 mod 32
 template <int TM> struct MlpCfg {                                     // TM = 16, 32, 64 or 128 rows per tile
   static constexpr int THREADS = TM >= 64 ? 4 * TM : 256;             // 8 warps per (up to) 64 rows
-  static constexpr int R = TM >= 64 ? 8 : TM / 8;                     // rows per thread
+  static constexpr int R = TM >= 64 ? 4 : TM / 16;                    // rows per thread
   static constexpr int KC = TM == 64 ? 8 : 16;                        // k per staged chunk (64: two CTAs per SM)
   static constexpr int AS_LD = KC + 4;                                // AEV chunk row stride: 4 mod 8 floats
   static constexpr int AS_FLOATS = TM * AS_LD;                        // one AEV chunk [TM][KC+4]
@@ -79,20 +85,23 @@ struct MlpPipe {               // shared-memory staging state, uniform across th
   uint32_t gc;                 // chunks consumed so far (buffer = gc & 1, parity = (gc >> 1) & 1)
 };
 
-// column c (< NT) of the thread with column slot q, N = 32*NT
-template <int NT>
-__device__ __forceinline__ int mlp_col(int q, int c) {
-  return NT == 5 ? (c < 4 ? 4 * q + c : 128 + q) : NT == 4 ? 4 * q + c : (c < 2 ? 2 * q + c : 64 + q);
+// column c (< N/16) of the thread with column slot cgi (< 16)
+template <int N>
+__device__ __forceinline__ int mlp_col(int cgi, int c) {
+  constexpr int NF4 = N / 64;
+  return c < 4 * NF4 ? 64 * (c >> 2) + 4 * cgi + (c & 3) : 64 * NF4 + 2 * cgi + (c - 4 * NF4);
 }
 
-// acc[r][c] = sum_k A[rowbase + 8r][k] * B[k][mlp_col(q, c)],  k < K, r < R,  rowbase = 64*half + rg.
+// acc[r][c] = sum_k A[rowbase + 16r][k] * B[k][mlp_col<N>(cgi, c)],  k < K, r < R,  rowbase = 64*half + rg.
 // A_GLOBAL: A is the AEV tile in global memory (row stride AEV_LEN), streamed; else A is a
 // row-major shared-memory activation with row stride lda.
 template <int TM, int K, int N, bool A_GLOBAL>
 __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A, int lda,
                                          const float* __restrict__ Bg, bool active,
-                                         float (&acc)[MlpCfg<TM>::R][N / 32]) {
-  constexpr int NT = N / 32;
+                                         float (&acc)[MlpCfg<TM>::R][N / 16]) {
+  constexpr int NT = N / 16;
+  constexpr int NF4 = N / 64;                            // float4 column groups per thread
+  constexpr bool HAS2 = (N % 64) == 32;                  // plus one float2 group (N = 160, 96)
   constexpr int R = MlpCfg<TM>::R;
   constexpr int MLP_KC = MlpCfg<TM>::KC, MLP_AS_LD = MlpCfg<TM>::AS_LD, MLP_BS_FLOATS = MlpCfg<TM>::BS_FLOATS;
   constexpr int NCH = K / MLP_KC;
@@ -100,7 +109,7 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
   constexpr uint32_t CH_BYTES = MLP_KC * N * sizeof(float);
   constexpr int AS_FLOATS = MlpCfg<TM>::AS_FLOATS;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  const int rowbase = 64 * (w >> 3) + (lane >> 2), q = 4 * (w & 7) + (lane & 3);
+  const int rowbase = 64 * (w >> 3) + (lane >> 1), cgi = 2 * (w & 7) + (lane & 1);
 #pragma unroll
   for (int r = 0; r < R; ++r)
 #pragma unroll
@@ -110,10 +119,10 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
       tc::mbar_arrive_expect_tx(&P.full[buf], CH_BYTES);
       tc::bulk_g2s(P.Bs + buf * MLP_BS_FLOATS, Bg + (size_t)ch * MLP_KC * N, CH_BYTES, &P.full[buf]);
     }
-    if (A_GLOBAL) {                                      // TM rows x 4 granules
-      if (tid < GR * TM)
-        cp_async16(P.As + buf * AS_FLOATS + (tid / GR) * MLP_AS_LD + 4 * (tid % GR),
-                   A + (size_t)(tid / GR) * AEV_LEN + ch * MLP_KC + 4 * (tid % GR));
+    if (A_GLOBAL) {                                      // TM rows x GR granules
+      for (int t = tid; t < GR * TM; t += MlpCfg<TM>::THREADS)
+        cp_async16(P.As + buf * AS_FLOATS + (t / GR) * MLP_AS_LD + 4 * (t % GR),
+                   A + (size_t)(t / GR) * AEV_LEN + ch * MLP_KC + 4 * (t % GR));
       cp_async_commit();
     }
   };
@@ -130,7 +139,7 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
     const float* bs = P.Bs + buf * MLP_BS_FLOATS;
     const float* at = A_GLOBAL ? P.As + buf * AS_FLOATS + rowbase * MLP_AS_LD
                                : A + (size_t)rowbase * lda + ch * MLP_KC;
-    const int astr = 8 * (A_GLOBAL ? MLP_AS_LD : lda);
+    const int astr = 16 * (A_GLOBAL ? MLP_AS_LD : lda);
 #pragma unroll
     for (int k4 = 0; k4 < MLP_KC / 4; ++k4) {
       float4 a[R];
@@ -140,17 +149,14 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
       for (int j = 0; j < 4; ++j) {
         const float* brow = bs + (4 * k4 + j) * N;
         float b[NT];
-        if (NT == 5) {
-          const float4 v = *reinterpret_cast<const float4*>(brow + 4 * q);
-          b[0] = v.x; b[1] = v.y; b[2] = v.z; b[3] = v.w;
-          b[NT - 1] = brow[128 + q];
-        } else if (NT == 4) {
-          const float4 v = *reinterpret_cast<const float4*>(brow + 4 * q);
-          b[0] = v.x; b[1] = v.y; b[2] = v.z; b[3] = v.w;
-        } else {
-          const float2 v = *reinterpret_cast<const float2*>(brow + 2 * q);
-          b[0] = v.x; b[1] = v.y;
-          b[NT - 1] = brow[64 + q];
+#pragma unroll
+        for (int f = 0; f < NF4; ++f) {
+          const float4 v = *reinterpret_cast<const float4*>(brow + 64 * f + 4 * cgi);
+          b[4 * f] = v.x; b[4 * f + 1] = v.y; b[4 * f + 2] = v.z; b[4 * f + 3] = v.w;
+        }
+        if (HAS2) {
+          const float2 v = *reinterpret_cast<const float2*>(brow + 64 * NF4 + 2 * cgi);
+          b[NT - 2] = v.x; b[NT - 1] = v.y;
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -179,7 +185,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   pipe.gc = 0;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   constexpr int R = MlpCfg<TM>::R;
-  const int rowbase = 64 * (w >> 3) + (lane >> 2), q = 4 * (w & 7) + (lane & 3);
+  const int rowbase = 64 * (w >> 3) + (lane >> 1), cgi = 2 * (w & 7) + (lane & 1);
   const int row0 = blockIdx.x * TM;
   int el = 0;
 #pragma unroll
@@ -197,35 +203,35 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
 
   // ---- forward ----
   {
-    constexpr int NT = D1 / 32;
+    constexpr int NT = D1 / 16;
     float acc[R][NT];
     mlp_gemm<TM, D0, D1, true>(pipe, aev + (size_t)row0 * AEV_LEN, 0, Wp + MLP_P_OFF0, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
-        const int n = mlp_col<NT>(q, c);
+        const int n = mlp_col<D1>(cgi, c);
         const float bias = __ldg(V + MLP_V_B1 + n);
 #pragma unroll
-        for (int r = 0; r < R; ++r) H1[(rowbase + 8 * r) * MLP_LD1 + n] = celu_f(acc[r][c] + bias);
+        for (int r = 0; r < R; ++r) H1[(rowbase + 16 * r) * MLP_LD1 + n] = celu_f(acc[r][c] + bias);
       }
     }
   }
   {
-    constexpr int NT = D2 / 32;
+    constexpr int NT = D2 / 16;
     float acc[R][NT];
     mlp_gemm<TM, D1, D2, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF1, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
-        const int n = mlp_col<NT>(q, c);
+        const int n = mlp_col<D2>(cgi, c);
         const float bias = __ldg(V + MLP_V_B2 + n);
 #pragma unroll
-        for (int r = 0; r < R; ++r) H2[(rowbase + 8 * r) * MLP_LD2 + n] = celu_f(acc[r][c] + bias);
+        for (int r = 0; r < R; ++r) H2[(rowbase + 16 * r) * MLP_LD2 + n] = celu_f(acc[r][c] + bias);
       }
     }
   }
   {
-    constexpr int NT = D3 / 32;
+    constexpr int NT = D3 / 16;
     float acc[R][NT];
     mlp_gemm<TM, D2, D3, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF2, active, acc);
     float part[R];
@@ -234,23 +240,22 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
-        const int n = mlp_col<NT>(q, c);
+        const int n = mlp_col<D3>(cgi, c);
         const float bias = __ldg(V + MLP_V_B3 + n), w4 = __ldg(V + MLP_V_W4 + n);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
           const float h = celu_f(acc[r][c] + bias);
           part[r] = fmaf(w4, h, part[r]);
-          H3[(rowbase + 8 * r) * MLP_LD3 + n] = w4 * dcelu_from_h(h);   // delta3 = dE/dz3
+          H3[(rowbase + 16 * r) * MLP_LD3 + n] = w4 * dcelu_from_h(h);   // delta3 = dE/dz3
         }
       }
     }
-    // e_i = b4 + sum over the 96 columns: 4 lanes (xor tree), then the 8 column groups in order
+    // e_i = b4 + sum over the 96 columns: 2 lanes, then the 8 warps' column groups in a fixed tree
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       float s = part[r];
       s += __shfl_xor_sync(0xffffffffu, s, 1);
-      s += __shfl_xor_sync(0xffffffffu, s, 2);
-      if ((lane & 3) == 0) esum[(rowbase + 8 * r) * 8 + (w & 7)] = s;
+      if ((lane & 1) == 0) esum[(rowbase + 16 * r) * 8 + (w & 7)] = s;
     }
     __syncthreads();
     if (tid < TM && row0 + tid < P.row_end[el]) {
@@ -260,7 +265,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   }
   // ---- backward (input gradient only) ----
   {
-    constexpr int NT = D2 / 32;
+    constexpr int NT = D2 / 16;
     float acc[R][NT];
     mlp_gemm<TM, D3, D2, false>(pipe, H3, MLP_LD3, Wp + MLP_P_OFF3, active, acc);
     if (active) {
@@ -268,13 +273,13 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
       for (int c = 0; c < NT; ++c)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-          float* hp = H2 + (rowbase + 8 * r) * MLP_LD2 + mlp_col<NT>(q, c);
+          float* hp = H2 + (rowbase + 16 * r) * MLP_LD2 + mlp_col<D2>(cgi, c);
           *hp = acc[r][c] * dcelu_from_h(*hp);          // delta2 over h2 (own elements only)
         }
     }
   }
   {
-    constexpr int NT = D1 / 32;
+    constexpr int NT = D1 / 16;
     float acc[R][NT];
     mlp_gemm<TM, D2, D1, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF4, active, acc);
     if (active) {
@@ -282,20 +287,21 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
       for (int c = 0; c < NT; ++c)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-          float* hp = H1 + (rowbase + 8 * r) * MLP_LD1 + mlp_col<NT>(q, c);
+          float* hp = H1 + (rowbase + 16 * r) * MLP_LD1 + mlp_col<D1>(cgi, c);
           *hp = acc[r][c] * dcelu_from_h(*hp);          // delta1
         }
     }
   }
 #pragma unroll 1
   for (int pass = 0; pass < D0 / 128; ++pass) {
-    float acc[R][4];
+    float acc[R][8];
     mlp_gemm<TM, D1, 128, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF5 + pass * D1 * 128, active, acc);
     if (active) {
 #pragma unroll
       for (int r = 0; r < R; ++r) {
-        float* dst = g + (size_t)(row0 + rowbase + 8 * r) * AEV_LEN + pass * 128 + 4 * q;
+        float* dst = g + (size_t)(row0 + rowbase + 16 * r) * AEV_LEN + pass * 128 + 4 * cgi;
         *reinterpret_cast<float4*>(dst) = make_float4(acc[r][0], acc[r][1], acc[r][2], acc[r][3]);
+        *reinterpret_cast<float4*>(dst + 64) = make_float4(acc[r][4], acc[r][5], acc[r][6], acc[r][7]);
       }
     }
   }
