@@ -70,14 +70,6 @@ __device__ __forceinline__ float dcelu_from_h(float h) {
   return h > 0.0f ? 1.0f : fmaf(h, 1.0f / CELU_ALPHA, 1.0f);
 }
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-  uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
-
 struct MlpPipe {               // shared-memory staging state, uniform across the CTA
   float* Bs;                   // [2][MLP_BS_FLOATS]
   float* As;                   // [2][AS_FLOATS]  (phase 0 only)
