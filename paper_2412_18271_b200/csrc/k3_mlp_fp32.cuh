@@ -32,16 +32,25 @@
 namespace pfc {
 
 constexpr int MLP_LD1 = D1 + 4, MLP_LD2 = D2 + 4, MLP_LD3 = D3 + 4;   // row strides (floats): 4 mod 32
-template <int TM> struct MlpCfg {                                     // TM = 16, 32, 64 or 128 rows per tile
+// DEEP = false: two staging buffers, one CTA barrier per chunk -- best when several CTAs share an
+// SM and hide each other's chunk latency (configs 3 and 4).  DEEP = true: an 8-stage ring guarded
+// by full / empty mbarriers with six chunks (60 KB) in flight and no CTA barrier inside a phase --
+// for batches of a few tiles per SM, where a tile's time is otherwise 86 chunks x the L2 latency.
+template <int TM, bool DEEP = false> struct MlpCfg {                  // TM = 16, 32, 64 or 128 rows per tile
   static constexpr int THREADS = TM >= 64 ? 4 * TM : 256;             // 8 warps per (up to) 64 rows
+  static constexpr int WARPS = THREADS / 32;
   static constexpr int R = TM >= 64 ? 4 : TM / 16;                    // rows per thread
   static constexpr int KC = TM == 64 ? 8 : 16;                        // k per staged chunk (64: two CTAs per SM)
+  static constexpr int S = DEEP ? 8 : 2;                              // staging buffers
+  static constexpr int LEAD = DEEP ? 6 : 1;                           // chunks issued ahead of the consumers
   static constexpr int AS_LD = KC + 4;                                // AEV chunk row stride: 4 mod 8 floats
   static constexpr int AS_FLOATS = TM * AS_LD;                        // one AEV chunk [TM][KC+4]
   static constexpr int BS_FLOATS = KC * D1;                           // one weight buffer (widest N = 160)
   static constexpr size_t SMEM = sizeof(float) * ((size_t)TM * (MLP_LD1 + MLP_LD2 + MLP_LD3) +
-                                                  2 * BS_FLOATS + (size_t)TM * 8) + 64;
-  static_assert(2 * AS_FLOATS <= TM * MLP_LD2, "AEV chunks live in the h2 region during phase 0");
+                                                  S * BS_FLOATS + (size_t)TM * 8) + 3 * S * 8 + 64;
+  static_assert(S * AS_FLOATS <= TM * (MLP_LD2 + MLP_LD3), "AEV chunks live in the h2 + h3 regions during phase 0");
+  static_assert((D0 / KC) % S == 0, "phase 0 ends on a ring boundary (full / fullA parity bookkeeping)");
+  static_assert(!DEEP || TM <= 32, "the deep ring is for small tiles");
 };
 
 // weight image per element (floats): phases 0..5, each B[K][N] row-major
@@ -70,11 +79,25 @@ __device__ __forceinline__ float dcelu_from_h(float h) {
   return h > 0.0f ? 1.0f : fmaf(h, 1.0f / CELU_ALPHA, 1.0f);
 }
 
-struct MlpPipe {               // shared-memory staging state, uniform across the CTA
-  float* Bs;                   // [2][MLP_BS_FLOATS]
-  float* As;                   // [2][AS_FLOATS]  (phase 0 only)
-  uint64_t* full;              // [2] mbarriers: weight chunk landed
-  uint32_t gc;                 // chunks consumed so far (buffer = gc & 1, parity = (gc >> 1) & 1)
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint64_t* bar) {   // arrives when my cp.asyncs landed
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(tc::smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(tc::smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+
+// Shared-memory staging state, uniform across the CTA.  Chunk g (counted over the whole tile)
+// uses buffer g % S.  full[st] (count 1: the TMA issuer) completes when the weight chunk has landed.
+// Deep ring only: fullA[st] (count THREADS: every thread's cp.async granules of the AEV chunk,
+// phase 0) and empty[st] (count WARPS: every warp has finished reading the buffer); a chunk is
+// issued LEAD = S - 2 chunks ahead, into the buffer released two chunks ago, so warps may drift
+// one chunk apart without stalling.
+struct MlpPipe {
+  float* Bs;                   // [S][BS_FLOATS]
+  float* As;                   // [S][AS_FLOATS]  (phase 0 only)
+  uint64_t *full, *fullA, *empty;
+  uint32_t gc;                 // chunks consumed so far
 };
 
 // column c (< N/16) of the thread with column slot cgi (< 16)
@@ -87,49 +110,48 @@ __device__ __forceinline__ int mlp_col(int cgi, int c) {
 // acc[r][c] = sum_k A[rowbase + 16r][k] * B[k][mlp_col<N>(cgi, c)],  k < K, r < R,  rowbase = 64*half + rg.
 // A_GLOBAL: A is the AEV tile in global memory (row stride AEV_LEN), streamed; else A is a
 // row-major shared-memory activation with row stride lda.
-template <int TM, int K, int N, bool A_GLOBAL>
+template <int TM, bool DEEP, int K, int N, bool A_GLOBAL>
 __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A, int lda,
                                          const float* __restrict__ Bg, bool active,
-                                         float (&acc)[MlpCfg<TM>::R][N / 16]) {
+                                         float (&acc)[MlpCfg<TM, DEEP>::R][N / 16]) {
+  using Cfg = MlpCfg<TM, DEEP>;
   constexpr int NT = N / 16;
   constexpr int NF4 = N / 64;                            // float4 column groups per thread
   constexpr bool HAS2 = (N % 64) == 32;                  // plus one float2 group (N = 160, 96)
-  constexpr int R = MlpCfg<TM>::R;
-  constexpr int MLP_KC = MlpCfg<TM>::KC, MLP_AS_LD = MlpCfg<TM>::AS_LD, MLP_BS_FLOATS = MlpCfg<TM>::BS_FLOATS;
+  constexpr int R = Cfg::R, S = Cfg::S, LEAD = Cfg::LEAD;
+  constexpr int MLP_KC = Cfg::KC, MLP_AS_LD = Cfg::AS_LD, MLP_BS_FLOATS = Cfg::BS_FLOATS;
   constexpr int NCH = K / MLP_KC;
   constexpr int GR = MLP_KC / 4;                         // 16-byte granules per AEV chunk row
   constexpr uint32_t CH_BYTES = MLP_KC * N * sizeof(float);
-  constexpr int AS_FLOATS = MlpCfg<TM>::AS_FLOATS;
+  constexpr int AS_FLOATS = Cfg::AS_FLOATS;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const int rowbase = 64 * (w >> 3) + (lane >> 1), cgi = 2 * (w & 7) + (lane & 1);
 #pragma unroll
   for (int r = 0; r < R; ++r)
 #pragma unroll
     for (int c = 0; c < NT; ++c) acc[r][c] = 0.0f;
-  auto issue = [&](int ch, uint32_t buf) {
+  // the deep ring signals an AEV chunk through fullA (every thread's granules), a weight-only chunk
+  // through full; the two-buffer pipeline uses full + cp.async.wait_group + the CTA barrier
+  uint64_t* fullb = (DEEP && A_GLOBAL) ? P.fullA : P.full;
+  constexpr uint32_t BASE = (DEEP && !A_GLOBAL) ? D0 / MLP_KC : 0;   // chunks before this barrier set's first use
+  auto issue = [&](int ch, uint32_t gch) {               // chunk ch of this phase = chunk gch of the tile
+    const uint32_t st = gch % S;
     if (tid == 0) {
-      tc::mbar_arrive_expect_tx(&P.full[buf], CH_BYTES);
-      tc::bulk_g2s(P.Bs + buf * MLP_BS_FLOATS, Bg + (size_t)ch * MLP_KC * N, CH_BYTES, &P.full[buf]);
+      if (DEEP && A_GLOBAL) mbar_expect_tx(&fullb[st], CH_BYTES);
+      else tc::mbar_arrive_expect_tx(&fullb[st], CH_BYTES);
+      tc::bulk_g2s(P.Bs + st * MLP_BS_FLOATS, Bg + (size_t)ch * MLP_KC * N, CH_BYTES, &fullb[st]);
     }
     if (A_GLOBAL) {                                      // TM rows x GR granules
-      for (int t = tid; t < GR * TM; t += MlpCfg<TM>::THREADS)
-        cp_async16(P.As + buf * AS_FLOATS + (t / GR) * MLP_AS_LD + 4 * (t % GR),
+      for (int t = tid; t < GR * TM; t += Cfg::THREADS)
+        cp_async16(P.As + st * AS_FLOATS + (t / GR) * MLP_AS_LD + 4 * (t % GR),
                    A + (size_t)(t / GR) * AEV_LEN + ch * MLP_KC + 4 * (t % GR));
-      cp_async_commit();
+      if (DEEP) cp_async_mbar_arrive_noinc(&fullb[st]);
+      else cp_async_commit();
     }
   };
-  __syncthreads();                  // previous phase: activation stores visible, staging buffers free
-  issue(0, P.gc & 1u);
-  for (int ch = 0; ch < NCH; ++ch) {
-    const uint32_t buf = P.gc & 1u;
-    if (A_GLOBAL) cp_async_wait<0>();
-    tc::mbar_wait(&P.full[buf], (P.gc >> 1) & 1u);
-    __syncthreads();                // all A granules visible; the other buffer is no longer read
-    if (ch + 1 < NCH) issue(ch + 1, buf ^ 1u);
-    ++P.gc;
-    if (!active) continue;
-    const float* bs = P.Bs + buf * MLP_BS_FLOATS;
-    const float* at = A_GLOBAL ? P.As + buf * AS_FLOATS + rowbase * MLP_AS_LD
+  auto compute = [&](int ch, uint32_t st) {
+    const float* bs = P.Bs + st * MLP_BS_FLOATS;
+    const float* at = A_GLOBAL ? P.As + st * AS_FLOATS + rowbase * MLP_AS_LD
                                : A + (size_t)rowbase * lda + ch * MLP_KC;
     const int astr = 16 * (A_GLOBAL ? MLP_AS_LD : lda);
 #pragma unroll
@@ -158,25 +180,60 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
         }
       }
     }
+  };
+  __syncthreads();                  // previous phase: activation stores visible, every staging buffer released
+  if constexpr (!DEEP) {
+    issue(0, P.gc);
+    for (int ch = 0; ch < NCH; ++ch) {
+      const uint32_t st = P.gc & 1u;
+      if (A_GLOBAL) cp_async_wait<0>();
+      tc::mbar_wait(&P.full[st], (P.gc >> 1) & 1u);
+      __syncthreads();              // all A granules visible; the other buffer is no longer read
+      if (ch + 1 < NCH) issue(ch + 1, P.gc + 1);
+      ++P.gc;
+      if (active) compute(ch, st);
+    }
+  } else {
+#pragma unroll
+    for (int c = 0; c < LEAD && c < NCH; ++c) issue(c, P.gc + c);
+#pragma unroll 1
+    for (int ch = 0; ch < NCH; ++ch) {
+      const uint32_t gch = P.gc, st = gch % S;
+      if (ch + LEAD < NCH) {
+        if (ch >= S - LEAD) {       // the target buffer was last read as chunk gch + LEAD - S of this phase
+          const uint32_t gp = gch + LEAD - S;
+          tc::mbar_wait(&P.empty[gp % S], (gp / S) & 1u);
+        }
+        issue(ch + LEAD, gch + LEAD);
+      }
+      tc::mbar_wait(&fullb[st], ((gch - BASE) / S) & 1u);
+      ++P.gc;
+      if (active) compute(ch, st);
+      __syncwarp();                 // every lane's reads of this buffer are done
+      if (lane == 0) tc::mbar_arrive(&P.empty[st]);
+    }
   }
 }
 
-template <int TM>
-__global__ void __launch_bounds__(MlpCfg<TM>::THREADS, TM == 64 ? 2 : 1)
+template <int TM, bool DEEP>
+__global__ void __launch_bounds__(MlpCfg<TM, DEEP>::THREADS, TM == 64 ? 2 : 1)
 k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict__ aev,
                    float* __restrict__ g, float* __restrict__ e_row) {
   extern __shared__ __align__(16) float smem[];
   float* H1 = smem;                                   // [TM][LD1]  h1, later delta1
-  float* H2 = H1 + TM * MLP_LD1;                      // [TM][LD2]  h2, later delta2 (phase 0: AEV chunks)
+  float* H2 = H1 + TM * MLP_LD1;                      // [TM][LD2]  h2, later delta2 (phase 0: AEV chunks, into h3)
   float* H3 = H2 + TM * MLP_LD2;                      // [TM][LD3]  delta3
+  using Cfg = MlpCfg<TM, DEEP>;
   MlpPipe pipe;
   pipe.Bs = H3 + TM * MLP_LD3;
   pipe.As = H2;
-  float* esum = pipe.Bs + 2 * MlpCfg<TM>::BS_FLOATS;          // [TM][8] partial energies per column group
+  float* esum = pipe.Bs + Cfg::S * Cfg::BS_FLOATS;    // [TM][8] partial energies per column group
   pipe.full = reinterpret_cast<uint64_t*>(esum + TM * 8);
+  pipe.fullA = pipe.full + Cfg::S;
+  pipe.empty = pipe.fullA + Cfg::S;
   pipe.gc = 0;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  constexpr int R = MlpCfg<TM>::R;
+  constexpr int R = Cfg::R;
   const int rowbase = 64 * (w >> 3) + (lane >> 1), cgi = 2 * (w & 7) + (lane & 1);
   const int row0 = blockIdx.x * TM;
   int el = 0;
@@ -187,8 +244,11 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   if (row0 >= P.row_end[el]) return;                  // a tile of padding only (CTA-uniform)
   const bool active = row0 + 64 * (w >> 3) < P.row_end[el];   // warp-uniform: my 64 rows hold an atom
   if (tid == 0) {
-    tc::mbar_init(&pipe.full[0], 1);
-    tc::mbar_init(&pipe.full[1], 1);
+    for (int st = 0; st < Cfg::S; ++st) {
+      tc::mbar_init(&pipe.full[st], 1);
+      tc::mbar_init(&pipe.fullA[st], Cfg::THREADS);
+      tc::mbar_init(&pipe.empty[st], Cfg::WARPS);
+    }
     tc::mbar_fence_init();
   }
   // (the first __syncthreads of mlp_gemm orders the init before any use)
@@ -197,7 +257,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   {
     constexpr int NT = D1 / 16;
     float acc[R][NT];
-    mlp_gemm<TM, D0, D1, true>(pipe, aev + (size_t)row0 * AEV_LEN, 0, Wp + MLP_P_OFF0, active, acc);
+    mlp_gemm<TM, DEEP, D0, D1, true>(pipe, aev + (size_t)row0 * AEV_LEN, 0, Wp + MLP_P_OFF0, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
@@ -211,7 +271,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   {
     constexpr int NT = D2 / 16;
     float acc[R][NT];
-    mlp_gemm<TM, D1, D2, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF1, active, acc);
+    mlp_gemm<TM, DEEP, D1, D2, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF1, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
@@ -225,7 +285,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   {
     constexpr int NT = D3 / 16;
     float acc[R][NT];
-    mlp_gemm<TM, D2, D3, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF2, active, acc);
+    mlp_gemm<TM, DEEP, D2, D3, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF2, active, acc);
     float part[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) part[r] = 0.0f;
@@ -259,7 +319,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   {
     constexpr int NT = D2 / 16;
     float acc[R][NT];
-    mlp_gemm<TM, D3, D2, false>(pipe, H3, MLP_LD3, Wp + MLP_P_OFF3, active, acc);
+    mlp_gemm<TM, DEEP, D3, D2, false>(pipe, H3, MLP_LD3, Wp + MLP_P_OFF3, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c)
@@ -273,7 +333,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   {
     constexpr int NT = D1 / 16;
     float acc[R][NT];
-    mlp_gemm<TM, D2, D1, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF4, active, acc);
+    mlp_gemm<TM, DEEP, D2, D1, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF4, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c)
@@ -287,7 +347,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
 #pragma unroll 1
   for (int pass = 0; pass < D0 / 128; ++pass) {
     float acc[R][8];
-    mlp_gemm<TM, D1, 128, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF5 + pass * D1 * 128, active, acc);
+    mlp_gemm<TM, DEEP, D1, 128, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF5 + pass * D1 * 128, active, acc);
     if (active) {
 #pragma unroll
       for (int r = 0; r < R; ++r) {

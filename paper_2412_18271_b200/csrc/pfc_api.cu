@@ -148,6 +148,7 @@ struct pfc_ctx {
   TcParams tcp;
   int mlp_path;
   int mlp_tm = 128;             // FFMA K3 tile height
+  bool mlp_deep = false;        // FFMA K3 staging: 8-stage mbarrier ring (few tiles per SM) or two buffers
   int n_sms = 148;
   int n_cell_sys, n_cell_atoms;
   int launches_ef, launches_step;
@@ -215,16 +216,20 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
          b.row_of_atom, b.aev, b.status);
   mark(2);
   if (c->mlp_path == PFC_MLP_FP32) {
-    switch (c->mlp_tm) {                                 // tile height chosen by pfc_create
-      case 128: LAUNCH(c, k3_mlp_fp32_kernel<128>, s.n_rows / 128, MlpCfg<128>::THREADS, MlpCfg<128>::SMEM, st,
-                       c->mlp, b.aev, b.g, b.e_row); break;
-      case 64:  LAUNCH(c, k3_mlp_fp32_kernel<64>, s.n_rows / 64, MlpCfg<64>::THREADS, MlpCfg<64>::SMEM, st,
-                       c->mlp, b.aev, b.g, b.e_row); break;
-      case 32:  LAUNCH(c, k3_mlp_fp32_kernel<32>, s.n_rows / 32, MlpCfg<32>::THREADS, MlpCfg<32>::SMEM, st,
-                       c->mlp, b.aev, b.g, b.e_row); break;
-      default:  LAUNCH(c, k3_mlp_fp32_kernel<16>, s.n_rows / 16, MlpCfg<16>::THREADS, MlpCfg<16>::SMEM, st,
-                       c->mlp, b.aev, b.g, b.e_row); break;
+#define K3_LAUNCH(TM_, DEEP_)                                                                          \
+  LAUNCH(c, (k3_mlp_fp32_kernel<TM_, DEEP_>), s.n_rows / TM_, (MlpCfg<TM_, DEEP_>::THREADS),             \
+         (MlpCfg<TM_, DEEP_>::SMEM), st, c->mlp, b.aev, b.g, b.e_row)
+    if (c->mlp_deep) {                                   // tile height and staging chosen by pfc_create
+      if (c->mlp_tm == 32) K3_LAUNCH(32, true); else K3_LAUNCH(16, true);
+    } else {
+      switch (c->mlp_tm) {
+        case 128: K3_LAUNCH(128, false); break;
+        case 64:  K3_LAUNCH(64, false); break;
+        case 32:  K3_LAUNCH(32, false); break;
+        default:  K3_LAUNCH(16, false); break;
+      }
     }
+#undef K3_LAUNCH
   } else {
     const int grid = c->tcp.n_tiles < c->n_sms ? c->tcp.n_tiles : c->n_sms;   // persistent: one CTA per SM
     if (c->mlp_path == PFC_MLP_TF32X3)
@@ -464,14 +469,12 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (cudaMemset(b.aev, 0, sizeof(float) * (size_t)c->sz.n_rows * AEV_LEN) != cudaSuccess) ok = false;
   if (cudaMemset(b.status, 0, 256) != cudaSuccess) ok = false;
   if (cudaMemset(b.xlo, 0, sizeof(float4) * N) != cudaSuccess) ok = false;
-  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)MlpCfg<128>::SMEM) != cudaSuccess) ok = false;
-  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)MlpCfg<64>::SMEM) != cudaSuccess) ok = false;
-  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)MlpCfg<32>::SMEM) != cudaSuccess) ok = false;
-  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                           (int)MlpCfg<16>::SMEM) != cudaSuccess) ok = false;
+#define K3_SMEM_ATTR(TM_, DEEP_)                                                                       \
+  if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<TM_, DEEP_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                           (int)MlpCfg<TM_, DEEP_>::SMEM) != cudaSuccess) ok = false
+  K3_SMEM_ATTR(128, false); K3_SMEM_ATTR(64, false); K3_SMEM_ATTR(32, false); K3_SMEM_ATTR(16, false);
+  K3_SMEM_ATTR(32, true); K3_SMEM_ATTR(16, true);
+#undef K3_SMEM_ATTR
   if (cudaFuncSetAttribute(k3_mlp_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)TC_SMEM_BYTES) != cudaSuccess) ok = false;
   if (cudaFuncSetAttribute(k3_mlp_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -483,17 +486,21 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
       c->n_sms = sms;
   }
   {
-    // FFMA K3 tile height.  Measured on B200 (config 4, K3 alone): 32-row tiles, three CTAs per SM,
-    // 2.14 ms; 64 rows, two CTAs per SM, 2.16 ms; 128 rows, one CTA, 2.22 ms -- and on config 3
-    // 0.23 / 0.28 / 0.35 ms: co-resident small tiles hide the per-chunk latency best and quantise
-    // the grid finest.  A batch that cannot give every SM a 32-row tile uses 16-row tiles (a lone
-    // 16-row tile takes 50 us, a 64-row one 99 us).  PFC_K3_TM overrides (tuning only).
+    // FFMA K3 tile height and staging.  Measured on B200 (K3 alone): config 4, 32-row tiles, three
+    // CTAs per SM, 2.11 ms; 64 rows, two CTAs per SM, 2.22 ms; 128 rows, one CTA, 2.17 ms -- and on
+    // config 3 0.23 / 0.29 / 0.34 ms: co-resident small tiles hide the per-chunk latency best and
+    // quantise the grid finest.  A batch that cannot give every SM a 32-row tile uses 16-row tiles
+    // with the deep staging ring (config 0: 47 -> 43 us, config 2: 49 -> 45 us against two buffers;
+    // with several CTAs per SM the ring is slower: config 4 2.52 ms, config 3 0.27 ms).
+    // PFC_K3_TM / PFC_K3_DEEP override (tuning only).
     auto tiles = [&](int tm) { int n = 0; for (int e = 0; e < NSPEC; ++e) n += (count[e] + tm - 1) / tm; return n; };
     c->mlp_tm = tiles(32) >= c->n_sms ? 32 : 16;
+    c->mlp_deep = c->mlp_tm == 16;
     if (const char* ov = getenv("PFC_K3_TM")) {
       const int v = atoi(ov);
       if (v == 16 || v == 32 || v == 64 || v == 128) c->mlp_tm = v;
     }
+    if (const char* ov = getenv("PFC_K3_DEEP")) c->mlp_deep = atoi(ov) != 0 && c->mlp_tm <= 32;
   }
   if (cudaDeviceSynchronize() != cudaSuccess) ok = false;
   if (!ok) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
