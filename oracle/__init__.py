@@ -181,3 +181,52 @@ def step(pos, vel, species, sys_offsets, weights, dt, n_steps, cell: bool = Fals
                           _p(F, c_double), _p(pe, c_double), _p(ke, c_double))
     assert rc == 0
     return {"pos": pos, "vel": vel, "F": F, "pe": pe, "ke": ke}
+
+
+def philox4x32_10(ctr, key):
+    """Philox4x32-10 block (O9 / reading S28): ctr[4], key[2] uint32 -> 4 uint32."""
+    from ctypes import c_uint32
+    L = _L()
+    c = np.ascontiguousarray(ctr, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    L.oracle_philox4x32_10.restype = None
+    L.oracle_philox4x32_10(_p(c, c_uint32), _p(k, c_uint32), _p(out, c_uint32))
+    return out
+
+
+def langevin_normals(atom: int, step: int, seed: int):
+    """The three standard normals of (atom, step) (O9)."""
+    from ctypes import c_uint32, c_uint64
+    L = _L()
+    xi = np.zeros(3)
+    L.oracle_langevin_normals.restype = None
+    L.oracle_langevin_normals.argtypes = [c_uint32, c_uint32, c_uint64, ctypes.POINTER(c_double)]
+    L.oracle_langevin_normals(int(atom), int(step), int(seed), _p(xi, c_double))
+    return xi
+
+
+def step_langevin(pos, vel, species, sys_offsets, weights, dt, n_steps, gamma, temperature, seed,
+                  step0: int = 0, cell: bool = False, masses=None, free: bool = False):
+    """O9: n_steps of BAOAB Langevin dynamics.  free=True drops the forces (pins).
+    Returns dict(pos, vel, F)."""
+    from ctypes import c_uint32, c_uint64
+    pos = np.array(pos, dtype=np.float64, order="C", copy=True)
+    vel = np.array(vel, dtype=np.float64, order="C", copy=True)
+    spc, off = _i32(species), _i32(sys_offsets)
+    n, ns = pos.shape[0], off.shape[0] - 1
+    m = np.ascontiguousarray(MASSES_AMU if masses is None else masses, dtype=np.float64)
+    w = np.ascontiguousarray(weights if weights is not None else np.zeros(1), dtype=np.float32)
+    F = np.zeros((n, 3))
+    L = _L()
+    L.oracle_step_langevin.restype = c_int
+    L.oracle_step_langevin.argtypes = [c_int, c_int, ctypes.POINTER(c_int32), ctypes.POINTER(c_double),
+                                       ctypes.POINTER(c_double), ctypes.POINTER(c_int32),
+                                       ctypes.POINTER(c_float), ctypes.POINTER(c_double), c_double, c_int, c_int,
+                                       c_int, c_double, c_double, c_uint64, c_uint32, ctypes.POINTER(c_double)]
+    rc = L.oracle_step_langevin(n, ns, _p(off, c_int32), _p(pos, c_double), _p(vel, c_double), _p(spc, c_int32),
+                                _p(w, c_float), _p(m, c_double), float(dt), int(n_steps), int(cell),
+                                2 if free else 0, float(gamma), float(temperature), int(seed), int(step0),
+                                _p(F, c_double))
+    assert rc == 0
+    return {"pos": pos, "vel": vel, "F": F}

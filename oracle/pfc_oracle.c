@@ -581,3 +581,76 @@ int oracle_step(int n_atoms, int n_sys, const int32_t *sys_off, double *pos, dou
     free(F); free(E);
     return 0;
 }
+
+/* ---- O9: Langevin dynamics (the paper's timing protocol, PAPER.md:94:
+ * "Langevin integrator, friction 0.1 ps^-1").  The paper names no splitting; reading S27 takes
+ * BAOAB (Leimkuhler & Matthews) built on the O8 kicks:
+ *   B: v += dt/2 a(x)      A: x += dt/2 v
+ *   O: v = c1 v + c2 sqrt(kB T ACC / m) xi,  c1 = exp(-gamma dt), c2 = sqrt(1 - c1^2)
+ *   A: x += dt/2 v         F(x)         B: v += dt/2 a(x)
+ * gamma = 0 gives c1 = 1, c2 = 0: velocity-Verlet.  The normals xi are NOT drawn here from a
+ * library stream: both sides implement the same counter-based generator (reading S28):
+ * Philox4x32-10 (Salmon et al., SC'11) with counter (atom, step, 0, 0), key (seed_lo, seed_hi);
+ * u = ((word >> 8) + 0.5) 2^-24; Box-Muller: xi_x = r cos(2 pi u1), xi_y = r sin(2 pi u1) with
+ * r = sqrt(-2 ln u0) from words 0,1; xi_z = sqrt(-2 ln u2) cos(2 pi u3) from words 2,3. */
+static const double KB_EV = 8.617333262e-5;      /* eV/K */
+
+static void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+void oracle_philox4x32_10(const uint32_t *ctr, const uint32_t *key, uint32_t *out) { philox4x32_10(ctr, key, out); }
+
+/* the three standard normals of (atom, step) */
+void oracle_langevin_normals(uint32_t atom, uint32_t step, uint64_t seed, double xi[3]) {
+    uint32_t ctr[4] = {atom, step, 0u, 0u}, key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)}, w[4];
+    philox4x32_10(ctr, key, w);
+    double u[4];
+    for (int q = 0; q < 4; ++q) u[q] = ((double)(w[q] >> 8) + 0.5) * (1.0 / 16777216.0);
+    double r = sqrt(-2.0 * log(u[0]));
+    xi[0] = r * cos(2.0 * PI * u[1]);
+    xi[1] = r * sin(2.0 * PI * u[1]);
+    xi[2] = sqrt(-2.0 * log(u[2])) * cos(2.0 * PI * u[3]);
+}
+
+/* n_steps of BAOAB; step indices step0+1 .. step0+n_steps feed the generator.  potential_kind 2 = no
+ * forces (free particles: the O step alone thermalises, used by the pins). */
+int oracle_step_langevin(int n_atoms, int n_sys, const int32_t *sys_off, double *pos, double *vel,
+                         const int32_t *species, const float *weights, const double *masses,
+                         double dt, int n_steps, int nbr_mode, int potential_kind,
+                         double gamma, double temperature, uint64_t seed, uint32_t step0, double *F_out) {
+    double *F = (double *)calloc(3 * (size_t)n_atoms, sizeof(double));
+    double *E = (double *)malloc(sizeof(double) * (size_t)n_sys);
+    const double c1 = exp(-gamma * dt), c2 = sqrt(1.0 - c1 * c1);
+    if (potential_kind == 0)
+        oracle_energy_forces(n_atoms, n_sys, sys_off, pos, species, weights, nbr_mode, E, F, NULL, NULL, NULL);
+    for (int step = 1; step <= n_steps; ++step) {
+        for (int i = 0; i < n_atoms; ++i) {
+            double im = ACC / masses[species[i]], xi[3];
+            double sigma = sqrt(KB_EV * temperature * im);
+            oracle_langevin_normals((uint32_t)i, step0 + (uint32_t)step, seed, xi);
+            for (int c = 0; c < 3; ++c) {
+                vel[3 * i + c] += 0.5 * dt * F[3 * i + c] * im;          /* B */
+                pos[3 * i + c] += 0.5 * dt * vel[3 * i + c];             /* A */
+                vel[3 * i + c] = c1 * vel[3 * i + c] + c2 * sigma * xi[c];   /* O */
+                pos[3 * i + c] += 0.5 * dt * vel[3 * i + c];             /* A */
+            }
+        }
+        if (potential_kind == 0)
+            oracle_energy_forces(n_atoms, n_sys, sys_off, pos, species, weights, nbr_mode, E, F, NULL, NULL, NULL);
+        for (int i = 0; i < n_atoms; ++i) {
+            double im = ACC / masses[species[i]];
+            for (int c = 0; c < 3; ++c) vel[3 * i + c] += 0.5 * dt * F[3 * i + c] * im;   /* B */
+        }
+    }
+    if (F_out) memcpy(F_out, F, sizeof(double) * 3 * (size_t)n_atoms);
+    free(F); free(E);
+    return 0;
+}
