@@ -123,6 +123,28 @@ int pfc_set_state(pfc_t *ctx, float *pos, float *vel, float *E, float *F, void *
  * the stream) pos, vel, F, E hold the synchronous (x_n, v_n, F(x_n), E(x_n)). */
 int pfc_step(pfc_t *ctx, int32_t n_steps, float dt_fs);
 
+/* n_steps of Langevin dynamics on the bound state (the paper's timing
+ * protocol is a Langevin integrator with friction 0.1 ps^-1; O9, readings
+ * S27/S28): BAOAB on the velocity-Verlet kicks,
+ *   v += dt/2 a;  x += dt/2 v;  v = c1 v + c2 sqrt(kB T ACC/m) xi;  x += dt/2 v;  forces;  v += dt/2 a,
+ * c1 = exp(-friction dt), c2 = sqrt(1 - c1^2).  friction_per_fs in fs^-1 (0.1 ps^-1 = 1e-4),
+ * temperature_K in kelvin.  xi are standard normals from Philox4x32-10 with counter
+ * (global atom index, step index, 0, 0) and key = seed, Box-Muller in fp32; the step index counts
+ * Langevin steps since pfc_set_state, starting at 1, and lives in device memory, so a step is one
+ * replayed CUDA graph like pfc_step.  friction 0 reproduces pfc_step up to rounding.
+ * Same asynchrony, state and error conventions as pfc_step. */
+int pfc_step_langevin(pfc_t *ctx, int32_t n_steps, float dt_fs, float friction_per_fs,
+                      float temperature_K, uint64_t seed);
+
+/* Trajectory frames (the paper's protocol writes 10 frames per 1000 steps): binds
+ * frames DEVICE [max_frames][n_atoms] float4 (caller-owned; NULL unbinds).  Every later pfc_step /
+ * pfc_step_langevin call copies the positions after each stride-th step (counted since
+ * pfc_set_state) into the next frame, device to device on the bound stream, until max_frames are
+ * written.  pfc_frames_written returns the count (host bookkeeping; sync the stream before reading
+ * the frames). */
+int pfc_set_frames(pfc_t *ctx, float *frames, int32_t stride, int32_t max_frames);
+int pfc_frames_written(pfc_t *ctx, int32_t *n);
+
 /* Host-buffer convenience path (used for end-to-end timing): copies pos/vel
  * HOST [n_atoms][4] to internal device buffers, runs n_steps, copies pos, vel,
  * F (optional, may be NULL) and E HOST [n_systems] back, and synchronises. */

@@ -158,7 +158,13 @@ struct pfc_ctx {
   cudaStream_t stream = nullptr, cap_stream = nullptr;
   bool bound = false, forces_stale = true;
   float cur_dt = -1.0f;
-  cudaGraphExec_t g_forces = nullptr, g_step = nullptr;
+  cudaGraphExec_t g_forces = nullptr, g_step = nullptr, g_lstep = nullptr;   // forces; Verlet step; Langevin step
+  float4* frames = nullptr;     // caller's frame buffer (pfc_set_frames)
+  int frame_stride = 0, frame_cap = 0, frames_written = 0;
+  long long steps_total = 0;    // steps since pfc_set_state (frame cadence)
+  float lg_gamma = -1.f, lg_T = -1.f, lg_dt = -1.f;
+  unsigned long long lg_seed = 0;
+  int launches_lstep = 0;
   int launch_counter = 0;
 };
 
@@ -257,11 +263,19 @@ void enqueue_verlet(pfc_ctx* c, cudaStream_t st) {
 void drop_graphs(pfc_ctx* c) {
   if (c->g_forces) cudaGraphExecDestroy(c->g_forces);
   if (c->g_step) cudaGraphExecDestroy(c->g_step);
-  c->g_forces = c->g_step = nullptr;
+  if (c->g_lstep) cudaGraphExecDestroy(c->g_lstep);
+  c->g_forces = c->g_step = c->g_lstep = nullptr;
 }
 
 // capture {optional fused Verlet kernel, forces} for the bound state
-int capture(pfc_ctx* c, bool with_verlet, cudaGraphExec_t* out, int* n_launches) {
+template <int MODE>
+void enqueue_langevin(pfc_ctx* c, cudaStream_t st) {
+  LAUNCH(c, k5_langevin_kernel<MODE>, cdiv(c->sz.n_atoms, K5_THREADS), K5_THREADS, 0, st, c->sz.n_atoms, c->b.sp,
+         c->b.species, c->frc, c->pos, c->vel, c->b.xlo);
+}
+
+// kind 0: forces only; 1: fused Verlet kernel + forces; 2: fused Langevin kernel + forces
+int capture(pfc_ctx* c, int kind, cudaGraphExec_t* out, int* n_launches) {
   // capture on a private stream (the caller's may be the legacy stream, which cannot
   // capture); the instantiated graph is launched on the caller's stream.
   cudaGraph_t graph = nullptr;
@@ -269,7 +283,8 @@ int capture(pfc_ctx* c, bool with_verlet, cudaGraphExec_t* out, int* n_launches)
     return PFC_ERR_CAPTURE;
   if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) return PFC_ERR_CAPTURE;
   c->launch_counter = 0;
-  if (with_verlet) enqueue_verlet<2>(c, c->cap_stream);
+  if (kind == 1) enqueue_verlet<2>(c, c->cap_stream);
+  if (kind == 2) enqueue_langevin<2>(c, c->cap_stream);
   enqueue_forces(c, c->pos, c->E, c->frc, c->cap_stream);
   *n_launches = c->launch_counter;
   cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
@@ -544,17 +559,33 @@ int pfc_set_state(pfc_t* c, float* pos, float* vel, float* E, float* F, void* st
   c->stream = st;
   c->bound = true;
   c->forces_stale = true;
+  c->steps_total = 0;
+  k5_reset_counter_kernel<<<1, 1, 0, st>>>(c->b.sp);
   if (cudaMemsetAsync(c->b.xlo, 0, sizeof(float4) * c->sz.n_atoms, st) != cudaSuccess) return PFC_ERR_CUDA;
   return PFC_OK;
 }
 
-int pfc_step(pfc_t* c, int32_t n_steps, float dt_fs) {
-  if (!c || n_steps < 0 || !(dt_fs > 0.0f)) return PFC_ERR_ARG;
-  if (!c->bound) return PFC_ERR_STATE;
+// after step `steps_total` (1-based) of the bound state: positions x_n are final once the step's
+// drift kernel and force graph are enqueued -- store a frame every frame_stride steps
+static int maybe_store_frame(pfc_ctx* c, cudaStream_t st) {
+  ++c->steps_total;
+  if (!c->frames || c->frame_stride <= 0 || c->steps_total % c->frame_stride != 0) return PFC_OK;
+  if (c->frames_written >= c->frame_cap) return PFC_OK;
+  const size_t nb = sizeof(float4) * (size_t)c->sz.n_atoms;
+  if (cudaMemcpyAsync(c->frames + (size_t)c->frames_written * c->sz.n_atoms, c->pos, nb, cudaMemcpyDeviceToDevice,
+                      st) != cudaSuccess)
+    return PFC_ERR_CUDA;
+  ++c->frames_written;
+  return PFC_OK;
+}
+
+static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
   cudaStream_t st = c->stream;
   int rc;
-  if (!c->g_forces && (rc = capture(c, false, &c->g_forces, &c->launches_ef)) != PFC_OK) return rc;
-  if (!c->g_step && (rc = capture(c, true, &c->g_step, &c->launches_step)) != PFC_OK) return rc;
+  if (!c->g_forces && (rc = capture(c, 0, &c->g_forces, &c->launches_ef)) != PFC_OK) return rc;
+  cudaGraphExec_t* gs = langevin ? &c->g_lstep : &c->g_step;
+  if (!*gs && (rc = capture(c, langevin ? 2 : 1, gs, langevin ? &c->launches_lstep : &c->launches_step)) != PFC_OK)
+    return rc;
   if (dt_fs != c->cur_dt) {
     k5_set_params_kernel<<<1, 1, 0, st>>>(c->b.sp, dt_fs);
     c->cur_dt = dt_fs;
@@ -566,12 +597,51 @@ int pfc_step(pfc_t* c, int32_t n_steps, float dt_fs) {
   if (n_steps == 0) return PFC_OK;
   // step 1: half kick + drift, forces.  steps 2..n: one graph each = fused
   // (trailing half kick + leading half kick + drift), forces.  Then the last half kick.
-  enqueue_verlet<1>(c, st);
+  if (langevin) enqueue_langevin<1>(c, st); else enqueue_verlet<1>(c, st);
   if (cudaGraphLaunch(c->g_forces, st) != cudaSuccess) return PFC_ERR_CUDA;
-  for (int s = 1; s < n_steps; ++s)
-    if (cudaGraphLaunch(c->g_step, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
+  for (int s = 1; s < n_steps; ++s) {
+    if (cudaGraphLaunch(*gs, st) != cudaSuccess) return PFC_ERR_CUDA;
+    if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
+  }
   enqueue_verlet<0>(c, st);
   return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_step(pfc_t* c, int32_t n_steps, float dt_fs) {
+  if (!c || n_steps < 0 || !(dt_fs > 0.0f)) return PFC_ERR_ARG;
+  if (!c->bound) return PFC_ERR_STATE;
+  return run_steps(c, n_steps, dt_fs, false);
+}
+
+int pfc_step_langevin(pfc_t* c, int32_t n_steps, float dt_fs, float friction_per_fs, float temperature_K,
+                      uint64_t seed) {
+  if (!c || n_steps < 0 || !(dt_fs > 0.0f) || !(friction_per_fs >= 0.0f) || !(temperature_K >= 0.0f))
+    return PFC_ERR_ARG;
+  if (!c->bound) return PFC_ERR_STATE;
+  if (friction_per_fs != c->lg_gamma || temperature_K != c->lg_T || dt_fs != c->lg_dt || seed != c->lg_seed) {
+    const double c1 = exp(-(double)friction_per_fs * (double)dt_fs), c2 = sqrt(1.0 - c1 * c1);
+    k5_set_langevin_kernel<<<1, 1, 0, c->stream>>>(c->b.sp, (float)c1, (float)c2,
+                                                    (float)(8.617333262e-5 * (double)temperature_K),
+                                                    (uint32_t)seed, (uint32_t)(seed >> 32));
+    c->lg_gamma = friction_per_fs; c->lg_T = temperature_K; c->lg_dt = dt_fs; c->lg_seed = seed;
+  }
+  return run_steps(c, n_steps, dt_fs, true);
+}
+
+int pfc_set_frames(pfc_t* c, float* frames, int32_t stride, int32_t max_frames) {
+  if (!c || stride < 0 || max_frames < 0 || (frames && (stride < 1 || max_frames < 1))) return PFC_ERR_ARG;
+  c->frames = (float4*)frames;
+  c->frame_stride = frames ? stride : 0;
+  c->frame_cap = frames ? max_frames : 0;
+  c->frames_written = 0;
+  return PFC_OK;
+}
+
+int pfc_frames_written(pfc_t* c, int32_t* n) {
+  if (!c || !n) return PFC_ERR_ARG;
+  *n = c->frames_written;
+  return PFC_OK;
 }
 
 int pfc_run_host(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, float dt_fs, float* E_h, float* F_h,

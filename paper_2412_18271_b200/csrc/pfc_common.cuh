@@ -48,6 +48,12 @@ __constant__ ModelTables c_tab;
 struct StepParams {
   float dt;        // fs
   float half_dt;   // dt/2
+  // Langevin (O9): v <- c1 v + sigma[species] xi,  sigma_s = c2 sqrt(kB T ACC / m_s)
+  float c1;
+  float sigma[NSPEC];
+  uint32_t seed_lo, seed_hi;
+  uint32_t step;   // Langevin steps taken since pfc_set_state: counter word 1 of the generator
+  uint32_t ticket; // blocks of the running Langevin kernel that have finished (last one advances step)
 };
 
 __device__ __forceinline__ float ex2_approx(float x) {

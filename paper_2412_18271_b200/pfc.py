@@ -32,7 +32,7 @@ N_STAGES = 6
 STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum")
 
 EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_profile_stages", "pfc_set_state", "pfc_step",
-           "pfc_run_host", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
+           "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
            "pfc_copy_to_host", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
 
 
@@ -69,6 +69,9 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_profile_stages.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_float)]
     lib.pfc_set_state.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.pfc_step.argtypes = [c_void_p, c_int32, c_float]
+    lib.pfc_step_langevin.argtypes = [c_void_p, c_int32, c_float, c_float, c_float, ctypes.c_uint64]
+    lib.pfc_set_frames.argtypes = [c_void_p, c_void_p, c_int32, c_int32]
+    lib.pfc_frames_written.argtypes = [c_void_p, POINTER(c_int32)]
     lib.pfc_run_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p, c_void_p]
     lib.pfc_get_neighbors.argtypes = [c_void_p, pp_i32, pp_i32, pp_i32, pp_i32]
     lib.pfc_get_capacities.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32)]
@@ -175,6 +178,25 @@ class Pfc:
 
     def step(self, n_steps: int, dt_fs: float = 0.5):
         _check(self._lib.pfc_step(self._h, int(n_steps), float(dt_fs)), "pfc_step")
+
+    def step_langevin(self, n_steps: int, dt_fs: float, friction_per_fs: float, temperature_K: float, seed: int):
+        _check(self._lib.pfc_step_langevin(self._h, int(n_steps), float(dt_fs), float(friction_per_fs),
+                                           float(temperature_K), int(seed)), "pfc_step_langevin")
+
+    def set_frames(self, frames, stride: int):
+        """frames: device tensor [max_frames, N, 4] float32 (None unbinds)."""
+        if frames is None:
+            _check(self._lib.pfc_set_frames(self._h, None, 0, 0), "pfc_set_frames")
+        else:
+            self._expect(frames, (frames.shape[0], self.n_atoms, 4))
+            _check(self._lib.pfc_set_frames(self._h, frames.data_ptr(), int(stride), int(frames.shape[0])),
+                   "pfc_set_frames")
+        self._frames = frames                   # keep alive while bound
+
+    def frames_written(self) -> int:
+        n = c_int32()
+        _check(self._lib.pfc_frames_written(self._h, byref(n)), "pfc_frames_written")
+        return int(n.value)
 
     # -- pfc_run_host -------------------------------------------------------------
     def run_host(self, pos_host, vel_host, n_steps: int, dt_fs: float, E_host, F_host=None, stream=None):
