@@ -155,11 +155,21 @@ def job_value(atoms_per_rank, steps, world, seconds):
     return world * atoms_per_rank * steps / seconds
 
 
+INTEGRATOR = {"kind": "verlet"}                       # set by --integrator (paper protocol: langevin)
+
+
+def _advance(p, n_steps):
+    if INTEGRATOR["kind"] == "langevin":
+        p.step_langevin(n_steps, DT_FS, 1e-4, 300.0, seed=2412)      # friction 0.1 ps^-1, 300 K
+    else:
+        p.step(n_steps, DT_FS)
+
+
 def _time_steps(torch, p, stream, n_steps):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(stream):
         e0.record(stream)
-        p.step(n_steps, DT_FS)
+        _advance(p, n_steps)
         e1.record(stream)
     stream.synchronize()
     return e0.elapsed_time(e1) * 1e-3
@@ -189,7 +199,11 @@ def run_pfc(args):
     pos, vel = torch.from_numpy(pos0).to(dev), torch.from_numpy(vel0).to(dev)
     with torch.cuda.stream(stream):
         E, F = p.set_state(pos, vel, stream=stream)
-        p.step(args.warmup, DT_FS)                               # W untimed steps (includes graph capture)
+        frames = None
+        if args.integrator == "langevin":                        # the paper's protocol also writes 10 frames
+            frames = torch.empty(10, N, 4, dtype=torch.float32, device=dev)
+            p.set_frames(frames, max(1, (args.warmup + args.steps) // 10))
+        _advance(p, args.warmup)                                 # W untimed steps (includes graph capture)
     stream.synchronize()
 
     def barrier():
@@ -273,7 +287,7 @@ def run_pfc(args):
             "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": wl.name, "config_index": args.config, "atoms": N, "systems": wl.n_systems,
-                       "dt_fs": DT_FS, "mlp_path": "fp32_ffma" if args.mlp == 0 else "tf32x3_tcgen05",
+                       "dt_fs": DT_FS, "integrator": args.integrator, "mlp_path": "fp32_ffma" if args.mlp == 0 else "tf32x3_tcgen05",
                        "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "per-step working set (aev + g + lists + edge) exceeds the 126 MB L2"
                              if N * 3072 > 126e6 else "working set fits L2: neighbour/AEV/MLP buffers are "
@@ -319,9 +333,12 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", type=int, default=4, choices=range(5))
     ap.add_argument("--impl", default="pfc", choices=["pfc", "reference"])
+    ap.add_argument("--integrator", default="verlet", choices=["verlet", "langevin"],
+                    help="langevin = the paper's timing protocol (friction 0.1 ps^-1, 10 frames), PAPER.md:94")
     ap.add_argument("--mlp", type=int, default=0, help="0 = FP32 FFMA, 1 = tcgen05 TF32x3")
     ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (100 steps each)")
     args = ap.parse_args()
+    INTEGRATOR["kind"] = args.integrator
     if args.warmup < 3 and args.impl == "pfc":
         args.warmup = 3
     if args.impl == "reference":
