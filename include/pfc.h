@@ -102,6 +102,16 @@ int pfc_create(const pfc_desc_t *desc, pfc_t **out);
  * MLP forward/backward (K3), force chain rule + gather (K4), energy sum. */
 int pfc_energy_forces(pfc_t *ctx, const float *pos, float *E, float *F, void *stream);
 
+/* The provider call in the paper's own units: the callback of
+ * PAPER.md:29-47 receives positions in nm and returns the potential energy in kJ/mol
+ * ("RETURN_ENERGY", forces then follow by differentiation) or energy and
+ * explicit forces in kJ/mol/nm.  pos_nm DEVICE [n_atoms][3] packed float;
+ * E_kj DEVICE [n_systems]; F_kj_nm DEVICE [n_atoms][3] packed float, or NULL for the
+ * energy-only mode.  Packing, the whole of pfc_energy_forces and the conversion (1 nm = 10 A,
+ * 1 eV = 96.485332 kJ/mol) are enqueued on `stream`; nothing is synchronised.  Uses internal
+ * staging buffers: PFC_ERR_STATE if a pfc_run_host state is currently bound to them. */
+int pfc_energy_forces_nm(pfc_t *ctx, const float *pos_nm, float *E_kj, float *F_kj_nm, void *stream);
+
 /* Measurement helper: the same kernel sequence as pfc_energy_forces with a CUDA
  * event recorded on `stream` at every stage boundary; synchronises and returns
  * the device time of each stage in milliseconds, ms HOST [PFC_N_STAGES]:

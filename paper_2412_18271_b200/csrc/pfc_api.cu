@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "../../include/pfc.h"
+#include "k0_units.cuh"
 #include "k1_neighbors.cuh"
 #include "k2_aev.cuh"
 #include "k3_mlp_fp32.cuh"
@@ -531,6 +532,21 @@ int pfc_energy_forces(pfc_t* c, const float* pos, float* E, float* F, void* stre
   cudaStream_t st = (cudaStream_t)stream;
   c->launch_counter = 0;
   enqueue_forces(c, (const float4*)pos, E, (float4*)F, st);
+  if (!c->bound) c->stream = st;
+  return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_energy_forces_nm(pfc_t* c, const float* pos_nm, float* E_kj, float* F_kj_nm, void* stream) {
+  if (!c || !pos_nm || !E_kj) return PFC_ERR_ARG;
+  if (c->bound && (c->pos == c->b.h_pos)) return PFC_ERR_STATE;   // the staging buffers hold a pfc_run_host state
+  cudaStream_t st = (cudaStream_t)stream;
+  const int N = c->sz.n_atoms, NS = c->sz.n_systems;
+  Buffers& b = c->b;
+  c->launch_counter = 0;
+  LAUNCH(c, k0_pack_nm_kernel, cdiv(N, K0_THREADS), K0_THREADS, 0, st, N, pos_nm, b.h_pos);
+  enqueue_forces(c, b.h_pos, b.h_E, b.h_frc, st);
+  LAUNCH(c, k0_unpack_kj_kernel, cdiv(N > NS ? N : NS, K0_THREADS), K0_THREADS, 0, st, N, NS, b.h_frc, b.h_E,
+         F_kj_nm, E_kj);
   if (!c->bound) c->stream = st;
   return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
 }

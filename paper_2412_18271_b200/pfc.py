@@ -31,7 +31,7 @@ STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
 N_STAGES = 6
 STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum")
 
-EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_profile_stages", "pfc_set_state", "pfc_step",
+EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy_forces_nm", "pfc_profile_stages", "pfc_set_state", "pfc_step",
            "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
            "pfc_copy_to_host", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
 
@@ -66,6 +66,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_workspace_bytes.restype = c_size_t
     lib.pfc_create.argtypes = [POINTER(_Desc), POINTER(c_void_p)]
     lib.pfc_energy_forces.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pfc_energy_forces_nm.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.pfc_profile_stages.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(c_float)]
     lib.pfc_set_state.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.pfc_step.argtypes = [c_void_p, c_int32, c_float]
@@ -178,6 +179,18 @@ class Pfc:
 
     def step(self, n_steps: int, dt_fs: float = 0.5):
         _check(self._lib.pfc_step(self._h, int(n_steps), float(dt_fs)), "pfc_step")
+
+    def energy_forces_nm(self, pos_nm, want_forces: bool = True, stream=None):
+        """Provider call in the paper's units: pos_nm cuda [N,3] float32 (nm) -> (E kJ/mol [n_systems],
+        F kJ/mol/nm [N,3] or None).  Marshalling only; the conversion runs in the library's kernels."""
+        import torch
+        self._expect(pos_nm, (self.n_atoms, 3))
+        E = torch.empty(self.n_systems, dtype=torch.float32, device=self.device)
+        F = torch.empty(self.n_atoms, 3, dtype=torch.float32, device=self.device) if want_forces else None
+        _check(self._lib.pfc_energy_forces_nm(self._h, pos_nm.data_ptr(), E.data_ptr(),
+                                              F.data_ptr() if want_forces else None, _stream_ptr(stream)),
+               "pfc_energy_forces_nm")
+        return E, F
 
     def step_langevin(self, n_steps: int, dt_fs: float, friction_per_fs: float, temperature_K: float, seed: int):
         _check(self._lib.pfc_step_langevin(self._h, int(n_steps), float(dt_fs), float(friction_per_fs),
