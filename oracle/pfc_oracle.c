@@ -17,7 +17,10 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): P1/P2 golden values
  * (tests/golden/), P3 finite differences, P4 invariances, P5 torch fp64
  * celu/matmul/autograd, P6 independent torch-autograd AEV, P7 brute-force vs
- * cell list, P8 dt^2 NVE error, P9 reversibility, P10 harmonic oscillator.
+ * cell list, P8 dt^2 NVE error, P9 reversibility, P10 harmonic oscillator;
+ * O9 (Langevin, at the end of this file): P13 Philox known-answer vectors, P14
+ * moments of the normals, P15 zero friction = O8, P16 free-particle
+ * thermalisation (tests/test_oracle_langevin.py).
  * P12: absolute energies of this random-weight potential are "parity
  * unpinned" beyond those (no printed value exists anywhere).
  *
