@@ -161,6 +161,14 @@ int pfc_frames_written(pfc_t *ctx, int32_t *n);
 int pfc_run_host(pfc_t *ctx, float *pos_host, float *vel_host, int32_t n_steps, float dt_fs,
                  float *E_host, float *F_host, void *stream);
 
+/* As pfc_run_host, for a caller that keeps the MD state on the host between calls (the callback
+ * regime of PAPER.md:29-47: one force evaluation per step): F_host HOST [n_atoms][4] is REQUIRED and
+ * on entry holds the forces at pos_host as a previous pfc_run_host / pfc_run_host_resume returned
+ * them; they are uploaded instead of being recomputed, so n_steps cost n_steps force evaluations
+ * (pfc_run_host costs n_steps + 1).  Passing forces that do not belong to pos_host is undefined. */
+int pfc_run_host_resume(pfc_t *ctx, float *pos_host, float *vel_host, float *F_host, int32_t n_steps,
+                        float dt_fs, float *E_host, void *stream);
+
 /* Parity getters: DEVICE pointers into the workspace, valid until the next
  * call that enqueues work.  Lists are int32 CSR, rows ascending by neighbour
  * index (O2/S7). */

@@ -660,16 +660,18 @@ int pfc_frames_written(pfc_t* c, int32_t* n) {
   return PFC_OK;
 }
 
-int pfc_run_host(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, float dt_fs, float* E_h, float* F_h,
-                 void* stream) {
-  if (!c || !pos_h || !vel_h || !E_h) return PFC_ERR_ARG;
+static int run_host_impl(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, float dt_fs, float* E_h,
+                         float* F_h, void* stream, bool forces_in) {
+  if (!c || !pos_h || !vel_h || !E_h || (forces_in && !F_h)) return PFC_ERR_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t nb = sizeof(float4) * (size_t)c->sz.n_atoms;
   Buffers& b = c->b;
   if (cudaMemcpyAsync(b.h_pos, pos_h, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpyAsync(b.h_vel, vel_h, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if (forces_in && cudaMemcpyAsync(b.h_frc, F_h, nb, cudaMemcpyHostToDevice, st) != cudaSuccess) return PFC_ERR_CUDA;
   int rc = pfc_set_state(c, (float*)b.h_pos, (float*)b.h_vel, b.h_E, (float*)b.h_frc, stream);
   if (rc != PFC_OK) return rc;
+  if (forces_in) c->forces_stale = false;          // the caller vouches: F_h = forces at pos_h
   if ((rc = pfc_step(c, n_steps, dt_fs)) != PFC_OK) return rc;
   if (cudaMemcpyAsync(pos_h, b.h_pos, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpyAsync(vel_h, b.h_vel, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
@@ -677,6 +679,16 @@ int pfc_run_host(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, float dt
   if (cudaMemcpyAsync(E_h, b.h_E, sizeof(float) * c->sz.n_systems, cudaMemcpyDeviceToHost, st) != cudaSuccess)
     return PFC_ERR_CUDA;
   return cudaStreamSynchronize(st) == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
+int pfc_run_host(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, float dt_fs, float* E_h, float* F_h,
+                 void* stream) {
+  return run_host_impl(c, pos_h, vel_h, n_steps, dt_fs, E_h, F_h, stream, false);
+}
+
+int pfc_run_host_resume(pfc_t* c, float* pos_h, float* vel_h, float* F_h, int32_t n_steps, float dt_fs,
+                        float* E_h, void* stream) {
+  return run_host_impl(c, pos_h, vel_h, n_steps, dt_fs, E_h, F_h, stream, true);
 }
 
 int pfc_get_neighbors(pfc_t* c, const int32_t** r_off, const int32_t** r_idx, const int32_t** a_off,

@@ -32,7 +32,7 @@ N_STAGES = 6
 STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum")
 
 EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy_forces_nm", "pfc_profile_stages", "pfc_set_state", "pfc_step",
-           "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
+           "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host", "pfc_run_host_resume", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
            "pfc_copy_to_host", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
 
 
@@ -74,6 +74,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_set_frames.argtypes = [c_void_p, c_void_p, c_int32, c_int32]
     lib.pfc_frames_written.argtypes = [c_void_p, POINTER(c_int32)]
     lib.pfc_run_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p, c_void_p]
+    lib.pfc_run_host_resume.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p]
     lib.pfc_get_neighbors.argtypes = [c_void_p, pp_i32, pp_i32, pp_i32, pp_i32]
     lib.pfc_get_capacities.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32)]
     lib.pfc_get_intermediates.argtypes = [c_void_p, pp_f, pp_f, pp_i32, POINTER(c_int32)]
@@ -220,6 +221,13 @@ class Pfc:
             return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
         _check(self._lib.pfc_run_host(self._h, ptr(pos_host), ptr(vel_host), int(n_steps), float(dt_fs),
                                       ptr(E_host), ptr(F_host), _stream_ptr(stream)), "pfc_run_host")
+
+    def run_host_resume(self, pos_host, vel_host, F_host, n_steps: int, dt_fs: float, E_host, stream=None):
+        """As run_host, with F_host [N,4] holding the forces at pos_host on entry (uploaded, not recomputed)."""
+        def ptr(a):
+            return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+        _check(self._lib.pfc_run_host_resume(self._h, ptr(pos_host), ptr(vel_host), ptr(F_host), int(n_steps),
+                                             float(dt_fs), ptr(E_host), _stream_ptr(stream)), "pfc_run_host_resume")
 
     # -- getters ------------------------------------------------------------------
     def status(self) -> int:

@@ -233,6 +233,27 @@ def test_run_host_matches_device_path(pfc, weights):
     p.close(); p2.close()
 
 
+def test_run_host_resume_one_force_evaluation_per_call(pfc, weights):
+    """The callback regime: state on the host, one step per call, forces carried over by the caller."""
+    wl = W.config1(n_replicas=4)
+    ph = torch.from_numpy(pfc.pack4(wl.pos)).pin_memory()
+    vh = torch.from_numpy(pfc.pack4(wl.vel)).pin_memory()
+    Eh = torch.empty(wl.n_systems, dtype=torch.float32).pin_memory()
+    Fh = torch.empty(wl.n_atoms, 4, dtype=torch.float32).pin_memory()
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    p.run_host(ph, vh, 0, 0.5, Eh, Fh)                        # forces at the start
+    ef, step = p.launch_counts()
+    for _ in range(20):
+        p.run_host_resume(ph, vh, Fh, 1, 0.5, Eh)
+    ref = oracle.step(wl.pos, wl.vel, wl.species, wl.sys_offsets, weights, 0.5, 20)
+    x = ph.numpy()[:, :3].astype(np.float64)
+    assert _rmsd_per_system(x, ref["pos"], wl.sys_offsets).max() <= RMSD_TOL
+    assert np.abs(vh.numpy()[:, :3] - ref["vel"]).max() <= VEL_TOL
+    assert np.abs(Fh.numpy()[:, :3] - ref["F"]).max() <= F_ATOL_INTERNAL
+    assert np.abs(Eh.numpy() - ref["pe"][-1]).max() <= E_RTOL * np.maximum(np.abs(ref["pe"][-1]), 1.0).max()
+    p.close()
+
+
 # ---- edge and degenerate cases ------------------------------------------------------------
 def _eval(pfc, weights, pos, species, off):
     p = pfc.Pfc(species, off, weights)
