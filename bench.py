@@ -96,6 +96,9 @@ def _oracle_steps_per_s(wl, weights, n_steps):
     return wl.n_atoms * (n_steps + 1) / dt, dt
 
 
+WORKLOAD_NAMES = ("cfg0_molecule22", "cfg1_256x22", "cfg2_water1500", "cfg3_droplet20000", "cfg4_ragged4096")
+
+
 def _sample_workload(k, budget_atoms):
     """A bounded sample of config k for the CPU legs: whole replicas / a smaller droplet."""
     if k == 0:
@@ -130,8 +133,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / (args.steps + 1) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"config {args.config}", "sample": what, "atoms_in_sample": wl.n_atoms,
-                   "dt_fs": DT_FS},
+        "config": {"workload": WORKLOAD_NAMES[args.config], "config_index": args.config, "sample": what,
+                   "atoms_in_sample": wl.n_atoms, "dt_fs": DT_FS},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -279,7 +282,8 @@ def run_pfc(args):
         # ---- the oracle on the host cores, bounded sample ----
         import oracle
         swl, what = _sample_workload(args.config, 14000)
-        n_cpu_steps = 4 if swl.n_atoms > 5000 else 20
+        rate, _ = _oracle_steps_per_s(swl, weights, 1)               # calibration: atom-evaluations / s
+        n_cpu_steps = int(min(400, max(3, 12.0 * rate / swl.n_atoms)))   # about 12 s of CPU work
         cpu_v, cpu_t = _oracle_steps_per_s(swl, weights, n_cpu_steps)
         cpu = {"value": cpu_v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                "sample": f"{what}, {n_cpu_steps} steps ({cpu_t:.1f} s)"}
