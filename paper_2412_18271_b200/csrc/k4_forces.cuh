@@ -170,23 +170,35 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
       S.tK[q] = 2.0f * fcj * fmaf(0.5f * Gr, fck, G0 * dfck);
     }
     __syncwarp();
+    // rows (smaller index j) this chunk of the lexicographic triple order touches: a neighbour n
+    // meets only partners j < n with j in [j_lo, j_hi] and, if its own row is among them, the
+    // partners k > n whose triple lies in the chunk -- in ascending partner order, as a scan over
+    // all partners would, at a cost that does not grow with the number of chunks
+    int j_lo = 0, j_hi = m - 2, kk;
+    if (T > K4_TCH) {                             // (a single chunk holds every row)
+      tri_decode(t0, m, j_lo, kk);
+      tri_decode(t0 + nt - 1, m, j_hi, kk);
+    }
 #pragma unroll
     for (int h = 0; h < 3; ++h) {
       const int n = (int)lane + 32 * h;
       if (n < m) {                                // (h*32 < m is warp-uniform; lanes beyond idle)
         const float4 un = S.ur[n];
-        for (int k = 0; k < m; ++k) {
-          if (k == n) continue;
-          const int lo = min(n, k), hi = max(n, k);
-          const int t = tri_row_start(lo, m) + (hi - lo - 1) - t0;
-          if (t < 0 || t >= nt) continue;
+        auto meet = [&](int k, int t, float R) {
           const float4 uk = S.ur[k];
           const float C = S.tC[t];
-          const float R = (n < k) ? S.tJ[t] : S.tK[t];
           const float cphi = un.x * uk.x + un.y * uk.y + un.z * uk.z;
           Sx[h] = fmaf(C, uk.x, Sx[h]); Sy[h] = fmaf(C, uk.y, Sy[h]); Sz[h] = fmaf(C, uk.z, Sz[h]);
           Sc[h] = fmaf(C, cphi, Sc[h]);
           Sr[h] += R;
+        };
+        for (int j = j_lo; j <= min(j_hi, n - 1); ++j) {          // n is the larger index of (j, n)
+          const int t = tri_row_start(j, m) + (n - j - 1) - t0;
+          if (t >= 0 && t < nt) meet(j, t, S.tK[t]);
+        }
+        if (n >= j_lo && n <= j_hi) {                             // n is the smaller index of (n, k)
+          const int base = tri_row_start(n, m) - (n + 1) - t0;    // t = base + k
+          for (int k = max(n + 1, -base); k <= min(m - 1, nt - 1 - base); ++k) meet(k, base + k, S.tJ[base + k]);
         }
       }
     }
