@@ -172,7 +172,7 @@ struct CellGrid {          // one per cell-list system, in device memory
   int n_cells;
 };
 
-constexpr int CELL_THREADS = 256;
+constexpr int CELL_THREADS = 1024;          // one CTA per cell-list system walks all its atoms / cells
 // 2^-10 of slack: binning round-off ((x-lo)*inv_edge carries ~nc*1.2e-7 of error) can never
 // put two atoms closer than the cutoff into non-adjacent cells; the predicate decides.
 constexpr float CELL_EDGE_MIN = 5.2f * (1.0f + 9.765625e-4f);

@@ -254,7 +254,9 @@ k4b_gather_kernel(int n_atoms, const int* __restrict__ r_off, const int* __restr
 }
 
 // per-system potential energy: one CTA per system, fixed-order tree, fp64 partials
-constexpr int ESUM_THREADS = 128;
+// (128 threads for small replicas; 1024 for cell-list systems, whose thousands of atoms would
+// otherwise be a long serial chain of loads per thread)
+template <int ESUM_THREADS>
 __global__ void __launch_bounds__(ESUM_THREADS)
 k_energy_sum_kernel(const int* __restrict__ sys_off, const float4* __restrict__ frc,
                     float* __restrict__ E, uint32_t* __restrict__ status) {

@@ -251,7 +251,8 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
   LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.r_off, b.r_idx, s.cap_r, b.edge, b.self,
          b.row_of_atom, b.e_row, F);
   mark(5);
-  LAUNCH(c, k_energy_sum_kernel, s.n_systems, ESUM_THREADS, 0, st, b.sys_off, F, E, b.status);
+  if (c->n_cell_sys > 0) LAUNCH(c, k_energy_sum_kernel<1024>, s.n_systems, 1024, 0, st, b.sys_off, F, E, b.status);
+  else LAUNCH(c, k_energy_sum_kernel<128>, s.n_systems, 128, 0, st, b.sys_off, F, E, b.status);
   mark(6);
 }
 
