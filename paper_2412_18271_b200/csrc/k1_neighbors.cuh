@@ -295,13 +295,17 @@ k1_cell_scan_kernel(const int* __restrict__ cell_sys, const int* __restrict__ ce
 
 // scatter atoms into their cells (slot order inside a cell is arbitrary: rows are
 // ordered by index afterwards, so the final lists do not depend on it)
+// cell_xyz[slot] = {x, y, z, bitcast(atom index)}: the rows kernels stream a cell line's positions
+// contiguously instead of gathering pos[cell_atoms[p]] (two dependent loads per round)
 __global__ void k1_cell_fill_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
-                                    const int* __restrict__ atom_cell, int* __restrict__ cell_cursor,
-                                    int* __restrict__ cell_atoms) {
+                                    const int* __restrict__ atom_cell, const float4* __restrict__ pos,
+                                    int* __restrict__ cell_cursor, float4* __restrict__ cell_xyz) {
   int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= n_cell_atoms) return;
   int slot = atomicAdd(&cell_cursor[atom_cell[q]], 1);
-  cell_atoms[slot] = cell_atom_list[q];
+  const int i = cell_atom_list[q];
+  const float4 p = pos[i];
+  cell_xyz[slot] = make_float4(p.x, p.y, p.z, __int_as_float(i));
 }
 
 // neighbour rows through the cell list: one warp per atom.
@@ -313,7 +317,7 @@ __global__ void __launch_bounds__(K1_WARPS * 32)
 k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
                     const int* __restrict__ atom_cell_sys, const int* __restrict__ atom_cell,
                     const float4* __restrict__ pos, const CellGrid* __restrict__ grids,
-                    const int* __restrict__ cell_start, const int* __restrict__ cell_atoms,
+                    const int* __restrict__ cell_start, const float4* __restrict__ cell_xyz,
                     int2* __restrict__ cnt, const int* __restrict__ r_off, const int* __restrict__ a_off,
                     int* __restrict__ r_idx, int* __restrict__ a_idx, int cap_r, int cap_a,
                     uint32_t* __restrict__ status) {
@@ -338,11 +342,12 @@ k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
       int s0 = cell_start[c0], s1 = cell_start[c1 + 1];
       for (int p0 = s0; p0 < s1; p0 += 32) {
         int p = p0 + (int)lane;
-        int j = (p < s1) ? cell_atoms[p] : i;
+        int j = i;
         float d2 = 1e30f;
-        if (j != i) {
-          float4 pj = pos[j];
-          d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+        if (p < s1) {
+          const float4 pj = cell_xyz[p];
+          j = __float_as_int(pj.w);
+          if (j != i) d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
         }
         uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
         if (FILL) {

@@ -66,7 +66,8 @@ struct Buffers {
   float* bias_tc;
   // cell list
   int *cell_sys, *cell_cap_base, *cell_slot_base, *cell_atom_list, *atom_cell_sys, *atom_cell;
-  int *cell_count, *cell_start, *cell_cursor, *cell_atoms;
+  int *cell_count, *cell_start, *cell_cursor;
+  float4* cell_xyz;             // positions in cell order, atom index in .w
   CellGrid* grids;
   // internal state for pfc_run_host
   float4 *h_pos, *h_vel, *h_frc;
@@ -108,7 +109,7 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.cell_atom_list = c.take<int>((size_t)s.n_cell_atoms + 1);
   t.atom_cell_sys = c.take<int>((size_t)s.n_cell_atoms + 1);
   t.atom_cell = c.take<int>((size_t)s.n_cell_atoms + 1);
-  t.cell_atoms = c.take<int>((size_t)s.n_cell_atoms + 1);
+  t.cell_xyz = c.take<float4>((size_t)s.n_cell_atoms + 1);
   t.cell_count = c.take<int>((size_t)s.cell_slots + 1);
   t.cell_start = c.take<int>((size_t)s.cell_slots + 1);
   t.cell_cursor = c.take<int>((size_t)s.cell_slots + 1);
@@ -201,9 +202,9 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
     LAUNCH(c, k1_cell_scan_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.cell_slot_base, b.grids,
            b.cell_count, b.cell_start, b.cell_cursor);
     LAUNCH(c, k1_cell_fill_kernel, cdiv(nca, 256), 256, 0, st, nca, b.cell_atom_list, b.atom_cell,
-           b.cell_cursor, b.cell_atoms);
+           pos, b.cell_cursor, b.cell_xyz);
     LAUNCH(c, k1_cell_rows_kernel<false>, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
-           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_atoms, b.cnt, b.r_off, b.a_off,
+           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_xyz, b.cnt, b.r_off, b.a_off,
            b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
   }
   if (s.n_scan_blocks > 1)
@@ -215,7 +216,7 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
   if (c->n_cell_sys > 0) {
     const int nca = c->n_cell_atoms;
     LAUNCH(c, k1_cell_rows_kernel<true>, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
-           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_atoms, b.cnt, b.r_off, b.a_off,
+           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_xyz, b.cnt, b.r_off, b.a_off,
            b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
   }
   mark(1);
