@@ -40,7 +40,8 @@ template <int TM, bool DEEP = false> struct MlpCfg {                  // TM = 16
   static constexpr int THREADS = TM >= 64 ? 4 * TM : 256;             // 8 warps per (up to) 64 rows
   static constexpr int WARPS = THREADS / 32;
   static constexpr int R = TM >= 64 ? 4 : TM / 16;                    // rows per thread
-  static constexpr int KC = TM == 64 ? 8 : 16;                        // k per staged chunk (64: two CTAs per SM)
+  static constexpr bool PACKED = TM == 32 && !DEEP;                   // fma.rn.f32x2 inner loop (two CTAs per SM)
+  static constexpr int KC = PACKED ? 32 : TM == 64 ? 8 : 16;          // k per staged chunk (64: two CTAs per SM)
   static constexpr int S = DEEP ? 8 : 2;                              // staging buffers
   static constexpr int LEAD = DEEP ? 6 : 1;                           // chunks issued ahead of the consumers
   static constexpr int AS_LD = KC + 4;                                // AEV chunk row stride: 4 mod 8 floats
@@ -63,6 +64,14 @@ constexpr int MLP_P_OFF5 = MLP_P_OFF4 + D2 * D1;       // W1    K=160 N=3x128 (p
 constexpr int MLP_P_FLOATS = MLP_P_OFF5 + D1 * D0;     // 188,416
 constexpr int MLP_V_B1 = 0, MLP_V_B2 = D1, MLP_V_B3 = D1 + D2, MLP_V_W4 = D1 + D2 + D3,
               MLP_V_B4 = D1 + D2 + 2 * D3, MLP_V_FLOATS = 484;
+
+// d += a * b on two fp32 lanes (sm_100: SASS FFMA2)
+__device__ __forceinline__ void ffma2(float2& d, float2 a, float2 b) {
+  unsigned long long ua = *reinterpret_cast<unsigned long long*>(&a), ub = *reinterpret_cast<unsigned long long*>(&b),
+                     ud = *reinterpret_cast<unsigned long long*>(&d);
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(ud) : "l"(ua), "l"(ub));
+  d = *reinterpret_cast<float2*>(&ud);
+}
 
 struct MlpParams {
   const float* wpack[NSPEC];   // MLP_P_FLOATS per element
@@ -149,6 +158,17 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
       else cp_async_commit();
     }
   };
+  // PACKED (the 32-row kernel): accumulator pairs (sum over even k, sum over odd k) advanced by one
+  // fma.rn.f32x2 (SASS FFMA2) per pair -- half the FMA issue slots; the pair is added at the end.
+  // Otherwise one accumulator, k ascending.
+  constexpr bool PACKED = Cfg::PACKED;
+  float2 acc2[PACKED ? R : 1][PACKED ? NT : 1];
+  if (PACKED) {
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+      for (int c = 0; c < NT; ++c) acc2[PACKED ? r : 0][PACKED ? c : 0] = make_float2(0.0f, 0.0f);
+  }
   auto compute = [&](int ch, uint32_t st) {
     const float* bs = P.Bs + st * MLP_BS_FLOATS;
     const float* at = A_GLOBAL ? P.As + st * AS_FLOATS + rowbase * MLP_AS_LD
@@ -160,23 +180,32 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
 #pragma unroll
       for (int r = 0; r < R; ++r) a[r] = *reinterpret_cast<const float4*>(at + r * astr + 4 * k4);
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const float* brow = bs + (4 * k4 + j) * N;
-        float b[NT];
+      for (int j = 0; j < 2; ++j) {                      // k pair 2*k4 + j of the chunk: B2[pair][n][2]
+        const float* brow = bs + (2 * k4 + j) * (2 * N);
+        float2 b[NT];
 #pragma unroll
         for (int f = 0; f < NF4; ++f) {
-          const float4 v = *reinterpret_cast<const float4*>(brow + 64 * f + 4 * cgi);
-          b[4 * f] = v.x; b[4 * f + 1] = v.y; b[4 * f + 2] = v.z; b[4 * f + 3] = v.w;
+          const float4 v0 = *reinterpret_cast<const float4*>(brow + 2 * (64 * f + 4 * cgi));
+          const float4 v1 = *reinterpret_cast<const float4*>(brow + 2 * (64 * f + 4 * cgi) + 4);
+          b[4 * f] = make_float2(v0.x, v0.y); b[4 * f + 1] = make_float2(v0.z, v0.w);
+          b[4 * f + 2] = make_float2(v1.x, v1.y); b[4 * f + 3] = make_float2(v1.z, v1.w);
         }
         if (HAS2) {
-          const float2 v = *reinterpret_cast<const float2*>(brow + 64 * NF4 + 2 * cgi);
-          b[NT - 2] = v.x; b[NT - 1] = v.y;
+          const float4 v = *reinterpret_cast<const float4*>(brow + 2 * (64 * NF4 + 2 * cgi));
+          b[NT - 2] = make_float2(v.x, v.y); b[NT - 1] = make_float2(v.z, v.w);
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-          const float av = j == 0 ? a[r].x : j == 1 ? a[r].y : j == 2 ? a[r].z : a[r].w;
+          const float2 av = j == 0 ? make_float2(a[r].x, a[r].y) : make_float2(a[r].z, a[r].w);
 #pragma unroll
-          for (int c = 0; c < NT; ++c) acc[r][c] = fmaf(av, b[c], acc[r][c]);
+          for (int c = 0; c < NT; ++c) {
+            if (PACKED) {
+              ffma2(acc2[PACKED ? r : 0][PACKED ? c : 0], av, b[c]);
+            } else {
+              acc[r][c] = fmaf(av.x, b[c].x, acc[r][c]);
+              acc[r][c] = fmaf(av.y, b[c].y, acc[r][c]);
+            }
+          }
         }
       }
     }
@@ -213,10 +242,16 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
       if (lane == 0) tc::mbar_arrive(&P.empty[st]);
     }
   }
+  if (PACKED) {
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+      for (int c = 0; c < NT; ++c) acc[r][c] = acc2[PACKED ? r : 0][PACKED ? c : 0].x + acc2[PACKED ? r : 0][PACKED ? c : 0].y;
+  }
 }
 
 template <int TM, bool DEEP>
-__global__ void __launch_bounds__(MlpCfg<TM, DEEP>::THREADS, TM == 64 ? 2 : 1)
+__global__ void __launch_bounds__(MlpCfg<TM, DEEP>::THREADS, (TM == 64 || MlpCfg<TM, DEEP>::PACKED) ? 2 : 1)
 k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict__ aev,
                    float* __restrict__ g, float* __restrict__ e_row) {
   extern __shared__ __align__(16) float smem[];

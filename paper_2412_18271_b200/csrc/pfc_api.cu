@@ -359,17 +359,18 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   carve(c->sz, d->workspace, &c->b);
   Buffers& b = c->b;
 
-  // FFMA path: per element, every GEMM phase as a row-major B[k][n] (forward: W^T, backward: W,
-  // the last one in three 128-column passes), so a 16-k chunk is one contiguous bulk copy
+  // FFMA path: per element, every GEMM phase as B[k/2][n][k%2] (forward: W^T, backward: W, the last
+  // one in three 128-column passes): a 16-k chunk is one contiguous bulk copy, and the two k of a
+  // pair sit side by side for the packed fma.rn.f32x2 of the 32-row kernel
   std::vector<float> w((size_t)NSPEC * DEV_W_PER_ELEM, 0.0f);
   for (int e = 0; e < NSPEC; ++e) {
     const float* src = d->weights + (size_t)e * W_PER_ELEM;
     const float *W1 = src, *b1 = W1 + D1 * D0, *W2 = b1 + D1, *b2 = W2 + D2 * D1, *W3 = b2 + D2,
                 *b3 = W3 + D3 * D2, *W4 = b3 + D3, *b4 = W4 + D3;
     float* dst = w.data() + (size_t)e * DEV_W_PER_ELEM;
-    auto pack = [&](float* out, int K, int N, auto bval) {        // out[k][n] = B[k][n]
+    auto pack = [&](float* out, int K, int N, auto bval) {        // out[k/2][n][k%2] = B[k][n]: k pairs interleaved
       for (int k = 0; k < K; ++k)
-        for (int n = 0; n < N; ++n) out[(size_t)k * N + n] = bval(k, n);
+        for (int n = 0; n < N; ++n) out[((size_t)(k >> 1) * N + n) * 2 + (k & 1)] = bval(k, n);
     };
     pack(dst + MLP_P_OFF0, D0, D1, [&](int k, int n) { return W1[n * D0 + k]; });
     pack(dst + MLP_P_OFF1, D1, D2, [&](int k, int n) { return W2[n * D1 + k]; });
