@@ -9,21 +9,25 @@
 // measurements in pfc_api.cu); 8 warps per (up to) 64 rows.
 // A warp owns min(TM,64) rows x N/8 columns: lane = (row group rg = lane/2, column group
 // cg = lane%2), thread rows 64*half + rg + 16r (r < R = min(TM,64)/16), thread columns: float4s at
-// 4*cgi + 64*f (f < N/64) plus, for N = 160 / 96, a float2 at 64*(N/64) + 2*cgi, cgi = 2*(warp%8) + cg.
+// 4*cgi + 64*f (f < N/64) plus, for N = 160 / 96, two more at 64*(N/64) + 2*cgi, cgi = 2*(warp%8) + cg.
 // The lane mapping is chosen for the shared-memory pipe, which is what bounds this kernel (ncu:
 // 84 % of the LSU wavefront peak with the earlier rg = lane/4, cg = lane%4 mapping).  Measured on
-// B200: an LDS.128 costs 2 cycles of the SM's shared-memory pipe when lanes with equal addresses are
-// adjacent (or there are only two addresses, alternating), 4 cycles otherwise; with 16 row groups
-// of two adjacent lanes BOTH operand loads are 2-cycle: per 4 k a warp spends 2R + 2N/16 pipe
-// cycles for R*N/16 FFMA issue cycles (TM = 64, N = 128: 24 vs 32).
+// B200 (csrc/probes, profiles/r1c_probes.md): an LDS.128 costs 2 cycles of the SM's shared-memory
+// pipe when lanes with equal addresses are adjacent (or there are only two addresses, alternating),
+// 4 cycles otherwise; with 16 row groups of two adjacent lanes BOTH operand loads are 2-cycle.
+//   * the 32-row kernel (the one large batches run) issues the FMAs as packed fma.rn.f32x2
+//     (SASS FFMA2): an accumulator PAIR per output holds the sums over even and over odd k, the
+//     activation pair comes straight from the float4 along k, the weight pair from the layout
+//     B[k/2][n][k%2] pfc_create writes; the pair is added once per phase.  Half the FMA issue slots,
+//     which pays at two CTAs per SM (116 registers) with 32-wide K chunks: 2.11 -> 1.96 ms;
 //   * activations h1/h2/h3 (later delta1/2/3) stay in shared memory, row-major with row stride
 //     = 4 mod 32 floats, so the eight row groups of a half warp read eight different bank groups;
-//   * the AEV tile is NOT held: phase 0 streams it in 16-wide K chunks with cp.async
-//     (into the h2 region, idle at that time) next to the weight chunks;
-//   * weights are laid out by pfc_create per phase as B[k][n], so a chunk of 16 k is one
-//     contiguous block fetched from L2 by ONE cp.async.bulk (TMA) on an mbarrier, double buffered
-//     (a 4-stage full/empty mbarrier ring with no CTA barrier inside a phase was measured slower:
-//     2.30 vs 2.18 ms at 128 rows, 2.37 vs 2.12 ms at 32 rows, config 4);
+//   * the AEV tile is NOT held: phase 0 streams it in K chunks with cp.async (into the h2/h3
+//     region, idle at that time) next to the weight chunks;
+//   * a weight chunk (KC k of one phase, all N columns) is one contiguous block fetched from L2 by
+//     ONE cp.async.bulk (TMA) on an mbarrier, double buffered, one CTA barrier per chunk; for
+//     batches of few tiles per SM an 8-stage full/empty mbarrier ring without CTA barriers inside a
+//     phase (DEEP) -- with several CTAs per SM the ring is slower (2.30 vs 2.18 ms at 128 rows);
 //   * warps whose 64 rows are all padding skip the arithmetic.
 #pragma once
 #include "pfc_common.cuh"
@@ -39,7 +43,8 @@ constexpr int MLP_LD1 = D1 + 4, MLP_LD2 = D2 + 4, MLP_LD3 = D3 + 4;   // row str
 template <int TM, bool DEEP = false> struct MlpCfg {                  // TM = 16, 32, 64 or 128 rows per tile
   static constexpr int THREADS = TM >= 64 ? 4 * TM : 256;             // 8 warps per (up to) 64 rows
   static constexpr int WARPS = THREADS / 32;
-  static constexpr int R = TM >= 64 ? 4 : TM / 16;                    // rows per thread
+  static constexpr int R = (TM >= 64 || (TM == 32 && !DEEP)) ? 4 : TM / 16;   // rows per thread
+  template <int N> __host__ __device__ static constexpr int nt() { return (TM == 32 && !DEEP) ? N / 32 : N / 16; }   // columns per thread
   static constexpr bool PACKED = TM == 32 && !DEEP;                   // fma.rn.f32x2 inner loop (two CTAs per SM)
   static constexpr int KC = PACKED ? 32 : TM == 64 ? 8 : 16;          // k per staged chunk (64: two CTAs per SM)
   static constexpr int S = DEEP ? 8 : 2;                              // staging buffers
@@ -116,15 +121,43 @@ __device__ __forceinline__ int mlp_col(int cgi, int c) {
   return c < 4 * NF4 ? 64 * (c >> 2) + 4 * cgi + (c & 3) : 64 * NF4 + 2 * cgi + (c - 4 * NF4);
 }
 
+// Which rows and columns a thread owns.
+//   default: 8 column warps per (up to) 64 rows; lane = (row group lane/2, column slot lane%2);
+//            rows 64*(w/8) + lane/2 + 16r, columns mlp_col<N>(2*(w%8) + lane%2, c).
+//   PACKED (32 rows): 4 row warps x 2 column warps; lane = (column slot lane/2, row group lane%2);
+//            rows 8*(w/2) + 4*(lane%2) + r (r < 4); column slot ct = 16*(w%2) + lane/2 (< 32) owns the
+//            pairs {2ct, 2ct+1} + 64f (f < (N/32)/2) and, for N = 160 / 96, the single 64*((N/32)/2) + ct.
+//            Per 4 k a warp then spends 2*4 shared-memory pipe cycles on the activations and
+//            2*(2,2,1) + (1,0,1) per k pair on the weights: 18 / 16 / 14 for N = 160 / 128 / 96, against
+//            24 / 20 / 16 with the default mapping at two rows per thread -- the kernel is bound by
+//            that pipe once the FMAs are packed (ncu: 77 % of its peak).
+template <int TM, bool DEEP> struct MlpLane {
+  static constexpr bool PACKED = MlpCfg<TM, DEEP>::PACKED;
+  int lane, w;
+  __device__ __forceinline__ MlpLane() : lane(threadIdx.x & 31), w(threadIdx.x >> 5) {}
+  __device__ __forceinline__ int ct() const { return PACKED ? 16 * (w & 1) + (lane >> 1) : 2 * (w & 7) + (lane & 1); }
+  __device__ __forceinline__ int row(int r) const {
+    return PACKED ? 8 * (w >> 1) + 4 * (lane & 1) + r : 64 * (w >> 3) + (lane >> 1) + 16 * r;
+  }
+  __device__ __forceinline__ int warp_row0() const { return PACKED ? 8 * (w >> 1) : 64 * (w >> 3); }
+  template <int N> __device__ __forceinline__ int col(int c) const {
+    if (PACKED) {
+      constexpr int NW = (N / 32) / 2;
+      return c < 2 * NW ? 64 * (c >> 1) + 2 * ct() + (c & 1) : 64 * NW + ct();
+    }
+    return mlp_col<N>(ct(), c);
+  }
+};
+
 // acc[r][c] = sum_k A[rowbase + 16r][k] * B[k][mlp_col<N>(cgi, c)],  k < K, r < R,  rowbase = 64*half + rg.
 // A_GLOBAL: A is the AEV tile in global memory (row stride AEV_LEN), streamed; else A is a
 // row-major shared-memory activation with row stride lda.
 template <int TM, bool DEEP, int K, int N, bool A_GLOBAL>
 __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A, int lda,
                                          const float* __restrict__ Bg, bool active,
-                                         float (&acc)[MlpCfg<TM, DEEP>::R][N / 16]) {
+                                         float (&acc)[MlpCfg<TM, DEEP>::R][MlpCfg<TM, DEEP>::template nt<N>()]) {
   using Cfg = MlpCfg<TM, DEEP>;
-  constexpr int NT = N / 16;
+  constexpr int NT = Cfg::template nt<N>();
   constexpr int NF4 = N / 64;                            // float4 column groups per thread
   constexpr bool HAS2 = (N % 64) == 32;                  // plus one float2 group (N = 160, 96)
   constexpr int R = Cfg::R, S = Cfg::S, LEAD = Cfg::LEAD;
@@ -171,6 +204,36 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
   }
   auto compute = [&](int ch, uint32_t st) {
     const float* bs = P.Bs + st * MLP_BS_FLOATS;
+    if constexpr (PACKED) {                              // MlpLane's PACKED mapping
+      constexpr int NW = NT / 2;
+      constexpr bool SINGLE = (NT & 1) != 0;
+      const int ct = 16 * (w & 1) + (lane >> 1), r0 = 8 * (w >> 1) + 4 * (lane & 1);
+      const float* at = A_GLOBAL ? P.As + st * AS_FLOATS + r0 * MLP_AS_LD : A + (size_t)r0 * lda + ch * MLP_KC;
+      const int astr = A_GLOBAL ? MLP_AS_LD : lda;
+#pragma unroll
+      for (int k4 = 0; k4 < MLP_KC / 4; ++k4) {
+        float4 a[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) a[r] = *reinterpret_cast<const float4*>(at + r * astr + 4 * k4);
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {                    // k pair 2*k4 + j of the chunk: B2[pair][n][2]
+          const float* brow = bs + (2 * k4 + j) * (2 * N);
+          float2 b[NT];
+#pragma unroll
+          for (int f = 0; f < NW; ++f) {
+            const float4 v = *reinterpret_cast<const float4*>(brow + 2 * (64 * f + 2 * ct));
+            b[2 * f] = make_float2(v.x, v.y); b[2 * f + 1] = make_float2(v.z, v.w);
+          }
+          if (SINGLE) b[NT - 1] = *reinterpret_cast<const float2*>(brow + 2 * (64 * NW + ct));
+#pragma unroll
+          for (int r = 0; r < R; ++r) {
+            const float2 av = j == 0 ? make_float2(a[r].x, a[r].y) : make_float2(a[r].z, a[r].w);
+#pragma unroll
+            for (int c = 0; c < NT; ++c) ffma2(acc2[PACKED ? r : 0][PACKED ? c : 0], av, b[c]);
+          }
+        }
+      }
+    } else {
     const float* at = A_GLOBAL ? P.As + st * AS_FLOATS + rowbase * MLP_AS_LD
                                : A + (size_t)rowbase * lda + ch * MLP_KC;
     const int astr = 16 * (A_GLOBAL ? MLP_AS_LD : lda);
@@ -208,6 +271,7 @@ __device__ __forceinline__ void mlp_gemm(MlpPipe& P, const float* __restrict__ A
           }
         }
       }
+    }
     }
   };
   __syncthreads();                  // previous phase: activation stores visible, every staging buffer released
@@ -269,7 +333,8 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   pipe.gc = 0;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   constexpr int R = Cfg::R;
-  const int rowbase = 64 * (w >> 3) + (lane >> 1), cgi = 2 * (w & 7) + (lane & 1);
+  constexpr bool PACKED = Cfg::PACKED;
+  const MlpLane<TM, DEEP> L;
   const int row0 = blockIdx.x * TM;
   int el = 0;
 #pragma unroll
@@ -277,7 +342,7 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
   const float* __restrict__ Wp = P.wpack[el];
   const float* __restrict__ V = P.vec[el];
   if (row0 >= P.row_end[el]) return;                  // a tile of padding only (CTA-uniform)
-  const bool active = row0 + 64 * (w >> 3) < P.row_end[el];   // warp-uniform: my 64 rows hold an atom
+  const bool active = row0 + L.warp_row0() < P.row_end[el];   // warp-uniform: my warp's rows hold an atom
   if (tid == 0) {
     for (int st = 0; st < Cfg::S; ++st) {
       tc::mbar_init(&pipe.full[st], 1);
@@ -290,35 +355,35 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
 
   // ---- forward ----
   {
-    constexpr int NT = D1 / 16;
+    constexpr int NT = Cfg::template nt<D1>();
     float acc[R][NT];
     mlp_gemm<TM, DEEP, D0, D1, true>(pipe, aev + (size_t)row0 * AEV_LEN, 0, Wp + MLP_P_OFF0, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
-        const int n = mlp_col<D1>(cgi, c);
+        const int n = L.template col<D1>(c);
         const float bias = __ldg(V + MLP_V_B1 + n);
 #pragma unroll
-        for (int r = 0; r < R; ++r) H1[(rowbase + 16 * r) * MLP_LD1 + n] = celu_f(acc[r][c] + bias);
+        for (int r = 0; r < R; ++r) H1[L.row(r) * MLP_LD1 + n] = celu_f(acc[r][c] + bias);
       }
     }
   }
   {
-    constexpr int NT = D2 / 16;
+    constexpr int NT = Cfg::template nt<D2>();
     float acc[R][NT];
     mlp_gemm<TM, DEEP, D1, D2, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF1, active, acc);
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
-        const int n = mlp_col<D2>(cgi, c);
+        const int n = L.template col<D2>(c);
         const float bias = __ldg(V + MLP_V_B2 + n);
 #pragma unroll
-        for (int r = 0; r < R; ++r) H2[(rowbase + 16 * r) * MLP_LD2 + n] = celu_f(acc[r][c] + bias);
+        for (int r = 0; r < R; ++r) H2[L.row(r) * MLP_LD2 + n] = celu_f(acc[r][c] + bias);
       }
     }
   }
   {
-    constexpr int NT = D3 / 16;
+    constexpr int NT = Cfg::template nt<D3>();
     float acc[R][NT];
     mlp_gemm<TM, DEEP, D2, D3, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF2, active, acc);
     float part[R];
@@ -327,32 +392,40 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
     if (active) {
 #pragma unroll
       for (int c = 0; c < NT; ++c) {
-        const int n = mlp_col<D3>(cgi, c);
+        const int n = L.template col<D3>(c);
         const float bias = __ldg(V + MLP_V_B3 + n), w4 = __ldg(V + MLP_V_W4 + n);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
           const float h = celu_f(acc[r][c] + bias);
           part[r] = fmaf(w4, h, part[r]);
-          H3[(rowbase + 16 * r) * MLP_LD3 + n] = w4 * dcelu_from_h(h);   // delta3 = dE/dz3
+          H3[L.row(r) * MLP_LD3 + n] = w4 * dcelu_from_h(h);   // delta3 = dE/dz3
         }
       }
     }
-    // e_i = b4 + sum over the 96 columns: 2 lanes, then the 8 warps' column groups in a fixed tree
+    // e_i = b4 + sum over the 96 columns: the lanes that share my rows (fixed xor tree), then the
+    // column warps in a fixed order
 #pragma unroll
     for (int r = 0; r < R; ++r) {
       float s = part[r];
-      s += __shfl_xor_sync(0xffffffffu, s, 1);
-      if ((lane & 1) == 0) esum[(rowbase + 16 * r) * 8 + (w & 7)] = s;
+      if (PACKED) {
+        s += __shfl_xor_sync(0xffffffffu, s, 2); s += __shfl_xor_sync(0xffffffffu, s, 4);
+        s += __shfl_xor_sync(0xffffffffu, s, 8); s += __shfl_xor_sync(0xffffffffu, s, 16);
+        if (lane < 2) esum[L.row(r) * 8 + (w & 1)] = s;
+      } else {
+        s += __shfl_xor_sync(0xffffffffu, s, 1);
+        if ((lane & 1) == 0) esum[L.row(r) * 8 + (w & 7)] = s;
+      }
     }
     __syncthreads();
     if (tid < TM && row0 + tid < P.row_end[el]) {
       const float* p = esum + tid * 8;
-      e_row[row0 + tid] = (((p[0] + p[1]) + (p[2] + p[3])) + ((p[4] + p[5]) + (p[6] + p[7]))) + __ldg(V + MLP_V_B4);
+      const float sum = PACKED ? p[0] + p[1] : ((p[0] + p[1]) + (p[2] + p[3])) + ((p[4] + p[5]) + (p[6] + p[7]));
+      e_row[row0 + tid] = sum + __ldg(V + MLP_V_B4);
     }
   }
   // ---- backward (input gradient only) ----
   {
-    constexpr int NT = D2 / 16;
+    constexpr int NT = Cfg::template nt<D2>();
     float acc[R][NT];
     mlp_gemm<TM, DEEP, D3, D2, false>(pipe, H3, MLP_LD3, Wp + MLP_P_OFF3, active, acc);
     if (active) {
@@ -360,13 +433,13 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
       for (int c = 0; c < NT; ++c)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-          float* hp = H2 + (rowbase + 16 * r) * MLP_LD2 + mlp_col<D2>(cgi, c);
+          float* hp = H2 + L.row(r) * MLP_LD2 + L.template col<D2>(c);
           *hp = acc[r][c] * dcelu_from_h(*hp);          // delta2 over h2 (own elements only)
         }
     }
   }
   {
-    constexpr int NT = D1 / 16;
+    constexpr int NT = Cfg::template nt<D1>();
     float acc[R][NT];
     mlp_gemm<TM, DEEP, D2, D1, false>(pipe, H2, MLP_LD2, Wp + MLP_P_OFF4, active, acc);
     if (active) {
@@ -374,21 +447,26 @@ k3_mlp_fp32_kernel(const __grid_constant__ MlpParams P, const float* __restrict_
       for (int c = 0; c < NT; ++c)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-          float* hp = H1 + (rowbase + 16 * r) * MLP_LD1 + mlp_col<D1>(cgi, c);
+          float* hp = H1 + L.row(r) * MLP_LD1 + L.template col<D1>(c);
           *hp = acc[r][c] * dcelu_from_h(*hp);          // delta1
         }
     }
   }
 #pragma unroll 1
   for (int pass = 0; pass < D0 / 128; ++pass) {
-    float acc[R][8];
+    float acc[R][Cfg::template nt<128>()];
     mlp_gemm<TM, DEEP, D1, 128, false>(pipe, H1, MLP_LD1, Wp + MLP_P_OFF5 + pass * D1 * 128, active, acc);
     if (active) {
 #pragma unroll
       for (int r = 0; r < R; ++r) {
-        float* dst = g + (size_t)(row0 + rowbase + 16 * r) * AEV_LEN + pass * 128 + 4 * cgi;
-        *reinterpret_cast<float4*>(dst) = make_float4(acc[r][0], acc[r][1], acc[r][2], acc[r][3]);
-        *reinterpret_cast<float4*>(dst + 64) = make_float4(acc[r][4], acc[r][5], acc[r][6], acc[r][7]);
+        float* dst = g + (size_t)(row0 + L.row(r)) * AEV_LEN + pass * 128;
+        if constexpr (PACKED) {
+          *reinterpret_cast<float2*>(dst + 2 * L.ct()) = make_float2(acc[r][0], acc[r][1]);
+          *reinterpret_cast<float2*>(dst + 64 + 2 * L.ct()) = make_float2(acc[r][2], acc[r][3]);
+        } else {
+          *reinterpret_cast<float4*>(dst + 4 * L.ct()) = make_float4(acc[r][0], acc[r][1], acc[r][2], acc[r][3]);
+          *reinterpret_cast<float4*>(dst + 64 + 4 * L.ct()) = make_float4(acc[r][4], acc[r][5], acc[r][6], acc[r][7]);
+        }
       }
     }
   }
