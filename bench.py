@@ -36,8 +36,8 @@ DT_FS = 0.5
 MLP_FLOPS_PER_ATOM = 4.0 * 94304                     # fwd + bwd, 94,304 MAC each, 2 flop per MAC = 377,216
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.5: SMs x FP32 lanes x 2 x max SM clock
 # dram__bytes_read.sum + dram__bytes_write.sum of one K3 launch, from the committed ncu --set full
-# captures (config 4 only): FFMA path profiles/r1c_fp32.md (353.2 + 307.0 MB), tensor path r1b_tc.md
-K3_TRAFFIC_BYTES = {(4, 0): 660.2e6}
+# capture (config 4, FFMA path): profiles/r1d_fp32.md (353.2 + 305.6 MB)
+K3_TRAFFIC_BYTES = {(4, 0): 658.8e6}
 
 
 def _peaks():
@@ -251,7 +251,7 @@ def run_pfc(args):
                     "peak_source": f"{peak_src} bf16 sustained x 0.5 (tf32:bf16 nominal ratio); "
                                    "achieved counts algorithmic flops once, the 3-term split issues 3x"}
         roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": K3_TRAFFIC_BYTES.get((args.config, args.mlp)),
-                     "traffic_source": "profiles/r1c_fp32.md (ncu --set full, one launch)"
+                     "traffic_source": "profiles/r1d_fp32.md (ncu --set full, one launch)"
                                        if (args.config, args.mlp) in K3_TRAFFIC_BYTES else None,
                      "algorithmic_bytes": 2 * 1536 * N,   # aev row read + g row written per atom
                      "kernel": "K3 MLP fwd+bwd",
