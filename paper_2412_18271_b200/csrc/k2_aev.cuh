@@ -201,6 +201,7 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __re
       while (t0 + n >= S.pre[bcur + 1]) ++bcur;
       const int hi = min(nt, S.pre[bcur + 1] - t0);
       float a2 = 0.0f;
+#pragma unroll 4
       for (; n < hi; ++n) a2 = fmaf(S.tA[n][pb], S.tW[n][pa], a2);
       S.out[RAD_LEN + 32 * bcur + lane] += a2;
     }

@@ -513,7 +513,10 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
     // with several CTAs per SM the ring is slower: config 4 2.52 ms, config 3 0.27 ms).
     // PFC_K3_TM / PFC_K3_DEEP override (tuning only).
     auto tiles = [&](int tm) { int n = 0; for (int e = 0; e < NSPEC; ++e) n += (count[e] + tm - 1) / tm; return n; };
-    c->mlp_tm = tiles(32) >= c->n_sms ? 32 : 16;
+    // (16-row tiles only when they spread the batch over clearly more SMs than 32-row tiles would:
+    // config 2, 95 vs 48 tiles, 47 vs 53 us; config 0 has 4 tiles either way and the packed 32-row
+    // kernel takes 37 us against 45 us)
+    c->mlp_tm = (tiles(32) >= c->n_sms || 2 * tiles(16) < 3 * tiles(32)) ? 32 : 16;
     c->mlp_deep = c->mlp_tm == 16;
     if (const char* ov = getenv("PFC_K3_TM")) {
       const int v = atoi(ov);
