@@ -397,3 +397,34 @@ def test_nve_energy_conservation_on_gpu(pfc, weights):
     assert np.abs(H - H[0]).max() < 5e-4
     assert np.abs(H - Href).max() < 2e-5
     p.close()
+
+
+# ---- every K3 tile variant, on element blocks that end inside a warp's rows / a tile ----------------
+@pytest.mark.parametrize("tm,deep", [(16, 0), (16, 1), (32, 0), (32, 1), (64, 0), (128, 0)])
+def test_k3_tile_variants_on_ragged_element_blocks(pfc, weights, tm, deep, monkeypatch):
+    """pfc_create picks one tile height per batch; PFC_K3_TM / PFC_K3_DEEP (tuning overrides) force the
+    others.  Element counts 1 / 9 / 33 / 41 end inside an 8-row warp group, a 16-row and a 32-row tile."""
+    rng = np.random.default_rng(20241218)
+    counts = [33, 41, 1, 9]                                     # H, C, N, O
+    species = np.repeat(np.arange(4, dtype=np.int32), counts)
+    rng.shuffle(species)
+    n = species.size
+    pts = []
+    while len(pts) < n:                                          # >= 1.0 A apart in a ball at 0.1 / A^3
+        c = rng.normal(size=3); c *= 5.8 * rng.random() ** (1 / 3) / np.linalg.norm(c)
+        if all(np.linalg.norm(c - q) >= 1.0 for q in pts):
+            pts.append(c)
+    pos = np.asarray(pts, dtype=np.float32)
+    off = np.array([0, 30, n], dtype=np.int32)                   # two systems
+    monkeypatch.setenv("PFC_K3_TM", str(tm))
+    monkeypatch.setenv("PFC_K3_DEEP", str(deep))
+    p = pfc.Pfc(species, off, weights)
+    E, F = p.energy_forces(_dev(pfc, pos))
+    torch.cuda.synchronize()
+    ref = oracle.energy_forces(pos.astype(np.float64), species, off, weights)
+    Eh, Fh = E.cpu().numpy().astype(np.float64), F.cpu().numpy().astype(np.float64)
+    assert (np.abs(Eh - ref["E"]) <= E_RTOL * np.maximum(np.abs(ref["E"]), 1.0)).all()
+    assert np.abs(Fh[:, :3] - ref["F"]).max() <= F_ATOL_INTERNAL
+    assert np.abs(Fh[:, 3] - ref["e"]).max() <= 1e-5 * max(1.0, np.abs(ref["e"]).max())   # per-atom energies
+    assert p.status() == 0
+    p.close()
