@@ -182,11 +182,14 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __re
       const float s = sqrtf(fmaf(-c, c, 1.0f));
       const float rbar = 0.5f * (uj.w + uk.w);
       const float w2 = 2.0f * S.fc[j] * S.fc[k];
+      const float2 cc2 = make_float2(c, c), ss2 = make_float2(s, s), half2 = make_float2(0.5f, 0.5f);
 #pragma unroll
-      for (int b = 0; b < NSHF_Z; ++b) {
-        float q1 = fmaf(0.5f, fmaf(c, c_tab.cos_z[b], s * c_tab.sin_z[b]), 0.5f);
-        q1 *= q1; q1 *= q1; q1 *= q1; q1 *= q1; q1 *= q1;           // ^32
-        S.tA[lane][b] = q1;
+      for (int b = 0; b < NSHF_Z / 2; ++b) {                        // two shifts at a time (packed fp32 pairs)
+        const float2 cz = make_float2(c_tab.cos_z[2 * b], c_tab.cos_z[2 * b + 1]);
+        const float2 sz = make_float2(c_tab.sin_z[2 * b], c_tab.sin_z[2 * b + 1]);
+        float2 q1 = pk_fma(half2, pk_fma(cc2, cz, pk_mul(ss2, sz)), half2);
+        q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1);   // ^32
+        *reinterpret_cast<float2*>(&S.tA[lane][2 * b]) = q1;
       }
 #pragma unroll
       for (int a = 0; a < NSHF_A; ++a) {

@@ -139,25 +139,31 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
       const float s = sqrtf(fmaf(-c, c, 1.0f));
       const float rbar = 0.5f * (uj.w + uk.w);
       const float* gp = S.gA + GA_STRIDE * pair_block(__float_as_int(fj.z), __float_as_int(fk.z));
-      float A[NSHF_Z], dA[NSHF_Z];
+      // angular factors two shifts at a time (packed fp32 pairs: half the issue slots)
+      float2 A2[NSHF_Z / 2], dA2[NSHF_Z / 2];
+      const float2 c2 = make_float2(c, c), s2 = make_float2(s, s), nc2 = make_float2(-c, -c);
+      const float2 half2 = make_float2(0.5f, 0.5f), m16 = make_float2(-16.0f, -16.0f);
 #pragma unroll
-      for (int b = 0; b < NSHF_Z; ++b) {
-        const float cz = c_tab.cos_z[b], sz_ = c_tab.sin_z[b];
-        const float q1 = fmaf(0.5f, fmaf(c, cz, s * sz_), 0.5f);
-        const float q2 = q1 * q1, q4 = q2 * q2, q8 = q4 * q4, q16 = q8 * q8;
-        A[b] = q16 * q16;
+      for (int b = 0; b < NSHF_Z / 2; ++b) {
+        const float2 cz = make_float2(c_tab.cos_z[2 * b], c_tab.cos_z[2 * b + 1]);
+        const float2 sz_ = make_float2(c_tab.sin_z[2 * b], c_tab.sin_z[2 * b + 1]);
+        const float2 q1 = pk_fma(half2, pk_fma(c2, cz, pk_mul(s2, sz_)), half2);
+        const float2 q2 = pk_mul(q1, q1), q4 = pk_mul(q2, q2), q8 = pk_mul(q4, q4), q16 = pk_mul(q8, q8);
+        A2[b] = pk_mul(q16, q16);
         // dA/dtheta = -16 q^31 sin(theta - theta_b),  sin(theta - theta_b) = s cz - c sz
-        dA[b] = -16.0f * (q16 * q8 * q4 * q2 * q1) * fmaf(s, cz, -c * sz_);
+        const float2 q31 = pk_mul(pk_mul(pk_mul(q16, q8), pk_mul(q4, q2)), q1);
+        dA2[b] = pk_mul(pk_mul(q31, m16), pk_fma(s2, cz, pk_mul(nc2, sz_)));
       }
       float G0 = 0.f, Gr = 0.f, Gt = 0.f;
 #pragma unroll
       for (int a = 0; a < NSHF_A; ++a) {
         const float4 g0 = *reinterpret_cast<const float4*>(gp + 8 * a);
         const float4 g1 = *reinterpret_cast<const float4*>(gp + 8 * a + 4);
-        const float ua = g0.x * A[0] + g0.y * A[1] + g0.z * A[2] + g0.w * A[3] +
-                         g1.x * A[4] + g1.y * A[5] + g1.z * A[6] + g1.w * A[7];
-        const float va = g0.x * dA[0] + g0.y * dA[1] + g0.z * dA[2] + g0.w * dA[3] +
-                         g1.x * dA[4] + g1.y * dA[5] + g1.z * dA[6] + g1.w * dA[7];
+        const float2 ga = make_float2(g0.x, g0.y), gb = make_float2(g0.z, g0.w), gc = make_float2(g1.x, g1.y),
+                     gd = make_float2(g1.z, g1.w);
+        const float2 u2 = pk_fma(gd, A2[3], pk_fma(gc, A2[2], pk_fma(gb, A2[1], pk_mul(ga, A2[0]))));
+        const float2 v2 = pk_fma(gd, dA2[3], pk_fma(gc, dA2[2], pk_fma(gb, dA2[1], pk_mul(ga, dA2[0]))));
+        const float ua = u2.x + u2.y, va = v2.x + v2.y;
         const float dr = rbar - c_tab.shf_a[a];
         const float B = ex2_approx(-(ETA_A * LOG2E) * dr * dr);
         const float dB = -2.0f * ETA_A * dr * B;

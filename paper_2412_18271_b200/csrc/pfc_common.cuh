@@ -76,6 +76,19 @@ __device__ __forceinline__ int pair_block(int za, int zb) {
   return s1 * NSPEC - ((s1 * (s1 - 1)) >> 1) + (s2 - s1);
 }
 
+// Packed fp32 pairs (sm_100: SASS FFMA2 / FMUL2): one issue slot for two lanes of arithmetic.
+__device__ __forceinline__ float2 pk_fma(float2 a, float2 b, float2 c) {
+  unsigned long long ua = *reinterpret_cast<unsigned long long*>(&a), ub = *reinterpret_cast<unsigned long long*>(&b),
+                     uc = *reinterpret_cast<unsigned long long*>(&c), ud;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(ud) : "l"(ua), "l"(ub), "l"(uc));
+  return *reinterpret_cast<float2*>(&ud);
+}
+__device__ __forceinline__ float2 pk_mul(float2 a, float2 b) {
+  unsigned long long ua = *reinterpret_cast<unsigned long long*>(&a), ub = *reinterpret_cast<unsigned long long*>(&b), ud;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(ud) : "l"(ua), "l"(ub));
+  return *reinterpret_cast<float2*>(&ud);
+}
+
 // Ampere-style asynchronous 16-byte copies global -> shared (L2 only, no L1 allocation)
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
