@@ -285,8 +285,14 @@ def run_pfc(args):
         rate, _ = _oracle_steps_per_s(swl, weights, 1)               # calibration: atom-evaluations / s
         n_cpu_steps = int(min(400, max(3, 12.0 * rate / swl.n_atoms)))   # about 12 s of CPU work
         cpu_v, cpu_t = _oracle_steps_per_s(swl, weights, n_cpu_steps)
-        cpu = {"value": cpu_v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"{what}, {n_cpu_steps} steps ({cpu_t:.1f} s)"}
+        cores = oracle.num_threads()
+        oracle.set_num_threads(1)                                    # and on one core: ~3 s
+        one_wl, one_what = _sample_workload(args.config, 1400)
+        one_v, one_t = _oracle_steps_per_s(one_wl, weights, int(min(200, max(2, 3.0 * rate / cores / one_wl.n_atoms))))
+        oracle.set_num_threads(cores)
+        cpu = {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"{what}, {n_cpu_steps} steps ({cpu_t:.1f} s)",
+               "single_thread": {"value": one_v, "sample": f"{one_what} ({one_t:.1f} s)"}}
 
         steps_per_s = args.steps / t
         line = {
