@@ -37,7 +37,9 @@ MLP_FLOPS_PER_ATOM = 4.0 * 94304                     # fwd + bwd, 94,304 MAC eac
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.5: SMs x FP32 lanes x 2 x max SM clock
 # dram__bytes_read.sum + dram__bytes_write.sum of one K3 launch, from the committed ncu --set full
 # capture (config 4, FFMA path): profiles/r1d_fp32.md (353.2 + 305.6 MB)
-K3_TRAFFIC_BYTES = {(4, 0): 658.8e6}
+K3_TRAFFIC_BYTES = {(4, 0): 658.8e6, (4, 1): 668.5e6}
+K3_TRAFFIC_SOURCE = {(4, 0): "profiles/r1d_fp32.md (ncu --set full, one launch)",
+                     (4, 1): "profiles/r1e_tc.md (ncu --set full, one launch)"}
 
 
 def _peaks():
@@ -198,6 +200,7 @@ def run_pfc(args):
     N = wl.n_atoms
     stream = torch.cuda.Stream(device=dev)
     p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=args.mlp, device=dev)
+    mlp = p.mlp_path()                                            # MLP_AUTO resolved by pfc_create
     pos0, vel0 = pfc.pack4(wl.pos), pfc.pack4(wl.vel)
     pos, vel = torch.from_numpy(pos0).to(dev), torch.from_numpy(vel0).to(dev)
     with torch.cuda.stream(stream):
@@ -242,7 +245,7 @@ def run_pfc(args):
         stage_ms /= reps
         k3_s = stage_ms[2] * 1e-3
         flops = MLP_FLOPS_PER_ATOM * N
-        if args.mlp == pfc.MLP_FP32:
+        if mlp == pfc.MLP_FP32:
             roof = {"bound": "alu", "achieved": flops / k3_s / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and max SM clock)"}
         else:
@@ -250,9 +253,8 @@ def run_pfc(args):
                     "peak": 0.5 * peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
                     "peak_source": f"{peak_src} bf16 sustained x 0.5 (tf32:bf16 nominal ratio); "
                                    "achieved counts algorithmic flops once, the 3-term split issues 3x"}
-        roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": K3_TRAFFIC_BYTES.get((args.config, args.mlp)),
-                     "traffic_source": "profiles/r1d_fp32.md (ncu --set full, one launch)"
-                                       if (args.config, args.mlp) in K3_TRAFFIC_BYTES else None,
+        roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": K3_TRAFFIC_BYTES.get((args.config, mlp)),
+                     "traffic_source": K3_TRAFFIC_SOURCE.get((args.config, mlp)),
                      "algorithmic_bytes": 2 * 1536 * N,   # aev row read + g row written per atom
                      "kernel": "K3 MLP fwd+bwd",
                      "kernel_ms": float(stage_ms[2]),
@@ -298,9 +300,12 @@ def run_pfc(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if mlp == 0 else "tf32x3",    # MLP contractions as a 3-term tf32 split, fp32 accumulate; all else f32
+            "data": "synthetic",
             "config": {"workload": wl.name, "config_index": args.config, "atoms": N, "systems": wl.n_systems,
-                       "dt_fs": DT_FS, "integrator": args.integrator, "mlp_path": "fp32_ffma" if args.mlp == 0 else "tf32x3_tcgen05",
+                       "dt_fs": DT_FS, "integrator": args.integrator, "mlp_path": "fp32_ffma" if mlp == 0 else "tf32x3_tcgen05",
+                       "mlp_path_requested": {0: "fp32", 1: "tf32x3", 2: "tf32x1", 3: "auto"}[args.mlp],
                        "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "per-step working set (aev + g + lists + edge) exceeds the 126 MB L2"
                              if N * 3072 > 126e6 else "working set fits L2: neighbour/AEV/MLP buffers are "
@@ -348,7 +353,8 @@ def main():
     ap.add_argument("--impl", default="pfc", choices=["pfc", "reference"])
     ap.add_argument("--integrator", default="verlet", choices=["verlet", "langevin"],
                     help="langevin = the paper's timing protocol (friction 0.1 ps^-1, 10 frames), PAPER.md:94")
-    ap.add_argument("--mlp", type=int, default=0, help="0 = FP32 FFMA, 1 = tcgen05 TF32x3")
+    ap.add_argument("--mlp", type=int, default=3, choices=[0, 1, 3],
+                    help="3 = auto (library default: tensor-core MLP from 4096 atoms on), 0 = FP32 FFMA, 1 = tcgen05 TF32x3")
     ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (100 steps each)")
     args = ap.parse_args()
     INTEGRATOR["kind"] = args.integrator

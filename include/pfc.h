@@ -67,6 +67,7 @@ extern "C" {
 #define PFC_MLP_FP32 0                  /* FP32 FFMA grouped MLP                 */
 #define PFC_MLP_TF32X3 1                /* tcgen05 kind::tf32, 3-term split      */
 #define PFC_MLP_TF32X1 2                /* tcgen05 plain TF32: tolerance evidence only (fails it) */
+#define PFC_MLP_AUTO 3                  /* TF32X3 for batches of >= 4096 atoms, FP32 below */
 
 typedef struct pfc_ctx pfc_t;           /* opaque; owned by the library          */
 
@@ -84,7 +85,7 @@ typedef struct {
   const float *masses_amu;       /* HOST [4] or NULL -> {1.008,12.011,14.007,15.999} */
   void *workspace;               /* DEVICE, 256-byte aligned, >= pfc_workspace_bytes() */
   size_t workspace_bytes;
-  int32_t mlp_path;              /* PFC_MLP_FP32, PFC_MLP_TF32X3 (or PFC_MLP_TF32X1) */
+  int32_t mlp_path;              /* PFC_MLP_AUTO (recommended), PFC_MLP_FP32, PFC_MLP_TF32X3 (or PFC_MLP_TF32X1) */
 } pfc_desc_t;
 
 /* Bytes of device workspace pfc_create needs for these sizes (0 on bad args). */
@@ -188,6 +189,9 @@ int pfc_copy_to_host(const void *device_src, void *host_dst, size_t bytes);
 
 /* Synchronises the bound/last-used stream and returns the sticky status bits. */
 int pfc_status(pfc_t *ctx, uint32_t *bits);
+
+/* The MLP path in use (PFC_MLP_AUTO resolved by pfc_create). */
+int pfc_mlp_path(pfc_t *ctx, int32_t *path);
 
 /* Number of kernel launches one energy_forces pass / one MD step enqueues. */
 int pfc_launch_counts(pfc_t *ctx, int32_t *per_energy_forces, int32_t *per_step);

@@ -72,6 +72,7 @@ struct TcParams {
   const float* bias[NSPEC];    // per element: b1[160] b2[128] b3[96] w4[96] b4[1]  (481 floats)
   int row_start[NSPEC + 1];
   int n_tiles;
+  float comp[6];               // expected relative truncation loss of the accumulator chain of phases 0..4 and the g passes
 };
 constexpr int TC_BIAS_B1 = 0, TC_BIAS_B2 = D1, TC_BIAS_B3 = D1 + D2, TC_BIAS_W4 = D1 + D2 + D3,
               TC_BIAS_B4 = D1 + D2 + D3 + D3, TC_BIAS_LEN = 484;
@@ -204,7 +205,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           tc::tmem_ld16(tlane + TC_S0_COL + 32 * c + 16 * hf, sm);
           tc::tmem_ld_wait();
 #pragma unroll
-          for (int k = 0; k < 16; ++k) z[k] = (z[k] + sm[k]) + __ldg(b + k);
+          for (int k = 0; k < 16; ++k) { const float t = z[k] + sm[k]; z[k] = fmaf(t, P.comp[0], t) + __ldg(b + k); }
         } else {
           tc::tmem_ld_wait();
 #pragma unroll
@@ -226,7 +227,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
         tc::tmem_ld_wait();
         const float* b = bias + TC_BIAS_B2 + 32 * c + 16 * hf;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) celu_both(z[k] + __ldg(b + k), h[k], d);
+        for (int k = 0; k < 16; ++k) celu_both(fmaf(z[k], P.comp[1], z[k]) + __ldg(b + k), h[k], d);
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish();
@@ -253,7 +254,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           for (int k = 0; k < 16; ++k) {
             float h, d;
             const float w = __ldg(w4 + k);
-            celu_both(z[k] + __ldg(b + k), h, d);
+            celu_both(fmaf(z[k], P.comp[2], z[k]) + __ldg(b + k), h, d);
             epart = fmaf(w, h, epart);
             dl[k] = w * d;
           }
@@ -276,8 +277,8 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
 #pragma unroll
         for (int k = 0; k < 16; ++k) {
           float h, d;
-          celu_both(z[k] + __ldg(b + k), h, d);
-          p[k] *= d;
+          celu_both(fmaf(z[k], P.comp[1], z[k]) + __ldg(b + k), h, d);
+          p[k] = fmaf(p[k], P.comp[3], p[k]) * d;
         }
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, p);
@@ -295,7 +296,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           for (int k = 0; k < 16; ++k) {
             float h, d;
             celu_both(z[k], h, d);                             // z1 already holds the bias
-            p[k] *= d;
+            p[k] = fmaf(p[k], P.comp[4], p[k]) * d;
           }
           uint8_t* slot = acquire();
           tc_store_a16(slot, r, hf, p);
@@ -311,9 +312,13 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           tc::tmem_ld_wait();
 #pragma unroll
           for (int k = 0; k < 4; ++k) {
-            reinterpret_cast<float4*>(dst + 32 * c)[k] = make_float4(v0[4 * k], v0[4 * k + 1], v0[4 * k + 2], v0[4 * k + 3]);
+            const float cg = P.comp[5];
+            reinterpret_cast<float4*>(dst + 32 * c)[k] =
+                make_float4(fmaf(cg, v0[4 * k], v0[4 * k]), fmaf(cg, v0[4 * k + 1], v0[4 * k + 1]),
+                            fmaf(cg, v0[4 * k + 2], v0[4 * k + 2]), fmaf(cg, v0[4 * k + 3], v0[4 * k + 3]));
             reinterpret_cast<float4*>(dst + 32 * (c + 1))[k] =
-                make_float4(v1[4 * k], v1[4 * k + 1], v1[4 * k + 2], v1[4 * k + 3]);
+                make_float4(fmaf(cg, v1[4 * k], v1[4 * k]), fmaf(cg, v1[4 * k + 1], v1[4 * k + 1]),
+                            fmaf(cg, v1[4 * k + 2], v1[4 * k + 2]), fmaf(cg, v1[4 * k + 3], v1[4 * k + 3]));
           }
         }
         tc::tc_fence_before();

@@ -311,7 +311,8 @@ size_t pfc_workspace_bytes(int32_t n_atoms, int32_t n_systems) {
 int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (!d || !out || !d->species || !d->sys_offsets || !d->weights) return PFC_ERR_ARG;
   if (d->n_atoms < 1 || d->n_systems < 1 || d->n_systems > d->n_atoms) return PFC_ERR_ARG;
-  if (d->mlp_path != PFC_MLP_FP32 && d->mlp_path != PFC_MLP_TF32X3 && d->mlp_path != PFC_MLP_TF32X1)
+  if (d->mlp_path != PFC_MLP_FP32 && d->mlp_path != PFC_MLP_TF32X3 && d->mlp_path != PFC_MLP_TF32X1 &&
+      d->mlp_path != PFC_MLP_AUTO)
     return PFC_ERR_ARG;
   const int N = d->n_atoms, NS = d->n_systems;
   if (d->sys_offsets[0] != 0 || d->sys_offsets[NS] != N) return PFC_ERR_SPECIES;
@@ -327,7 +328,9 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
 
   pfc_ctx* c = new (std::nothrow) pfc_ctx();
   if (!c) return PFC_ERR_ARG;
-  c->mlp_path = d->mlp_path;
+  // AUTO: the tensor-core MLP pays from a few thousand atoms on (config 1, 5,632 atoms: 0.125 vs 0.140
+  // ms/step; config 2, 1,500 atoms: 0.141 vs 0.114), where its 128-row tiles start to fill the SMs
+  c->mlp_path = d->mlp_path == PFC_MLP_AUTO ? (d->n_atoms >= 4096 ? PFC_MLP_TF32X3 : PFC_MLP_FP32) : d->mlp_path;
   c->sz = worst_case_sizes(N, NS);                      // capacities are the worst-case ones
   // static element grouping: rows sorted by element, blocks padded to ROW_PAD
   int row_start[NSPEC + 1];
@@ -444,6 +447,14 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   c->tcp.wpack = c->b.wtc;
   for (int e = 0; e <= NSPEC; ++e) c->tcp.row_start[e] = row_start[e];
   c->tcp.n_tiles = c->sz.n_rows / TC_TM;
+  {
+    // truncation steps of the main accumulator chain per phase (K/8, x3 where the three split terms
+    // share one accumulator); PFC_TC_COMP_F / _B scale the forward / backward compensation (experiment)
+    const int ntr[6] = {48, 60, 16, 36, 48, 60};
+    const float lf = getenv("PFC_TC_COMP_F") ? (float)atof(getenv("PFC_TC_COMP_F")) : 0.9f;
+    const float lb = getenv("PFC_TC_COMP_B") ? (float)atof(getenv("PFC_TC_COMP_B")) : 0.73f;
+    for (int q = 0; q < 6; ++q) c->tcp.comp[q] = (q < 3 ? lf : lb) * (float)ntr[q] * 2.15e-8f;
+  }
 
   ModelTables tab;
   {
@@ -733,6 +744,12 @@ int pfc_status(pfc_t* c, uint32_t* bits) {
   if (!c || !bits) return PFC_ERR_ARG;
   if (cudaStreamSynchronize(c->stream) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpy(bits, c->b.status, sizeof(uint32_t), cudaMemcpyDeviceToHost) != cudaSuccess) return PFC_ERR_CUDA;
+  return PFC_OK;
+}
+
+int pfc_mlp_path(pfc_t* c, int32_t* path) {
+  if (!c || !path) return PFC_ERR_ARG;
+  *path = c->mlp_path;
   return PFC_OK;
 }
 

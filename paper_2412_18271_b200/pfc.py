@@ -23,6 +23,7 @@ N_WEIGHTS = 378756
 MLP_FP32 = 0
 MLP_TF32X3 = 1
 MLP_TF32X1 = 2            # plain TF32: tolerance evidence only
+MLP_AUTO = 3              # TF32X3 from 4096 atoms on, FP32 below
 
 STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
                4: "angular row longer than PFC_MAX_ANGULAR", 8: "non-finite energy",
@@ -33,7 +34,7 @@ STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gathe
 
 EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy_forces_nm", "pfc_profile_stages", "pfc_set_state", "pfc_step",
            "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host", "pfc_run_host_resume", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
-           "pfc_copy_to_host", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
+           "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
 
 
 class PfcError(RuntimeError):
@@ -80,6 +81,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_get_intermediates.argtypes = [c_void_p, pp_f, pp_f, pp_i32, POINTER(c_int32)]
     lib.pfc_copy_to_host.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.pfc_status.argtypes = [c_void_p, POINTER(c_uint32)]
+    lib.pfc_mlp_path.argtypes = [c_void_p, POINTER(c_int32)]
     lib.pfc_launch_counts.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32)]
     lib.pfc_destroy.argtypes = [c_void_p]
     lib.pfc_error_string.argtypes = [c_int]
@@ -109,7 +111,7 @@ def _stream_ptr(stream) -> int:
 class Pfc:
     """One handle = one set of systems + one potential (pfc_create .. pfc_destroy)."""
 
-    def __init__(self, species, sys_offsets, weights, masses_amu=None, mlp_path: int = MLP_FP32,
+    def __init__(self, species, sys_offsets, weights, masses_amu=None, mlp_path: int = MLP_AUTO,
                  device="cuda:0"):
         import torch
         if not torch.cuda.is_available():
@@ -230,6 +232,12 @@ class Pfc:
                                              float(dt_fs), ptr(E_host), _stream_ptr(stream)), "pfc_run_host_resume")
 
     # -- getters ------------------------------------------------------------------
+    def mlp_path(self) -> int:
+        """The MLP path in use (MLP_AUTO resolved)."""
+        v = c_int32()
+        _check(self._lib.pfc_mlp_path(self._h, byref(v)), "pfc_mlp_path")
+        return int(v.value)
+
     def status(self) -> int:
         bits = c_uint32()
         _check(self._lib.pfc_status(self._h, byref(bits)), "pfc_status")
