@@ -75,10 +75,14 @@ def _check_energy_forces(E, F, ref, tight=True):
 
 
 # ---- step 0 on every config at full size: lists, E, F --------------------------------
-@pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
-def test_step0_lists_energy_forces_full_size(pfc, weights, k):
+# (the default MLP path is PFC_MLP_AUTO: the compensated tensor-core MLP on configs 1, 3, 4, FP32 FFMA on
+# configs 0 and 2; "fp32" pins the FFMA path on the large configs as well)
+@pytest.mark.parametrize("k,path", [(0, "auto"), (1, "auto"), (2, "auto"), (3, "auto"), (4, "auto"),
+                                    (1, "fp32"), (3, "fp32"), (4, "fp32")])
+def test_step0_lists_energy_forces_full_size(pfc, weights, k, path):
     wl = cfg(k)
-    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_AUTO if path == "auto" else pfc.MLP_FP32)
+    assert p.mlp_path() == (pfc.MLP_TF32X3 if (path == "auto" and wl.n_atoms >= 4096) else pfc.MLP_FP32)
     E, F = p.energy_forces(_dev(pfc, wl.pos))
     assert p.status() == 0
     # the definition is the O(N^2) enumeration; config 3 (20,000 atoms) goes through the
@@ -104,8 +108,8 @@ def test_config3_brute_force_enumeration_matches_cell_path(pfc, weights):
 
 
 # ---- 100-step trajectories -----------------------------------------------------------
-def _trajectory(pfc, weights, wl, n_steps, cell=False):
-    p = pfc.Pfc(wl.species, wl.sys_offsets, weights)
+def _trajectory(pfc, weights, wl, n_steps, cell=False, mlp_path=None):
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_AUTO if mlp_path is None else mlp_path)
     pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
     E, F = p.set_state(pos, vel)
     p.step(n_steps, wl.dt_fs)
@@ -153,6 +157,12 @@ def test_trajectory_config2(pfc, weights):
 
 def test_trajectory_config3_full_size(pfc, weights):
     _trajectory(pfc, weights, cfg(3), 100, cell=True)
+
+
+def test_trajectory_fp32_path_configs_1_and_3(pfc, weights):
+    """The FFMA path on the two configs whose default is the tensor-core MLP."""
+    _trajectory(pfc, weights, cfg(1), 100, mlp_path=pfc.MLP_FP32)
+    _trajectory(pfc, weights, cfg(3), 100, cell=True, mlp_path=pfc.MLP_FP32)
 
 
 def test_trajectory_config4_subset_of_64_replicas(pfc, weights):

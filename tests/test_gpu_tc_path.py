@@ -111,12 +111,30 @@ def test_tf32x3_trajectory_config0(pfc, weights):
 
 
 def test_tf32x3_trajectory_config1(pfc, weights):
-    """The decision case: 255 of the 256 replicas stay within 1e-4 A (median
-    2e-6 A), but the most chaotic one (replica 68: 2.0e-5 A on the FP32 path) reaches 4.6e-4 A with
-    the tensor-core MLP, whose accumulator truncation makes g about 4x less accurate than FFMA.
-    That misses north_star's trajectory bar, so FP32 FFMA stays the default K3 and this path is
-    opt-in; the test pins what the path does deliver."""
-    _trajectory(pfc, weights, W.make_config(1), 100, allow_outliers=1)
+    """The decision case.  Without the truncation compensation 255 of the 256
+    replicas stay within 1e-4 A but the most chaotic one (2.0e-5 A on the FP32 path) reaches 4.6e-4 A:
+    the accumulator's round-toward-zero loss is one-sided and integrates coherently.  With the
+    compensation (the shipped path) every replica stays within the bar (worst 3.8e-5 A)."""
+    _trajectory(pfc, weights, W.make_config(1), 100)
+
+
+def test_uncompensated_tf32x3_misses_the_trajectory_bar(pfc, weights, monkeypatch):
+    """Evidence for the compensation: switched off (PFC_TC_COMP_F/B = 0, experiment overrides) the
+    worst replica of config 1 leaves the 1e-4 A bar while all the others keep it."""
+    monkeypatch.setenv("PFC_TC_COMP_F", "0")
+    monkeypatch.setenv("PFC_TC_COMP_B", "0")
+    wl = W.make_config(1)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TF32X3)
+    pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+    p.set_state(pos, vel)
+    p.step(100, wl.dt_fs)
+    torch.cuda.synchronize()
+    ref = oracle.step(wl.pos, wl.vel, wl.species, wl.sys_offsets, weights, wl.dt_fs, 100)
+    d2 = ((pos.cpu().numpy()[:, :3].astype(np.float64) - ref["pos"]) ** 2).sum(1)
+    off = wl.sys_offsets
+    per_sys = np.sort([float(np.sqrt(d2[off[s]:off[s + 1]].mean())) for s in range(len(off) - 1)])[::-1]
+    assert per_sys[0] > RMSD_TOL and per_sys[1] <= RMSD_TOL, per_sys[:4]
+    p.close()
 
 
 def test_tf32x3_trajectory_config2(pfc, weights):
