@@ -90,15 +90,20 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
       g_pending = false;
     }
     if (e < re) {
-      float dEdr = 0.0f;
-      const float* gs = S.gR + NSHF_R * sp;
+      // two shells at a time in packed fp32 pairs (the exponentials stay scalar SFU calls)
+      const float2* gs = reinterpret_cast<const float2*>(S.gR + NSHF_R * sp);
+      const float2 r2 = make_float2(r, r), m1 = make_float2(-1.0f, -1.0f), fc2 = make_float2(fc, fc),
+                   dfc2 = make_float2(dfc, dfc), ke = make_float2(-(ETA_R * LOG2E), -(ETA_R * LOG2E)),
+                   k2e = make_float2(-2.0f * ETA_R, -2.0f * ETA_R);
+      float2 d2acc = make_float2(0.0f, 0.0f);
 #pragma unroll
-      for (int k = 0; k < NSHF_R; ++k) {
-        const float dr = r - c_tab.shf_r[k];
-        const float ex = ex2_approx(-(ETA_R * LOG2E) * dr * dr);
-        dEdr = fmaf(gs[k] * ex, fmaf(-2.0f * ETA_R * dr, fc, dfc), dEdr);
+      for (int k = 0; k < NSHF_R / 2; ++k) {
+        const float2 dr = pk_fma(make_float2(c_tab.shf_r[2 * k], c_tab.shf_r[2 * k + 1]), m1, r2);
+        const float2 arg = pk_mul(pk_mul(dr, dr), ke);
+        const float2 ex = make_float2(ex2_approx(arg.x), ex2_approx(arg.y));
+        d2acc = pk_fma(pk_mul(gs[k], ex), pk_fma(pk_mul(dr, k2e), fc2, dfc2), d2acc);
       }
-      dEdr *= 0.25f;
+      float dEdr = 0.25f * (d2acc.x + d2acc.y);
       px = dEdr * ux; py = dEdr * uy; pz = dEdr * uz;
     }
     const uint32_t mask = __ballot_sync(0xffffffffu, isang);
