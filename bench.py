@@ -36,8 +36,8 @@ DT_FS = 0.5
 MLP_FLOPS_PER_ATOM = 4.0 * 94304                     # fwd + bwd, 94,304 MAC each, 2 flop per MAC = 377,216
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.5: SMs x FP32 lanes x 2 x max SM clock
 # dram__bytes_read.sum + dram__bytes_write.sum of one K3 launch, from the committed ncu --set full
-# capture (config 4, FFMA path): profiles/r1d_fp32.md (353.2 + 305.6 MB)
-K3_TRAFFIC_BYTES = {(4, 0): 658.8e6, (4, 1): 668.5e6}
+# captures (config 4): FFMA path profiles/r1d_fp32.md (353.2 + 305.6 MB), tensor path r1e_tc.md (360.8 + 301.4 MB)
+K3_TRAFFIC_BYTES = {(4, 0): 658.8e6, (4, 1): 662.2e6}
 K3_TRAFFIC_SOURCE = {(4, 0): "profiles/r1d_fp32.md (ncu --set full, one launch)",
                      (4, 1): "profiles/r1e_tc.md (ncu --set full, one launch)"}
 
