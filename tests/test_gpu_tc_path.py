@@ -158,3 +158,30 @@ def test_tf32x3_bitwise_determinism(pfc, weights):
         p.close()
     for a, b in zip(*outs):
         assert np.array_equal(a, b)
+
+
+def test_compensation_holds_for_another_weight_draw(pfc):
+    """The compensation constants were fitted with the weights of seed 2412.  With
+    a different draw (seed 7) the one-sided error of g stays an order of magnitude below the
+    uncompensated -2.2e-6 and the 100-step trajectories of 64 replicas of config 1 stay within the bar."""
+    w7 = W.make_weights(7)
+    wl = W.config1(n_replicas=64)
+    ref = oracle.energy_forces(wl.pos.astype(np.float64), wl.species, wl.sys_offsets, w7, want_intermediates=True)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, w7, mlp_path=pfc.MLP_TF32X3)
+    pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+    E, F = p.energy_forces(pos)
+    torch.cuda.synchronize()
+    _, g = p.intermediates()
+    dg = g.astype(np.float64) - ref["g"]
+    slope = float(np.sum(dg * ref["g"]) / np.sum(ref["g"] ** 2))
+    assert abs(slope) <= 5e-7, slope
+    assert np.abs(dg).max() <= G_ATOL
+    p.set_state(pos, vel)
+    p.step(100, wl.dt_fs)
+    torch.cuda.synchronize()
+    r = oracle.step(wl.pos, wl.vel, wl.species, wl.sys_offsets, w7, wl.dt_fs, 100)
+    d2 = ((pos.cpu().numpy()[:, :3].astype(np.float64) - r["pos"]) ** 2).sum(1)
+    off = wl.sys_offsets
+    worst = max(float(np.sqrt(d2[off[s]:off[s + 1]].mean())) for s in range(len(off) - 1))
+    assert worst <= RMSD_TOL, worst
+    p.close()
