@@ -123,7 +123,7 @@ def _trajectory(pfc, weights, wl, n_steps, cell=False, mlp_path=None):
     # velocities: north_star states no bound; DESIGN.md "Tolerances" derives one from the position
     # bound: an error that reaches 1e-4 A while growing with e-folding time tau moves at 1e-4/tau;
     # measured tau >= 2.5 fs (config 3, steps 80-100: 3.4 fs) gives 4e-5 A/fs, taken like the
-    # position bound as a root mean square over the atoms of a system (reading S27: this potential
+    # position bound as a root mean square over the atoms of a system (reading S29: this potential
     # has no core repulsion; single atoms in a 0.08 A contact at step 100 of config 2 are
     # ill-conditioned).  Thermal H speed is 1.6e-2 A/fs.
     vrms = _rmsd_per_system(v, ref["vel"], wl.sys_offsets)
