@@ -69,6 +69,11 @@ extern "C" {
 #define PFC_MLP_TF32X1 2                /* tcgen05 plain TF32: tolerance evidence only (fails it) */
 #define PFC_MLP_AUTO 3                  /* TF32X3 for batches of >= 4096 atoms, FP32 below */
 
+/* Environment overrides read by pfc_create -- tuning and evidence experiments only, never needed in
+ * production: PFC_K3_TM (16|32|64|128) and PFC_K3_DEEP (0|1) force the tile height / staging ring
+ * of the FP32 MLP kernel; PFC_TC_COMP_F and PFC_TC_COMP_B scale the forward / backward truncation
+ * compensation of the tensor-core MLP (defaults 0.9 / 0.73; 0 switches it off). */
+
 typedef struct pfc_ctx pfc_t;           /* opaque; owned by the library          */
 
 /* All pointers in the descriptor are HOST pointers except `workspace`;
