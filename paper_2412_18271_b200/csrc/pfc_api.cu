@@ -328,8 +328,10 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
 
   pfc_ctx* c = new (std::nothrow) pfc_ctx();
   if (!c) return PFC_ERR_ARG;
-  // AUTO: the tensor-core MLP pays from a few thousand atoms on (config 1, 5,632 atoms: 0.125 vs 0.140
-  // ms/step; config 2, 1,500 atoms: 0.141 vs 0.114), where its 128-row tiles start to fill the SMs
+  // AUTO: the tensor-core MLP pays from about 4,000 atoms on, where its 128-row tiles start to fill the
+  // SMs.  Measured ms/step, FFMA vs tensor, replicas of config 1: 2,200 atoms 0.108 / 0.111, 3,960
+  // 0.113 / 0.115, 4,840 0.136 / 0.121, 5,632 0.139 / 0.124; of config 4: 3,758 atoms 0.143 / 0.145,
+  // 4,749 0.163 / 0.147; config 2 (1,500 atoms) 0.111 / 0.141
   c->mlp_path = d->mlp_path == PFC_MLP_AUTO ? (d->n_atoms >= 4096 ? PFC_MLP_TF32X3 : PFC_MLP_FP32) : d->mlp_path;
   c->sz = worst_case_sizes(N, NS);                      // capacities are the worst-case ones
   // static element grouping: rows sorted by element, blocks padded to ROW_PAD
