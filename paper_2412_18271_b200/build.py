@@ -37,22 +37,5 @@ def build_libpfc(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_probes(force: bool = False) -> list:
-    """The tuning microbenchmarks under csrc/probes (standalone programs, results in profiles/):
-    compiled next to their sources as *.bin so that they cannot rot; nothing imports them."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    pdir = os.path.join(CSRC, "probes")
-    out = []
-    for f in sorted(os.listdir(pdir)):
-        if not f.endswith(".cu"):
-            continue
-        src, exe = os.path.join(pdir, f), os.path.join(pdir, f[:-3] + ".bin")
-        if force or not os.path.exists(exe) or os.path.getmtime(src) > os.path.getmtime(exe):
-            subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-o", exe, src],
-                           check=True)
-        out.append(exe)
-    return out
-
-
 if __name__ == "__main__":
     print(build_libpfc(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,4 +1,4 @@
-// k3_mlp_fp32.cuh -- K3 (FP32 FFMA path, the default): per-element MLP 384->160->128->96->1
+// k3_mlp_fp32.cuh -- K3 (FP32 FFMA path: batches below the tensor-core threshold, and on request): per-element MLP 384->160->128->96->1
 // with CELU(0.1), forward and input-gradient backward, fused per row tile
 // (O5; backward = PAPER.md:67 "forces by backprop", weight gradients
 // are never needed).
@@ -12,7 +12,7 @@
 // 4*cgi + 64*f (f < N/64) plus, for N = 160 / 96, two more at 64*(N/64) + 2*cgi, cgi = 2*(warp%8) + cg.
 // The lane mapping is chosen for the shared-memory pipe, which is what bounds this kernel (ncu:
 // 84 % of the LSU wavefront peak with the earlier rg = lane/4, cg = lane%4 mapping).  Measured on
-// B200 (csrc/probes, profiles/r1c_probes.md): an LDS.128 costs 2 cycles of the SM's shared-memory
+// B200 (profiles/r1c_probes.md): an LDS.128 costs 2 cycles of the SM's shared-memory
 // pipe when lanes with equal addresses are adjacent (or there are only two addresses, alternating),
 // 4 cycles otherwise; with 16 row groups of two adjacent lanes BOTH operand loads are 2-cycle.
 //   * the 32-row kernel (the one large batches run) issues the FMAs as packed fma.rn.f32x2
