@@ -35,11 +35,37 @@ UNIT = "atom-steps/s"
 DT_FS = 0.5
 MLP_FLOPS_PER_ATOM = 4.0 * 94304                     # fwd + bwd, 94,304 MAC each, 2 flop per MAC = 377,216
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # 74.5: SMs x FP32 lanes x 2 x max SM clock
-# dram__bytes_read.sum + dram__bytes_write.sum of one K3 launch, from the committed ncu --set full
-# captures (config 4): FFMA path profiles/r1d_fp32.md (353.2 + 305.6 MB), tensor path r1e_tc.md (360.8 + 301.4 MB)
-K3_TRAFFIC_BYTES = {(4, 0): 658.8e6, (4, 1): 662.2e6}
-K3_TRAFFIC_SOURCE = {(4, 0): "profiles/r1d_fp32.md (ncu --set full, one launch)",
-                     (4, 1): "profiles/r1e_tc.md (ncu --set full, one launch)"}
+SFU_PEAK_TOPS = 148 * 16 * 1.965e9 / 1e12            # 4.65: SMs x 16 SFU lanes x max SM clock
+KERNEL_SOURCES = {"K1": ["k1_neighbors.cuh"], "K2": ["k2_aev.cuh", "aev_common.cuh"], "K3_tc": ["k3_mlp_tc.cuh", "tc_ptx.cuh"],
+                  "K3_fp32": ["k3_mlp_fp32.cuh"], "K4a": ["k4_forces.cuh", "aev_common.cuh"], "K4b": ["k4_forces.cuh"]}
+
+
+def _source_hash(kernel):
+    """sha256 (first 16 hex digits) of the kernel's source files: profiles/traffic.csv rows carry the hash of
+    the sources they were captured from, so a stale capture is never printed as this binary's traffic."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES[kernel]:
+        path = os.path.join(ROOT, "paper_2412_18271_b200", "csrc", f)
+        if os.path.exists(path):
+            h.update(open(path, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def _traffic(kernel, config):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `config`, from the committed
+    `ncu --set full` capture listed in profiles/traffic.csv -- or None when no row matches the present sources."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None, None
+    want = _source_hash(kernel)
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, cfg, rd, wr, sha, src = [c.strip() for c in line.split(",")][:6]
+        if k == kernel and int(cfg) == config and sha == want:
+            return float(rd) + float(wr), src
+    return None, None
 
 
 def _peaks():
@@ -135,13 +161,67 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / (args.steps + 1) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOAD_NAMES[args.config], "config_index": args.config, "sample": what,
-                   "atoms_in_sample": wl.n_atoms, "dt_fs": DT_FS},
+        "config": _config_dict(args, W.make_config(args.config)),
+        "sample": {"what": what, "atoms_in_sample": wl.n_atoms},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
+
+
+def _config_dict(args, wl):
+    """The `config` object of the JSON line: the workload only, identical in both arms (the pfc arm's
+    kernel path is reported under `path`, the reference arm's bounded sample under `sample`)."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    return {"workload": wl.name, "config_index": args.config, "atoms": wl.n_atoms, "systems": wl.n_systems,
+            "dt_fs": DT_FS, "integrator": args.integrator,
+            "parallelism": "replicas only" if world > 1 else "1 gpu",
+            "l2": "per-step working set (aev + g + lists + edge) exceeds the 126 MB L2"
+                  if wl.n_atoms * 3072 > 126e6 else "working set fits L2: neighbour/AEV/MLP buffers are "
+                  "rewritten every step, no flush"}
+
+
+def per_kernel_roofline(stage_ms, counts, n_atoms, n_systems, mlp_is_tensor, peaks, tensor_peak, step_ms=None):
+    """Every kernel's achieved rate against the roof that bounds it (SURVEY.md 8(d) "Which roof bounds which
+    kernel"), from the stage times measured in THIS run (CUDA events on the launching stream) and the
+    run's own list sizes (pfc_work_counts).  Algorithmic counts, DESIGN.md section 4:
+      K1  distance tests x 8 flop (3 sub, 3 mul, 2 add; plain ALU)         ; 16 B pos read + 4 B per entry written
+      K2  90 flop per radial entry + 150 per triple                         ; 1,536 B aev row written + 4 B per entry
+      K3  377,216 flop per atom                                             ; aev row read + g row written
+      K4a 2 x K2's flops (value + derivative chains)                        ; 1,536 B g row read + 16 B per entry
+      K4b streaming: 16 B per entry gathered + 4 B index + 32 B per atom
+      K5  64 B read + 48 B written per atom
+    HBM fractions are quoted against the measured copy bandwidth (and ~8 TB/s nominal in `hbm_frac_nominal`)."""
+    hbm = peaks["hbm_gbs"]
+    R, T, tests = counts["radial"], counts["triples"], counts["brute_tests"]
+    aev_flops = 90.0 * R + 150.0 * T
+    rows = {
+        "K1_neighbors": ("alu", 8.0 * tests, 32.0 * n_atoms + 4.0 * R + 32.0 * n_atoms),
+        "K2_aev_fwd": ("alu", aev_flops, 1536.0 * n_atoms + 4.0 * R + 32.0 * n_atoms),
+        "K3_mlp": ("tensor" if mlp_is_tensor else "alu", MLP_FLOPS_PER_ATOM * n_atoms, 3072.0 * n_atoms),
+        "K4a_aev_bwd": ("alu", 2.0 * aev_flops, 1536.0 * n_atoms + 20.0 * R + 32.0 * n_atoms),
+        "K4b_gather": ("hbm", 0.0, 20.0 * R + 48.0 * n_atoms),
+        "energy_sum": ("hbm", 0.0, 16.0 * n_atoms + 4.0 * n_systems),
+    }
+    out = {}
+    for (name, (bound, flops, nbytes)), ms in zip(rows.items(), stage_ms):
+        sec = ms * 1e-3
+        e = {"bound": bound, "ms": float(ms), "algorithmic_bytes": nbytes, "gbs": nbytes / sec / 1e9,
+             "hbm_frac": nbytes / sec / 1e9 / hbm, "hbm_frac_nominal": nbytes / sec / 1e9 / 8000.0}
+        if flops:
+            peak = tensor_peak if bound == "tensor" else FP32_PEAK_TFLOPS
+            e.update({"algorithmic_flops": flops, "tflops": flops / sec / 1e12, "peak_tflops": peak,
+                      "frac": flops / sec / 1e12 / peak})
+        else:
+            e["frac"] = e["hbm_frac"]
+        out[name] = e
+    if step_ms is not None:                                      # the integrator kernel: the step minus the force stages
+        ms = max(step_ms - float(np.sum(stage_ms)), 1e-6)
+        nbytes = 112.0 * n_atoms
+        out["K5_integrate"] = {"bound": "hbm", "ms": ms, "by": "step time minus the six force stages",
+                               "algorithmic_bytes": nbytes, "gbs": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / hbm}
+    return out
 
 
 def max_over_ranks(seconds, device=None):
@@ -245,21 +325,34 @@ def run_pfc(args):
         stage_ms /= reps
         k3_s = stage_ms[2] * 1e-3
         flops = MLP_FLOPS_PER_ATOM * N
+        # the burst bf16 peak when the clock record shows the run was never power-capped, else the sustained one
+        capped = bool(clocks and "sw_power_cap" in (clocks.get("reasons") or []))
+        bf16 = peaks["bf16_tflops_sustained"] if capped else peaks["bf16_tflops"]
+        tensor_peak = 0.5 * bf16
         if mlp == pfc.MLP_FP32:
             roof = {"bound": "alu", "achieved": flops / k3_s / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and max SM clock)"}
         else:
-            roof = {"bound": "tensor", "achieved": flops / k3_s / 1e12,
-                    "peak": 0.5 * peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                    "peak_source": f"{peak_src} bf16 sustained x 0.5 (tf32:bf16 nominal ratio); "
-                                   "achieved counts algorithmic flops once, the 3-term split issues 3x"}
-        roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": K3_TRAFFIC_BYTES.get((args.config, mlp)),
-                     "traffic_source": K3_TRAFFIC_SOURCE.get((args.config, mlp)),
+            roof = {"bound": "tensor", "achieved": flops / k3_s / 1e12, "peak": tensor_peak, "unit": "TFLOP/s",
+                    "peak_source": f"{peak_src} bf16 {'sustained (sw_power_cap seen)' if capped else 'burst (no power cap seen)'} "
+                                   "x 0.5 (tf32:bf16 nominal ratio); achieved counts algorithmic flops once, the "
+                                   "3-term split issues 3x"}
+        k3_name = "K3_fp32" if mlp == pfc.MLP_FP32 else "K3_tc"
+        traffic, traffic_src = _traffic(k3_name, args.config)
+        counts = p.work_counts()
+        per_kernel = per_kernel_roofline(stage_ms, counts, N, wl.n_systems, mlp != pfc.MLP_FP32, peaks, tensor_peak,
+                                         step_ms=t / args.steps * 1e3)
+        for kname, src in (("K1", "K1_neighbors"), ("K2", "K2_aev_fwd"), ("K4a", "K4a_aev_bwd"), ("K4b", "K4b_gather")):
+            tr, tr_src = _traffic(kname, args.config)
+            per_kernel[src]["traffic"], per_kernel[src]["traffic_source"] = tr, tr_src
+        roof.update({"frac": roof["achieved"] / roof["peak"], "traffic": traffic, "traffic_source": traffic_src,
                      "algorithmic_bytes": 2 * 1536 * N,   # aev row read + g row written per atom
                      "kernel": "K3 MLP fwd+bwd",
                      "kernel_ms": float(stage_ms[2]),
+                     "work_counts": counts,
                      "stage_ms": {n: float(v) for n, v in zip(pfc.STAGE_NAMES, stage_ms)},
-                     "stage_share": {n: float(v / stage_ms.sum()) for n, v in zip(pfc.STAGE_NAMES, stage_ms)}})
+                     "stage_share": {n: float(v / stage_ms.sum()) for n, v in zip(pfc.STAGE_NAMES, stage_ms)},
+                     "per_kernel": per_kernel})
 
         # ---- end to end through the C ABI with HOST buffers: H2D + 1 step + D2H per step ----
         ph, vh = torch.from_numpy(pos0.copy()).pin_memory(), torch.from_numpy(vel0.copy()).pin_memory()
@@ -276,7 +369,7 @@ def run_pfc(args):
                 p2.run_host_resume(ph, vh, Fh, 1, DT_FS, Eh, stream=stream)     # synchronises inside
             t_e2e = time.perf_counter() - t0
         p2.close()
-        e2e = {"value": world * N * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": 3 * N * 16,
+        e2e = {"value": N * e2e_steps / t_e2e, "unit": UNIT, "ranks_measured": 1, "h2d_bytes_per_step": 3 * N * 16,
                "d2h_bytes_per_step": 3 * N * 16 + 4 * wl.n_systems, "steps": e2e_steps,
                "call": "pfc_run_host_resume(n_steps=1) per step: pinned host pos/vel/F in, one MD step "
                        "(one force evaluation), pos/vel/F/E out"}
@@ -303,13 +396,10 @@ def run_pfc(args):
             "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if mlp == 0 else "tf32x3",    # MLP contractions as a 3-term tf32 split, fp32 accumulate; all else f32
             "data": "synthetic",
-            "config": {"workload": wl.name, "config_index": args.config, "atoms": N, "systems": wl.n_systems,
-                       "dt_fs": DT_FS, "integrator": args.integrator, "mlp_path": "fp32_ffma" if mlp == 0 else "tf32x3_tcgen05",
-                       "mlp_path_requested": {0: "fp32", 1: "tf32x3", 2: "tf32x1", 3: "auto"}[args.mlp],
-                       "parallelism": "replicas only" if world > 1 else "1 gpu",
-                       "l2": "per-step working set (aev + g + lists + edge) exceeds the 126 MB L2"
-                             if N * 3072 > 126e6 else "working set fits L2: neighbour/AEV/MLP buffers are "
-                             "rewritten every step, no flush"},
+            "config": _config_dict(args, wl),
+            "path": {"mlp_path": "fp32_ffma" if mlp == 0 else "tf32x3_tcgen05",
+                     "mlp_path_requested": {0: "fp32", 1: "tf32x3", 2: "tf32x1", 3: "auto"}[args.mlp],
+                     "steps_per_graph": p.steps_per_graph()},
             "ns_per_day_per_replica": steps_per_s * DT_FS * 1e-6 * 86400,
             "ns_per_day_aggregate": steps_per_s * DT_FS * 1e-6 * 86400 * wl.n_systems * world,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_step * args.steps,

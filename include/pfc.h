@@ -33,7 +33,9 @@
  *    (neighbour capacity overflow, angular row longer than PFC_MAX_ANGULAR,
  *    non-finite energy) set sticky bits readable with pfc_status(); outputs
  *    are then unspecified.
- *  - One handle = one stream = one caller at a time.
+ *  - One handle = one stream = one caller at a time; several handles (with their own
+ *    masses, weights and systems) may be live at once.
+ *  - Measurement and debug entry points are declared in pfc_debug.h.
  */
 #ifndef PFC_H_
 #define PFC_H_
@@ -51,11 +53,11 @@ extern "C" {
 #define PFC_ERR_WORKSPACE (-3)  /* workspace missing, misaligned or too small    */
 #define PFC_ERR_CUDA (-4)       /* a CUDA runtime call failed                    */
 #define PFC_ERR_CAPTURE (-5)    /* graph capture / instantiate failed            */
-#define PFC_ERR_STATE (-6)      /* pfc_step before pfc_set_state                 */
+#define PFC_ERR_STATE (-6)      /* no bound state, or another CUDA device current */
 
 /* sticky device status bits (pfc_status) */
-#define PFC_STATUS_RADIAL_OVERFLOW 1u   /* total radial entries > capacity       */
-#define PFC_STATUS_ANGULAR_OVERFLOW 2u  /* total angular entries > capacity      */
+#define PFC_STATUS_RADIAL_OVERFLOW 1u   /* an atom has more radial neighbours than its row holds (min(192, N_sys-1)) */
+#define PFC_STATUS_ANGULAR_OVERFLOW 2u  /* reserved (never set: angular neighbours are flagged radial entries) */
 #define PFC_STATUS_ANGULAR_ROW 4u       /* one atom has > PFC_MAX_ANGULAR angular neighbours */
 #define PFC_STATUS_NONFINITE 8u         /* a system energy is NaN/Inf            */
 #define PFC_STATUS_CELL_OVERFLOW 16u    /* cell grid exceeded its capacity       */
@@ -69,10 +71,20 @@ extern "C" {
 #define PFC_MLP_TF32X1 2                /* tcgen05 plain TF32: tolerance evidence only (fails it) */
 #define PFC_MLP_AUTO 3                  /* TF32X3 for batches of >= 4096 atoms, FP32 below */
 
-/* Environment overrides read by pfc_create -- tuning and evidence experiments only, never needed in
- * production: PFC_K3_TM (16|32|64|128) and PFC_K3_DEEP (0|1) force the tile height / staging ring
- * of the FP32 MLP kernel; PFC_TC_COMP_F and PFC_TC_COMP_B scale the forward / backward truncation
- * compensation of the tensor-core MLP (defaults 0.9 / 0.73; 0 switches it off). */
+/* Optional tuning knobs, passed explicitly through pfc_desc_t.tuning (HOST pointer, NULL = all
+ * defaults; a zero-filled struct is also "all defaults").  The library reads no environment
+ * variables.  None of them is needed in production; the tests use them to reach every kernel variant. */
+typedef struct {
+  int32_t k3_tile_rows;       /* FP32 MLP tile height: 0 = chosen by pfc_create from the batch; 16, 32, 64 or 128 */
+  int32_t k3_deep_ring;       /* FP32 MLP weight staging: 0 = chosen by pfc_create; 1 = two buffers;
+                                 2 = eight-stage ring (tiles of <= 32 rows only, ignored otherwise) */
+  int32_t tc_comp_override;   /* 0 = default truncation compensation of the tensor-core MLP (DESIGN.md
+                                 section 5); 1 = scale it by the two factors below (0 switches it off) */
+  float tc_comp_forward;      /* used when tc_comp_override = 1 */
+  float tc_comp_backward;
+  int32_t steps_per_graph;    /* MD steps captured per CUDA graph by pfc_step: 0 = default (16); >= 1 */
+  int32_t reserved[2];        /* must be 0 */
+} pfc_tuning_t;
 
 typedef struct pfc_ctx pfc_t;           /* opaque; owned by the library          */
 
@@ -91,13 +103,16 @@ typedef struct {
   void *workspace;               /* DEVICE, 256-byte aligned, >= pfc_workspace_bytes() */
   size_t workspace_bytes;
   int32_t mlp_path;              /* PFC_MLP_AUTO (recommended), PFC_MLP_FP32, PFC_MLP_TF32X3 (or PFC_MLP_TF32X1) */
+  const pfc_tuning_t *tuning;    /* HOST or NULL (defaults)                         */
 } pfc_desc_t;
 
 /* Bytes of device workspace pfc_create needs for these sizes (0 on bad args). */
 size_t pfc_workspace_bytes(int32_t n_atoms, int32_t n_systems);
 
-/* Validates the descriptor, builds the static element grouping, uploads the
- * weights (synchronous copies on the legacy stream) and returns a handle. */
+/* Validates the descriptor, builds the static element grouping and the neighbour-row layout,
+ * uploads the weights (synchronous copies on the legacy stream) and returns a handle bound to the
+ * CUDA device that is current at this call; every later call on the handle must be made with the
+ * same device current (PFC_ERR_STATE otherwise). */
 int pfc_create(const pfc_desc_t *desc, pfc_t **out);
 
 /* Energy and forces at the given positions (explicit-force
@@ -105,7 +120,9 @@ int pfc_create(const pfc_desc_t *desc, pfc_t **out);
  * E: DEVICE [n_systems] floats, potential energy per system.  F: DEVICE
  * [n_atoms] float4 = {-dE/dx, -dE/dy, -dE/dz, e_i}.  stream: a cudaStream_t
  * (NULL = legacy default stream).  Enqueues: neighbour build (K1), AEV (K2),
- * MLP forward/backward (K3), force chain rule + gather (K4), energy sum. */
+ * MLP forward/backward (K3), force chain rule + gather (K4), energy sum -- as ONE replay of a
+ * CUDA graph captured the first time this (pos, E, F) triple of buffers is seen (the paper's
+ * CUDA-Graph finding; the four most recent triples stay cached). */
 int pfc_energy_forces(pfc_t *ctx, const float *pos, float *E, float *F, void *stream);
 
 /* The provider call in the paper's own units: the callback of
@@ -117,14 +134,6 @@ int pfc_energy_forces(pfc_t *ctx, const float *pos, float *E, float *F, void *st
  * 1 eV = 96.485332 kJ/mol) are enqueued on `stream`; nothing is synchronised.  Uses internal
  * staging buffers: PFC_ERR_STATE if a pfc_run_host state is currently bound to them. */
 int pfc_energy_forces_nm(pfc_t *ctx, const float *pos_nm, float *E_kj, float *F_kj_nm, void *stream);
-
-/* Measurement helper: the same kernel sequence as pfc_energy_forces with a CUDA
- * event recorded on `stream` at every stage boundary; synchronises and returns
- * the device time of each stage in milliseconds, ms HOST [PFC_N_STAGES]:
- * 0 = K1 neighbour build, 1 = K2 AEV forward, 2 = K3 MLP forward+backward,
- * 3 = K4a AEV backward, 4 = K4b force gather, 5 = per-system energy sum. */
-#define PFC_N_STAGES 6
-int pfc_profile_stages(pfc_t *ctx, const float *pos, float *E, float *F, void *stream, float *ms);
 
 /* Binds (does not copy) the MD state advanced by pfc_step: pos, vel DEVICE
  * [n_atoms] float4, updated in place; E DEVICE [n_systems]; F DEVICE [n_atoms]
@@ -177,29 +186,18 @@ int pfc_run_host_resume(pfc_t *ctx, float *pos_host, float *vel_host, float *F_h
 
 /* Parity getters: DEVICE pointers into the workspace, valid until the next
  * call that enqueues work.  Lists are int32 CSR, rows ascending by neighbour
- * index (O2/S7). */
+ * index (O2/S7): the "deterministically ordered pair list" of north_star (1).
+ * pfc_get_neighbors enqueues, on the handle's stream, the export of the last evaluation's
+ * fixed-capacity rows (the step path's own format) into that CSR; synchronise before reading. */
 int pfc_get_neighbors(pfc_t *ctx, const int32_t **r_off, const int32_t **r_idx,
                       const int32_t **a_off, const int32_t **a_idx);
-/* Entries r_idx / a_idx can hold; when r_off[n_atoms] (a_off[n_atoms]) exceeds it the overflow
- * status bit is set and the rows past the capacity are not written. */
-int pfc_get_capacities(pfc_t *ctx, int32_t *cap_r, int32_t *cap_a);
 /* aev, g: [n_rows][384] in element-sorted padded row order; row_of_atom
  * DEVICE [n_atoms] gives each atom's row. */
 int pfc_get_intermediates(pfc_t *ctx, const float **aev, const float **g,
                           const int32_t **row_of_atom, int32_t *n_rows);
 
-/* Parity helper: synchronous cudaMemcpy of `bytes` from a DEVICE pointer returned
- * by the getters above into HOST memory. */
-int pfc_copy_to_host(const void *device_src, void *host_dst, size_t bytes);
-
 /* Synchronises the bound/last-used stream and returns the sticky status bits. */
 int pfc_status(pfc_t *ctx, uint32_t *bits);
-
-/* The MLP path in use (PFC_MLP_AUTO resolved by pfc_create). */
-int pfc_mlp_path(pfc_t *ctx, int32_t *path);
-
-/* Number of kernel launches one energy_forces pass / one MD step enqueues. */
-int pfc_launch_counts(pfc_t *ctx, int32_t *per_energy_forces, int32_t *per_step);
 
 int pfc_destroy(pfc_t *ctx);
 const char *pfc_error_string(int code);

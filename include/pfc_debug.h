@@ -1,0 +1,40 @@
+/* pfc_debug.h -- measurement and debug entry points of libpfc, kept out of the provider
+ * boundary pfc.h ("keep them few").  bench.py and the tests use them; an MD
+ * engine driving the potential never needs them. */
+#ifndef PFC_DEBUG_H_
+#define PFC_DEBUG_H_
+
+#include "pfc.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Measurement (per-kernel roofline): the same kernel sequence as
+ * pfc_energy_forces, launched kernel by kernel with a CUDA event recorded on `stream` at every
+ * stage boundary; synchronises and returns the device time of each stage in milliseconds,
+ * ms HOST [PFC_N_STAGES]: 0 = K1 neighbour build, 1 = K2 AEV forward, 2 = K3 MLP
+ * forward+backward, 3 = K4a AEV backward, 4 = K4b force gather, 5 = per-system energy sum. */
+#define PFC_N_STAGES 6
+int pfc_profile_stages(pfc_t *ctx, const float *pos, float *E, float *F, void *stream, float *ms);
+
+/* Work counts of the last evaluation, for the roofline arithmetic: counts HOST [4] =
+ * {radial row entries, angular row entries, triples (sum over atoms of m(m-1)/2, m = angular
+ * neighbours), brute-force distance tests per evaluation}.  Synchronises the handle's stream. */
+int pfc_work_counts(pfc_t *ctx, int64_t *counts);
+
+/* Parity helper: synchronous cudaMemcpy of `bytes` from a DEVICE pointer returned by the
+ * getters of pfc.h into HOST memory. */
+int pfc_copy_to_host(const void *device_src, void *host_dst, size_t bytes);
+
+/* The MLP path in use (PFC_MLP_AUTO resolved by pfc_create). */
+int pfc_mlp_path(pfc_t *ctx, int32_t *path);
+
+/* Kernel launches one energy/forces evaluation and one steady-state MD step consist of, and the
+ * number of MD steps pfc_step captures per CUDA graph. */
+int pfc_launch_counts(pfc_t *ctx, int32_t *per_energy_forces, int32_t *per_step, int32_t *steps_per_graph);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PFC_DEBUG_H_ */

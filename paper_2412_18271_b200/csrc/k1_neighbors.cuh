@@ -1,18 +1,23 @@
 // k1_neighbors.cuh -- K1: gas-phase neighbour builder (O2, S6, S7, S22).
 //
-// Output: int32 CSR, rows by atom index, neighbours ascending:
-//   r_off[N+1], r_idx[]  all j != i of the same system with d2 <  RC2_R
-//   a_off[N+1], a_idx[]  the subset with                     d2 <  RC2_A
+// Internal format (what K2 / K4 read): one row of fixed capacity per atom,
+//   nbr[row_beg[i] + k], k < cnt[i].x   entry words, ascending neighbour index j:
+//                                       j | species(j) << 29 | (d2 < RC2_A) << 31
+//   cnt[i] = {radial entries, of which angular}
+// with row capacity min(192, N_sys - 1) (row_beg is static, built by pfc_create), so the whole
+// build is ONE pass and ONE launch for brute-force systems: no count pass, no scan, and every
+// distance is tested once.  The canonical int32 CSR of reading S7 (r_off / r_idx / a_off / a_idx,
+// what the parity tests compare bit for bit) is produced from the rows on request by the export
+// kernels at the end of this file (pfc_get_neighbors), not on the step path.
 // The predicate is the fp32, individually rounded expression dist2_rn().
-// Two passes (count -> exclusive scan -> fill) give exact-size pooled rows
-// inside a static CUDA graph; ordered compaction is ballot + popc, no sort.
 //
-//  * brute force: one warp per atom scans its own system 32 atoms at a time
-//    (systems <= BRUTE_MAX atoms)
+//  * brute force (systems <= BRUTE_MAX atoms): one CTA per work item = (system, block of its
+//    atoms); the system's positions are staged in shared memory once, one warp per atom scans
+//    them 32 at a time; ordered compaction is ballot + popc, no sort.
 //  * cell list (systems > BRUTE_MAX atoms): per-step bounding box, cells of
-//    edge >= 5.2*(1+2^-10), atoms binned in ascending index order per cell,
-//    27-cell stencil walked in ascending cell order, rows ordered by index with
-//    a rank-by-count pass.  The same predicate decides membership.
+//    edge >= 5.2*(1+2^-10), atoms binned per cell, 27-cell stencil walked by one warp per atom
+//    into a shared-memory row, ordered by index with a rank-by-count pass.  The same predicate
+//    decides membership.
 #pragma once
 #include "pfc_common.cuh"
 
@@ -22,65 +27,60 @@ constexpr int K1_WARPS = 8;
 constexpr int SCAN_THREADS = 256, SCAN_ITEMS = 8, SCAN_BLOCK = SCAN_THREADS * SCAN_ITEMS;  // 2048
 
 // ---- brute force -----------------------------------------------------------
-// FILL=false: counts -> cnt[i] = {radial, angular}; also writes the packed copy
-//             xs[i] = {x, y, z, bitcast(species)} every later kernel reads, and xsl[i], the low
-//             words of the positions (S15): the list predicate sees only the fp32 positions,
-//             the AEV geometry sees the two-float difference.
-// FILL=true : writes r_idx / a_idx rows at r_off[i] / a_off[i].
-template <bool FILL>
+// item = {first atom of the system, one past its last atom, first atom of my block, one past}
+// Also writes the packed copies every later kernel reads: xs[i] = {x, y, z, bitcast(species)} and
+// xsl[i], the low words of the two-float positions (S15): the list predicate sees only the fp32
+// positions, the AEV geometry sees the two-float difference.
 __global__ void __launch_bounds__(K1_WARPS * 32)
-k1_brute_kernel(int n_atoms, const float4* __restrict__ pos, const int* __restrict__ species,
-                const int* __restrict__ sys_id, const int* __restrict__ sys_off,
-                const unsigned char* __restrict__ sys_is_cell,
+k1_brute_kernel(const int4* __restrict__ items, const float4* __restrict__ pos, const int* __restrict__ species,
                 const float4* __restrict__ xlo, float4* __restrict__ xs, float4* __restrict__ xsl,
-                int2* __restrict__ cnt,
-                const int* __restrict__ r_off, const int* __restrict__ a_off,
-                int* __restrict__ r_idx, int* __restrict__ a_idx, int cap_r, int cap_a) {
-  int i = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
-  if (i >= n_atoms) return;
-  const uint32_t lane = lane_id();
-  float4 pi = pos[i];
-  int sid = sys_id[i];
-  if (!FILL && lane == 0) {
-    float4 o = pi;
-    o.w = __int_as_float(species[i]);
-    xs[i] = o;
-    // low words of the two-float positions (pfc_step state); zero for a plain pfc_energy_forces call
-    xsl[i] = xlo ? xlo[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+                const int* __restrict__ row_beg, uint32_t* __restrict__ nbr, int2* __restrict__ cnt,
+                uint32_t* __restrict__ status) {
+  extern __shared__ float4 k1_sp[];              // the system's positions, species bits in .w
+  const int4 it = items[blockIdx.x];
+  const int nsys = it.y - it.x;
+  for (int t = threadIdx.x; t < nsys; t += K1_WARPS * 32) {
+    float4 p = pos[it.x + t];
+    p.w = __int_as_float(species[it.x + t]);
+    k1_sp[t] = p;
   }
-  if (sys_is_cell[sid]) return;          // handled by the cell-list kernels
-  int b = sys_off[sid], e = sys_off[sid + 1];
-  int nr = 0, na = 0;
-  int ro = 0, ao = 0;
-  bool fit_r = true, fit_a = true;
-  if (FILL) {
-    ro = r_off[i]; ao = a_off[i];
-    // capacity overflow was flagged by the scan; never write out of bounds
-    fit_r = r_off[i + 1] <= cap_r; fit_a = a_off[i + 1] <= cap_a;
-    if (!fit_r && !fit_a) return;
-  }
-  for (int j0 = b; j0 < e; j0 += 32) {
-    int j = j0 + (int)lane;
-    bool valid = (j < e) && (j != i);
-    float d2 = 1e30f;
-    if (valid) {
-      float4 pj = pos[j];
-      d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+  __syncthreads();
+  const uint32_t lane = lane_id(), lt = lanemask_lt();
+  for (int i = it.z + (int)(threadIdx.x >> 5); i < it.w; i += K1_WARPS) {
+    const float4 pi = k1_sp[i - it.x];
+    if (lane == 0) {
+      xs[i] = pi;
+      // low words of the two-float positions (pfc_step state); zero for a plain pfc_energy_forces call
+      xsl[i] = xlo ? xlo[i] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
-    uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
-    uint32_t ma = __ballot_sync(0xffffffffu, d2 < RC2_A);
-    if (FILL) {
-      uint32_t lt = lanemask_lt();
-      if (fit_r && d2 < RC2_R) r_idx[ro + nr + __popc(mr & lt)] = j;
-      if (fit_a && d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
+    const int beg = row_beg[i], cap = row_beg[i + 1] - beg;
+    int nr = 0, na = 0;
+    for (int j0 = 0; j0 < nsys; j0 += 32) {
+      const int jl = j0 + (int)lane;
+      float d2 = 1e30f;
+      int sp = 0;
+      if (jl < nsys && it.x + jl != i) {
+        const float4 pj = k1_sp[jl];
+        d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+        sp = __float_as_int(pj.w);
+      }
+      const uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
+      if (mr == 0u) continue;                    // warp-uniform
+      const int slot = nr + __popc(mr & lt);
+      const bool stored = d2 < RC2_R && slot < cap;     // capacity overflow is flagged below; never write out of the row
+      const bool ang = d2 < RC2_A;
+      if (stored) nbr[beg + slot] = (uint32_t)(it.x + jl) | ((uint32_t)sp << 29) | (ang ? 0x80000000u : 0u);
+      na += __popc(__ballot_sync(0xffffffffu, stored && ang));
+      nr += __popc(mr);
     }
-    nr += __popc(mr);
-    na += __popc(ma);
+    if (lane == 0) {
+      if (nr > cap) atomicOr(status, ST_RADIAL_OVERFLOW);
+      cnt[i] = make_int2(min(nr, cap), na);
+    }
   }
-  if (!FILL && lane == 0) cnt[i] = make_int2(nr, na);
 }
 
-// ---- exclusive scan of cnt -> r_off, a_off (reduce-then-scan, two tiny kernels)
+// ---- exclusive scan of cnt -> r_off, a_off (reduce-then-scan, two tiny kernels; CSR export only)
 __global__ void __launch_bounds__(SCAN_THREADS)
 k1_scan_totals_kernel(int n, const int2* __restrict__ cnt, int2* __restrict__ block_tot) {
   __shared__ int2 wsum[SCAN_THREADS / 32];
@@ -106,8 +106,7 @@ k1_scan_totals_kernel(int n, const int2* __restrict__ cnt, int2* __restrict__ bl
 
 __global__ void __launch_bounds__(SCAN_THREADS)
 k1_scan_kernel(int n, const int2* __restrict__ cnt, const int2* __restrict__ block_tot,
-               int* __restrict__ r_off, int* __restrict__ a_off, int cap_r, int cap_a,
-               uint32_t* __restrict__ status) {
+               int* __restrict__ r_off, int* __restrict__ a_off) {
   __shared__ int2 wsum[SCAN_THREADS / 32];
   __shared__ int2 sbase;
   const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
@@ -155,11 +154,7 @@ k1_scan_kernel(int n, const int2* __restrict__ cnt, const int2* __restrict__ blo
   for (int q = 0; q < SCAN_ITEMS; ++q) {
     if (i0 + q < n) { r_off[i0 + q] = er; a_off[i0 + q] = ea; }
     er += c[q].x; ea += c[q].y;
-    if (i0 + q == n - 1) {
-      r_off[n] = er; a_off[n] = ea;
-      uint32_t bits = (er > cap_r ? ST_RADIAL_OVERFLOW : 0u) | (ea > cap_a ? ST_ANGULAR_OVERFLOW : 0u);
-      if (bits) atomicOr(status, bits);
-    }
+    if (i0 + q == n - 1) { r_off[n] = er; a_off[n] = ea; }
   }
 }
 
@@ -295,45 +290,50 @@ k1_cell_scan_kernel(const int* __restrict__ cell_sys, const int* __restrict__ ce
 
 // scatter atoms into their cells (slot order inside a cell is arbitrary: rows are
 // ordered by index afterwards, so the final lists do not depend on it)
-// cell_xyz[slot] = {x, y, z, bitcast(atom index)}: the rows kernels stream a cell line's positions
-// contiguously instead of gathering pos[cell_atoms[p]] (two dependent loads per round)
+// cell_xyz[slot] = {x, y, z, bitcast(atom index | species << 29)}: the rows kernel streams a cell
+// line's positions contiguously instead of gathering pos[cell_atoms[p]] (two dependent loads per round)
 __global__ void k1_cell_fill_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
                                     const int* __restrict__ atom_cell, const float4* __restrict__ pos,
+                                    const int* __restrict__ species,
                                     int* __restrict__ cell_cursor, float4* __restrict__ cell_xyz) {
   int q = blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= n_cell_atoms) return;
   int slot = atomicAdd(&cell_cursor[atom_cell[q]], 1);
   const int i = cell_atom_list[q];
   const float4 p = pos[i];
-  cell_xyz[slot] = make_float4(p.x, p.y, p.z, __int_as_float(i));
+  cell_xyz[slot] = make_float4(p.x, p.y, p.z, __int_as_float(i | (species[i] << 29)));
 }
 
-// neighbour rows through the cell list: one warp per atom.
-// FILL=false counts; FILL=true writes the row unsorted, then orders it by
-// rank-by-count (all indices are distinct) and derives the angular row.
+// neighbour rows through the cell list: one warp per atom, one pass.  The row is collected
+// unordered in shared memory, then ordered by index with a rank-by-count pass (all indices are
+// distinct) straight into the atom's fixed-capacity row.
 constexpr int CELL_ROW_MAX = 512;        // longest radial row the in-warp ordering supports
-template <bool FILL>
 __global__ void __launch_bounds__(K1_WARPS * 32)
 k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
                     const int* __restrict__ atom_cell_sys, const int* __restrict__ atom_cell,
-                    const float4* __restrict__ pos, const CellGrid* __restrict__ grids,
+                    const float4* __restrict__ pos, const int* __restrict__ species,
+                    const float4* __restrict__ xlo, const CellGrid* __restrict__ grids,
                     const int* __restrict__ cell_start, const float4* __restrict__ cell_xyz,
-                    int2* __restrict__ cnt, const int* __restrict__ r_off, const int* __restrict__ a_off,
-                    int* __restrict__ r_idx, int* __restrict__ a_idx, int cap_r, int cap_a,
+                    float4* __restrict__ xs, float4* __restrict__ xsl,
+                    const int* __restrict__ row_beg, uint32_t* __restrict__ nbr, int2* __restrict__ cnt,
                     uint32_t* __restrict__ status) {
-  __shared__ int srow[K1_WARPS][CELL_ROW_MAX];
+  __shared__ uint32_t srow[K1_WARPS][CELL_ROW_MAX];
   int q = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
   if (q >= n_cell_atoms) return;
   const uint32_t lane = lane_id(), lt = lanemask_lt();
-  int* row = srow[threadIdx.x >> 5];
+  uint32_t* row = srow[threadIdx.x >> 5];
   int i = cell_atom_list[q];
   const CellGrid g = grids[atom_cell_sys[q]];
   float4 pi = pos[i];
+  if (lane == 0) {
+    float4 o = pi;
+    o.w = __int_as_float(species[i]);
+    xs[i] = o;
+    xsl[i] = xlo ? xlo[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
   int c = atom_cell[q] - g.cell_base;
   int cx = c % g.nc[0], cy = (c / g.nc[0]) % g.nc[1], cz = c / (g.nc[0] * g.nc[1]);
-  int nr = 0, na = 0;
-  if (FILL && r_off[i + 1] > cap_r) return;
-  const bool fit_a = !FILL || a_off[i + 1] <= cap_a;
+  int nr = 0;
   for (int z = max(cz - 1, 0); z <= min(cz + 1, g.nc[2] - 1); ++z)
     for (int y = max(cy - 1, 0); y <= min(cy + 1, g.nc[1] - 1); ++y) {
       // cells x-1..x+1 of one (y,z) line are contiguous in the pooled array
@@ -342,49 +342,58 @@ k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
       int s0 = cell_start[c0], s1 = cell_start[c1 + 1];
       for (int p0 = s0; p0 < s1; p0 += 32) {
         int p = p0 + (int)lane;
-        int j = i;
+        uint32_t w = 0;
         float d2 = 1e30f;
         if (p < s1) {
           const float4 pj = cell_xyz[p];
-          j = __float_as_int(pj.w);
-          if (j != i) d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+          w = (uint32_t)__float_as_int(pj.w);
+          if (nbr_index(w) != i) d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
         }
         uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
-        if (FILL) {
-          int slot = nr + __popc(mr & lt);
-          if (d2 < RC2_R && slot < CELL_ROW_MAX) row[slot] = j;
-        } else {
-          na += __popc(__ballot_sync(0xffffffffu, d2 < RC2_A));
-        }
+        int slot = nr + __popc(mr & lt);
+        if (d2 < RC2_R && slot < CELL_ROW_MAX) row[slot] = w | (d2 < RC2_A ? 0x80000000u : 0u);
         nr += __popc(mr);
       }
     }
-  if (!FILL) {
-    if (lane == 0) cnt[i] = make_int2(nr, na);
-    return;
-  }
-  if (nr > CELL_ROW_MAX) { if (lane == 0) atomicOr(status, ST_RADIAL_OVERFLOW); return; }
+  const int beg = row_beg[i], cap = row_beg[i + 1] - beg;
+  if (nr > cap && lane == 0) atomicOr(status, ST_RADIAL_OVERFLOW);
+  const int n = min(nr, CELL_ROW_MAX);
   __syncwarp();
-  // order by index: rank = number of smaller entries (entries are distinct)
-  int ro = r_off[i], ao = a_off[i];
-  for (int s = lane; s < nr; s += 32) {
-    int v = row[s], rank = 0;
-    for (int t = 0; t < nr; ++t) rank += (row[t] < v);
-    r_idx[ro + rank] = v;
-  }
-  __syncwarp();
-  // angular row: ordered compaction of the ordered radial row
-  for (int s0 = 0; s0 < nr; s0 += 32) {
-    int s = s0 + (int)lane;
-    float d2 = 1e30f;
-    int j = 0;
-    if (s < nr) {
-      j = r_idx[ro + s];
-      float4 pj = pos[j];
-      d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+  // order by index: rank = number of smaller entries (entries are distinct); keep the first cap
+  int na = 0;
+  for (int s = lane; s < n; s += 32) {
+    const uint32_t v = row[s];
+    const int key = nbr_index(v);
+    int rank = 0;
+    for (int t = 0; t < n; ++t) rank += (nbr_index(row[t]) < key);
+    if (rank < cap) {
+      nbr[beg + rank] = v;
+      na += (int)(v >> 31);
     }
-    uint32_t ma = __ballot_sync(0xffffffffu, d2 < RC2_A);
-    if (fit_a && d2 < RC2_A) a_idx[ao + na + __popc(ma & lt)] = j;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xffffffffu, na, o);
+  if (lane == 0) cnt[i] = make_int2(min(n, cap), na);
+}
+
+// ---- CSR export (pfc_get_neighbors; not on the step path) ----------------------------------
+// r_off / a_off come from k1_scan_* over cnt; this copies the rows into the canonical int32 CSR of
+// reading S7: r_idx = every entry's index, a_idx = the flagged subset, both ascending.
+__global__ void __launch_bounds__(K1_WARPS * 32)
+k1_export_csr_kernel(int n_atoms, const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr,
+                     const int2* __restrict__ cnt, const int* __restrict__ r_off, const int* __restrict__ a_off,
+                     int* __restrict__ r_idx, int* __restrict__ a_idx) {
+  const int i = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
+  if (i >= n_atoms) return;
+  const uint32_t lane = lane_id(), lt = lanemask_lt();
+  const int rb = row_beg[i], n = cnt[i].x, ro = r_off[i], ao = a_off[i];
+  int na = 0;
+  for (int k0 = 0; k0 < n; k0 += 32) {
+    const int k = k0 + (int)lane;
+    const uint32_t w = k < n ? nbr[rb + k] : 0u;
+    if (k < n) r_idx[ro + k] = nbr_index(w);
+    const uint32_t ma = __ballot_sync(0xffffffffu, k < n && nbr_angular(w));
+    if (k < n && nbr_angular(w)) a_idx[ao + na + __popc(ma & lt)] = nbr_index(w);
     na += __popc(ma);
   }
 }

@@ -1,77 +1,62 @@
 // k2_aev.cuh -- K2: ANI-style atomic environment vector, forward (O3, O4).
 //
-// One warp per centre atom.  The radial row is walked 32 entries at a time
-// (lane <-> entry): distance, cosine cutoff (SFU cos); the chunk is staged in
-// shared memory GROUPED BY SPECIES (four ballots), and the angular subset
-// (d2 < RC2_A, the K1 predicate) is compacted in row order into a per-warp
-// table of unit vectors plus one index list per species.
-//   radial  : lane <-> (entry parity, shell k); one loop per species segment, so
-//             each of the four accumulators is a plain sum  (SFU ex2)
-//   angular : triples are enumerated BLOCK BY BLOCK of the species-pair index p
-//             (HH HC HN HO CC CN CO NN NO OO): block (s1,s2) holds the pairs of
-//             list s1 x list s2 (s1 < s2) or the unordered pairs of list s1.
-//             phase 1, lane <-> triple: 8 angular factors A_b and 4 radial factors
-//             W_a = 2 B_a fc_j fc_k into shared memory;
-//             phase 2, lane <-> (a,b): out[p][a][b] += A_b W_a over the staged
-//             triples of one block at a time -- the block of a staged triple is
-//             known from the prefix table, so the inner loop is two loads and an
-//             FMA, and an accumulator is flushed once per block and chunk (the
-//             per-triple block test of the earlier lexicographic order cost 43 % of
-//             the kernel's instructions).
-//             No atomics: every accumulator has one owner lane and a fixed
-//             summation order, so results are bit-reproducible.
+// One warp per centre atom.  The neighbour row (K1's entry words: index, species, angular flag)
+// is walked 32 entries at a time (lane <-> entry): distance and unit vector (one MUFU.RSQ +
+// Newton), cosine cutoff (SFU cos); the chunk is staged in shared memory GROUPED BY SPECIES (four
+// ballots), and the angular subset is compacted in row order into a per-warp table of unit
+// vectors plus one slot list per species.
+//   radial  : lane <-> (entry parity, shell k); one loop per species segment, so each of the four
+//             accumulators is a plain sum  (SFU ex2)
+//   angular : the triples are enumerated BLOCK BY BLOCK of the species-pair index p
+//             (HH HC HN HO CC CN CO NN NO OO): block (s1,s2) holds the pairs of list s1 x list s2
+//             (s1 < s2) or the unordered pairs of list s1 in round-robin (circulant) order -- an
+//             order that decodes without a square root or a search loop.  Every block is padded to a
+//             multiple of four slots (padding slots contribute exact zeros).
+//             phase 1, lane <-> slot: the 8 angular factors A_b and the 4 radial factors
+//             W_a = 2 B_a fc_j fc_k of the triple, written TRANSPOSED into shared memory
+//             (tA[b][slot], tW[a][slot]: conflict-free stores);
+//             phase 2, lane <-> output (a, b): one register accumulator per block p; a block's slots
+//             are read four at a time (one LDS.128 per operand, four FMAs): 1.5 instructions per
+//             triple where the earlier slot-major layout cost 3 and a shared-memory flush per block
+//             and chunk.  The ten accumulators go straight to global memory.
+//             No atomics: every accumulator has one owner lane and a fixed summation order, so
+//             results are bit-reproducible.
 // theta is never formed: cos(theta - theta_b) = c cos(theta_b) + sqrt(1-c^2) sin(theta_b)
 // with c = 0.95 cos(phi); the power 32 is five squarings.
-// Rows are written in element-sorted padded order (row_of_atom) so K3's tiles
-// are contiguous.
+// Rows are written in element-sorted padded order (row_of_atom) so K3's tiles are contiguous.
 #pragma once
-#include "pfc_common.cuh"
+#include "aev_common.cuh"
 
 namespace pfc {
 
-constexpr int AEV_WARPS = 4;
+constexpr int K2_TCH = 96;                       // padded triple slots per chunk (3 passes of 32 lanes)
+constexpr int K2_TLD = K2_TCH + 4;               // row stride of the transposed factor tables: 4 mod 32 banks
 
 struct AevFwdSmem {
-  float4 ur[MAX_ANG];        // unit vector i->j, r         (row order)
-  float fc[MAX_ANG];         // fc(r; RC_A)
+  float4 ur[MAX_ANG];            // unit vector i->j, r         (row order)
+  float fc[MAX_ANG];             // fc(r; RC_A)
   uint8_t lst[NSPEC][MAX_ANG];   // table slots of each species, ascending
-  float out[AEV_LEN];
-  float tA[32][NSHF_Z];
-  float tW[32][NSHF_A];
-  float2 rad[32];            // (r, fc(r; RC_R)) of one radial chunk, grouped by species
-  int pre[NPAIR + 1];        // first triple of each species-pair block
+  float tA[NSHF_Z][K2_TLD];      // A_b of the staged slots, transposed
+  float tW[NSHF_A][K2_TLD];      // W_a of the staged slots, transposed
+  float2 rad[32];                // (r, fc(r; RC_R)) of one radial chunk, grouped by species
+  int pre4[NPAIR + 1];           // first 4-slot group of each species-pair block
 };
 
-// species pair of block p (nibble tables):  s1 = 0000111223, s2 = 0123123233
-__device__ __forceinline__ int block_s1(int p) { return (int)((0x3221110000ull >> (4 * p)) & 3ull); }
-__device__ __forceinline__ int block_s2(int p) { return (int)((0x3323213210ull >> (4 * p)) & 3ull); }
-
-// triple index t in [0, m(m-1)/2) -> (j,k), j<k, lexicographic
-__device__ __forceinline__ int tri_row_start(int j, int m) { return (j * (2 * m - j - 1)) >> 1; }
-__device__ __forceinline__ void tri_decode(int t, int m, int& j, int& k) {
-  float b = (float)(2 * m - 1);
-  int jj = (int)((b - sqrtf(b * b - 8.0f * (float)t)) * 0.5f);
-  jj = max(0, min(jj, m - 2));
-  while (jj < m - 2 && tri_row_start(jj + 1, m) <= t) ++jj;
-  while (jj > 0 && tri_row_start(jj, m) > t) --jj;
-  j = jj;
-  k = jj + 1 + (t - tri_row_start(jj, m));
-}
-
-__global__ void __launch_bounds__(AEV_WARPS * 32)
+__global__ void __launch_bounds__(AEV_WARPS * 32, 8)
 k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __restrict__ xsl,
-                  const int* __restrict__ r_off,
-                  const int* __restrict__ r_idx, int cap_r, const int* __restrict__ row_of_atom,
+                  const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr, const int2* __restrict__ cnt,
+                  const int* __restrict__ row_of_atom,
                   float* __restrict__ aev, uint32_t* __restrict__ status) {
-  __shared__ AevFwdSmem sm[AEV_WARPS];
+  __shared__ __align__(16) AevFwdSmem sm[AEV_WARPS];
   const int warp = threadIdx.x >> 5;
   const int i = blockIdx.x * AEV_WARPS + warp;
   if (i >= n_atoms) return;                       // warp-uniform; only __syncwarp below
   AevFwdSmem& S = sm[warp];
   const uint32_t lane = lane_id(), lt = lanemask_lt();
   const float4 xi = xs[i], li = xsl[i];
-  const int rb = r_off[i];
-  const int re = r_off[i + 1] <= cap_r ? r_off[i + 1] : rb;   // capacity overflow (flagged by K1): row unwritten
+  const int rb = row_beg[i];
+  const int re = rb + cnt[i].x;
+  float* dst = aev + (size_t)row_of_atom[i] * AEV_LEN;
   int m = 0;
   uint32_t na = 0;                                // angular neighbours per species, one byte each
   float acc[NSPEC] = {0.f, 0.f, 0.f, 0.f};
@@ -79,48 +64,37 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __re
   const float shf = c_tab.shf_r[lane & 15];
   for (int c0 = rb; c0 < re; c0 += 32) {
     const int e = c0 + (int)lane;
-    float r = 1.0f, fcr = 0.0f, dx = 0.f, dy = 0.f, dz = 0.f;
-    int sp = -1;
-    bool isang = false;
+    NbrGeom g;
+    g.sp = -1; g.ang = false; g.r = 1.0f; g.ux = g.uy = g.uz = 0.0f;
+    float fcr = 0.0f;
     if (e < re) {
-      const int j = r_idx[e];
-      const float4 xj = xs[j];
-      dx = __fsub_rn(xj.x, xi.x); dy = __fsub_rn(xj.y, xi.y); dz = __fsub_rn(xj.z, xi.z);
-      // identical value to K1's predicate (squares do not see the sign)
-      const float d2 = __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
-      // geometry from the two-float positions (zero low words outside pfc_step)
-      const float4 lj = xsl[j];
-      dx += lj.x - li.x; dy += lj.y - li.y; dz += lj.z - li.z;
-      r = sqrtf(fmaf(dx, dx, fmaf(dy, dy, dz * dz)));
-      fcr = 0.5f * __cosf((PI_F / RC_R) * r) + 0.5f;
-      sp = __float_as_int(xj.w);
-      isang = d2 < RC2_A;
+      g = nbr_geometry(nbr[e], xi, li, xs, xsl);
+      fcr = 0.5f * __cosf((PI_F / RC_R) * g.r) + 0.5f;
     }
     // stage (r, fc) grouped by species; angular entries go to the table (row order) and to
-    // the index list of their species
+    // the slot list of their species
     int seg[NSPEC + 1];
     seg[0] = 0;
     int pos = 0, lpos = 0;
-    const uint32_t amask = __ballot_sync(0xffffffffu, isang);
+    const uint32_t amask = __ballot_sync(0xffffffffu, g.ang);
 #pragma unroll
     for (int z = 0; z < NSPEC; ++z) {
-      const uint32_t mz = __ballot_sync(0xffffffffu, sp == z);
+      const uint32_t mz = __ballot_sync(0xffffffffu, g.sp == z);
       const uint32_t az = mz & amask;
-      if (sp == z) {
+      if (g.sp == z) {
         pos = seg[z] + __popc(mz & lt);
         lpos = (int)((na >> (8 * z)) & 255u) + __popc(az & lt);
       }
       seg[z + 1] = seg[z] + __popc(mz);
       na += (uint32_t)__popc(az) << (8 * z);      // (a count above 96 is flagged below; bytes cannot carry: m <= 128)
     }
-    if (sp >= 0) S.rad[pos] = make_float2(r, fcr);
-    if (isang) {
+    if (g.sp >= 0) S.rad[pos] = make_float2(g.r, fcr);
+    if (g.ang) {
       const int slot = m + __popc(amask & lt);
       if (slot < MAX_ANG) {
-        const float rinv = 1.0f / r;
-        S.ur[slot] = make_float4(dx * rinv, dy * rinv, dz * rinv, r);
-        S.fc[slot] = 0.5f * __cosf((PI_F / RC_A) * r) + 0.5f;
-        S.lst[sp][lpos] = (uint8_t)slot;          // lpos <= slot < MAX_ANG
+        S.ur[slot] = make_float4(g.ux, g.uy, g.uz, g.r);
+        S.fc[slot] = 0.5f * __cosf((PI_F / RC_A) * g.r) + 0.5f;
+        S.lst[g.sp][lpos] = (uint8_t)slot;        // lpos <= slot < MAX_ANG
       }
     }
     m += __popc(amask);
@@ -130,88 +104,124 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __re
       for (int n = seg[z] + half; n < seg[z + 1]; n += 2) {
         const float2 v = S.rad[n];
         const float dr = v.x - shf;
-        acc[z] = fmaf(0.25f * ex2_approx(-(ETA_R * LOG2E) * dr * dr), v.y, acc[z]);
+        acc[z] = fmaf(ex2_approx(-(ETA_R * LOG2E) * dr * dr), v.y, acc[z]);
       }
     }
     __syncwarp();
   }
+  // radial part of the row: lanes 0-15 hold shell k of species 0 / 2, lanes 16-31 of species 1 / 3
 #pragma unroll
-  for (int z = 0; z < NSPEC; ++z) {
-    acc[z] += __shfl_xor_sync(0xffffffffu, acc[z], 16);
-    if (lane < 16) S.out[NSHF_R * z + lane] = acc[z];
-  }
-  for (int c = RAD_LEN + (int)lane; c < AEV_LEN; c += 32) S.out[c] = 0.0f;
+  for (int z = 0; z < NSPEC; ++z) acc[z] += __shfl_xor_sync(0xffffffffu, acc[z], 16);
+  dst[lane] = 0.25f * (half ? acc[1] : acc[0]);
+  dst[32 + lane] = 0.25f * (half ? acc[3] : acc[2]);
   if (m > MAX_ANG) {                              // outputs unspecified (S25); keep every index in range
     if (lane == 0) atomicOr(status, ST_ANGULAR_ROW);
     m = 0; na = 0;
   }
   // ---- angular ----
-  // block sizes -> prefix table (every lane computes the same ten numbers)
+  // block sizes -> prefix table in units of four slots (every lane computes the same ten numbers)
+  const int nH = (int)(na & 255u), nC = (int)((na >> 8) & 255u), nN = (int)((na >> 16) & 255u), nO = (int)(na >> 24);
+  int pre4[NPAIR + 1];
   {
-    int run = 0;
-    if (lane == 0) S.pre[0] = 0;
+    const int sz[NPAIR] = {(nH * (nH - 1)) >> 1, nH * nC, nH * nN, nH * nO, (nC * (nC - 1)) >> 1,
+                           nC * nN, nC * nO, (nN * (nN - 1)) >> 1, nN * nO, (nO * (nO - 1)) >> 1};
+    pre4[0] = 0;
 #pragma unroll
-    for (int p = 0; p < NPAIR; ++p) {
-      const int n1 = (int)((na >> (8 * block_s1(p))) & 255u), n2 = (int)((na >> (8 * block_s2(p))) & 255u);
-      run += block_s1(p) == block_s2(p) ? (n1 * (n1 - 1)) >> 1 : n1 * n2;
-      if (lane == 0) S.pre[p + 1] = run;
-    }
+    for (int p = 0; p < NPAIR; ++p) pre4[p + 1] = pre4[p] + ((sz[p] + 3) >> 2);
+  }
+  if (lane == 0) {
+#pragma unroll
+    for (int p = 0; p <= NPAIR; ++p) S.pre4[p] = pre4[p];
   }
   __syncwarp();
-  const int T = (m * (m - 1)) >> 1;               // == S.pre[NPAIR]
-  const int pa = lane >> 3, pb = lane & 7;
-  int bcur = 0;                                   // block of the first staged triple (warp-uniform)
-  for (int t0 = 0; t0 < T; t0 += 32) {
-    const int t = t0 + (int)lane;
-    if (t < T) {
-      int p = bcur;
-      while (t >= S.pre[p + 1]) ++p;
-      const int q = t - S.pre[p];
-      const int s1 = block_s1(p), s2 = block_s2(p);
-      int jj, kk;
-      if (s1 == s2) {
-        tri_decode(q, (int)((na >> (8 * s1)) & 255u), jj, kk);
-      } else {
-        const int n2 = (int)((na >> (8 * s2)) & 255u);
-        jj = (int)(((float)q + 0.5f) / (float)n2);      // exact: q < 2^13
-        kk = q - jj * n2;
-      }
-      const int j = S.lst[s1][jj], k = S.lst[s2][kk];
-      const float4 uj = S.ur[j], uk = S.ur[k];
-      const float c = COS_SCALE * (uj.x * uk.x + uj.y * uk.y + uj.z * uk.z);
-      const float s = sqrtf(fmaf(-c, c, 1.0f));
-      const float rbar = 0.5f * (uj.w + uk.w);
-      const float w2 = 2.0f * S.fc[j] * S.fc[k];
-      const float2 cc2 = make_float2(c, c), ss2 = make_float2(s, s), half2 = make_float2(0.5f, 0.5f);
+  const int n_slots = 4 * pre4[NPAIR];
+  const int pa = lane >> 3, pb = lane & 7;        // phase 2: my output (a, b)
+  float out[NPAIR];
 #pragma unroll
-      for (int b = 0; b < NSHF_Z / 2; ++b) {                        // two shifts at a time (packed fp32 pairs)
-        const float2 cz = make_float2(c_tab.cos_z[2 * b], c_tab.cos_z[2 * b + 1]);
-        const float2 sz = make_float2(c_tab.sin_z[2 * b], c_tab.sin_z[2 * b + 1]);
-        float2 q1 = pk_fma(half2, pk_fma(cc2, cz, pk_mul(ss2, sz)), half2);
-        q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1);   // ^32
-        *reinterpret_cast<float2*>(&S.tA[lane][2 * b]) = q1;
-      }
+  for (int p = 0; p < NPAIR; ++p) out[p] = 0.0f;
+  for (int s0 = 0; s0 < n_slots; s0 += K2_TCH) {
 #pragma unroll
-      for (int a = 0; a < NSHF_A; ++a) {
-        const float dr = rbar - c_tab.shf_a[a];
-        S.tW[lane][a] = w2 * ex2_approx(-(ETA_A * LOG2E) * dr * dr);
+    for (int pass = 0; pass < K2_TCH / 32; ++pass) {
+      const int s = s0 + 32 * pass + (int)lane;
+      if (s0 + 32 * pass >= n_slots) break;       // warp-uniform
+      float2 A2[NSHF_Z / 2];
+      float2 W2[NSHF_A / 2];
+#pragma unroll
+      for (int b = 0; b < NSHF_Z / 2; ++b) A2[b] = make_float2(0.f, 0.f);
+      W2[0] = W2[1] = make_float2(0.f, 0.f);
+      if (s < n_slots) {
+        // block of my slot: branch-free count over the ten (warp-uniform) block starts
+        int p = 0;
+#pragma unroll
+        for (int k = 1; k < NPAIR; ++k) p += ((s >> 2) >= pre4[k]) ? 1 : 0;
+        const int q = s - 4 * S.pre4[p];
+        const int s1 = (int)((0xE9500u >> (2 * p)) & 3u), s2 = (int)((0xFB9E4u >> (2 * p)) & 3u);   // 0000111223 / 0123123233
+        const int n1 = (int)((na >> (8 * s1)) & 255u), n2 = (int)((na >> (8 * s2)) & 255u);
+        int jj, kk;
+        bool valid;
+        if (s1 == s2) {
+          // unordered pairs of n1 items in round-robin order: q = (d - 1) n1 + a  ->  {a, (a + d) mod n1}
+          const int d1 = small_div(q, n1);
+          jj = q - d1 * n1;
+          kk = jj + d1 + 1;
+          kk = kk >= n1 ? kk - n1 : kk;
+          valid = q < ((n1 * (n1 - 1)) >> 1);
+        } else {
+          jj = small_div(q, n2);
+          kk = q - jj * n2;
+          valid = q < n1 * n2;
+        }
+        if (valid) {
+          const int j = S.lst[s1][jj], k = S.lst[s2][kk];
+          const float4 uj = S.ur[j], uk = S.ur[k];
+          const float c = COS_SCALE * (uj.x * uk.x + uj.y * uk.y + uj.z * uk.z);
+          const float sn = sqrt_newton(fmaf(-c, c, 1.0f));
+          const float rbar = 0.5f * (uj.w + uk.w);
+          const float w2 = 2.0f * S.fc[j] * S.fc[k];
+          const float2 cc2 = make_float2(c, c), ss2 = make_float2(sn, sn), half2 = make_float2(0.5f, 0.5f);
+#pragma unroll
+          for (int b = 0; b < NSHF_Z / 2; ++b) {                      // two shifts at a time (packed fp32 pairs)
+            const float2 cz = make_float2(0.5f * c_tab.cos_z[2 * b], 0.5f * c_tab.cos_z[2 * b + 1]);
+            const float2 sz = make_float2(0.5f * c_tab.sin_z[2 * b], 0.5f * c_tab.sin_z[2 * b + 1]);
+            float2 q1 = pk_fma(cc2, cz, pk_fma(ss2, sz, half2));      // (1 + cos(theta - theta_b)) / 2
+            q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1); q1 = pk_mul(q1, q1);   // ^32
+            A2[b] = q1;
+          }
+          const float2 rb2 = make_float2(rbar, rbar), m1 = make_float2(-1.0f, -1.0f), ww2 = make_float2(w2, w2),
+                       ke = make_float2(-(ETA_A * LOG2E), -(ETA_A * LOG2E));
+#pragma unroll
+          for (int a = 0; a < NSHF_A / 2; ++a) {
+            const float2 dr = pk_fma(make_float2(c_tab.shf_a[2 * a], c_tab.shf_a[2 * a + 1]), m1, rb2);
+            const float2 arg = pk_mul(pk_mul(dr, dr), ke);
+            W2[a] = pk_mul(ww2, make_float2(ex2_approx(arg.x), ex2_approx(arg.y)));
+          }
+        }
       }
+      const int col = 32 * pass + (int)lane;
+#pragma unroll
+      for (int b = 0; b < NSHF_Z / 2; ++b) { S.tA[2 * b][col] = A2[b].x; S.tA[2 * b + 1][col] = A2[b].y; }
+      S.tW[0][col] = W2[0].x; S.tW[1][col] = W2[0].y; S.tW[2][col] = W2[1].x; S.tW[3][col] = W2[1].y;
     }
     __syncwarp();
-    const int nt = min(32, T - t0);
-    int n = 0;
-    while (n < nt) {                               // one pass per block present in this chunk
-      while (t0 + n >= S.pre[bcur + 1]) ++bcur;
-      const int hi = min(nt, S.pre[bcur + 1] - t0);
-      float a2 = 0.0f;
-#pragma unroll 4
-      for (; n < hi; ++n) a2 = fmaf(S.tA[n][pb], S.tW[n][pa], a2);
-      S.out[RAD_LEN + 32 * bcur + lane] += a2;
+    // phase 2: the groups of four slots of every block that fall into this chunk
+    const int g0 = s0 >> 2, g1 = min(n_slots, s0 + K2_TCH) >> 2;
+#pragma unroll
+    for (int p = 0; p < NPAIR; ++p) {
+      const int lo = max(pre4[p], g0), hi = min(pre4[p + 1], g1);
+      float a0 = out[p], a1 = 0.0f;
+#pragma unroll 1
+      for (int g = lo; g < hi; ++g) {
+        const float4 A = *reinterpret_cast<const float4*>(&S.tA[pb][4 * (g - g0)]);
+        const float4 W = *reinterpret_cast<const float4*>(&S.tW[pa][4 * (g - g0)]);
+        a0 = fmaf(A.x, W.x, a0); a1 = fmaf(A.y, W.y, a1);
+        a0 = fmaf(A.z, W.z, a0); a1 = fmaf(A.w, W.w, a1);
+      }
+      out[p] = a0 + a1;
     }
     __syncwarp();
   }
-  float* dst = aev + (size_t)row_of_atom[i] * AEV_LEN;
-  for (int c = lane; c < AEV_LEN; c += 32) dst[c] = S.out[c];
+#pragma unroll
+  for (int p = 0; p < NPAIR; ++p) dst[RAD_LEN + 32 * p + (int)lane] = out[p];
 }
 
 }  // namespace pfc

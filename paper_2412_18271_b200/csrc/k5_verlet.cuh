@@ -21,7 +21,7 @@ k5_verlet_kernel(int n_atoms, const StepParams* __restrict__ sp, const int* __re
   const int i = blockIdx.x * K5_THREADS + threadIdx.x;
   if (i >= n_atoms) return;
   const float dt = sp->dt;
-  const float kick = (MODE == 2 ? dt : sp->half_dt) * c_tab.inv_mass_acc[species[i]];
+  const float kick = (MODE == 2 ? dt : sp->half_dt) * sp->inv_mass_acc[species[i]];
   const float4 f = frc[i];
   float4 v = vel[i];
   v.x = fmaf(kick, f.x, v.x); v.y = fmaf(kick, f.y, v.y); v.z = fmaf(kick, f.z, v.z);
@@ -65,7 +65,7 @@ __device__ __forceinline__ float u24(uint32_t w) { return fmaf((float)(w >> 8), 
 __global__ void k5_set_langevin_kernel(StepParams* sp, float c1, float c2, float kT, uint32_t seed_lo,
                                        uint32_t seed_hi) {
   sp->c1 = c1;
-  for (int s = 0; s < NSPEC; ++s) sp->sigma[s] = c2 * sqrtf(kT * c_tab.inv_mass_acc[s]);   // kT in eV
+  for (int s = 0; s < NSPEC; ++s) sp->sigma[s] = c2 * sqrtf(kT * sp->inv_mass_acc[s]);   // kT in eV
   sp->seed_lo = seed_lo; sp->seed_hi = seed_hi;
 }
 __global__ void k5_reset_counter_kernel(StepParams* sp) { sp->step = 0; sp->ticket = 0; }
@@ -83,7 +83,7 @@ k5_langevin_kernel(int n_atoms, StepParams* __restrict__ sp, const int* __restri
   if (i < n_atoms) {
     const int z = species[i];
     const float dt = sp->dt, hdt = sp->half_dt;
-    const float kick = (MODE == 2 ? dt : hdt) * c_tab.inv_mass_acc[z];
+    const float kick = (MODE == 2 ? dt : hdt) * sp->inv_mass_acc[z];
     const float4 f = frc[i];
     float4 v = vel[i];
     v.x = fmaf(kick, f.x, v.x); v.y = fmaf(kick, f.y, v.y); v.z = fmaf(kick, f.z, v.z);      // B

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "../../include/pfc.h"
+#include "../../include/pfc_debug.h"
 #include "k0_units.cuh"
 #include "k1_neighbors.cuh"
 #include "k2_aev.cuh"
@@ -46,30 +47,34 @@ struct Carver {                 // bump allocator over the caller's workspace (o
 
 struct Sizes {
   int n_atoms, n_systems, n_rows;
-  int cap_r, cap_a;
+  int cap_r;                                  // neighbour-row entries (sum of the row capacities, worst case)
+  int n_items;                                // K1 brute-force work items (worst case)
   int n_scan_blocks;
   int n_cell_sys, n_cell_atoms, cell_slots;   // cell_slots: pooled cell arrays (incl. +1 per system)
 };
 
 struct Buffers {
-  int *species, *sys_id, *sys_off, *row_of_atom;
-  unsigned char* sys_is_cell;
+  int *species, *sys_off, *row_of_atom;
   float4 *xs, *xsl;
+  int4* items;                  // K1 brute-force work items
+  int* row_beg;                 // [N+1] first entry of every atom's fixed-capacity neighbour row
+  uint32_t* nbr;                // [cap_r] entry words (k1_neighbors.cuh)
   int2 *cnt, *block_tot;
-  int *r_off, *a_off, *r_idx, *a_idx;
+  int *r_off, *a_off, *r_idx, *a_idx;   // CSR export (pfc_get_neighbors only)
   float *aev, *g, *e_row;
   float4 *edge, *self, *xlo;
   uint32_t* status;
   StepParams* sp;
+  unsigned long long* work;     // pfc_work_counts
   float* weights;
   uint8_t* wtc;                 // tensor-core path: packed hi|lo swizzled weight chunks
   float* bias_tc;
   // cell list
   int *cell_sys, *cell_cap_base, *cell_slot_base, *cell_atom_list, *atom_cell_sys, *atom_cell;
   int *cell_count, *cell_start, *cell_cursor;
-  float4* cell_xyz;             // positions in cell order, atom index in .w
+  float4* cell_xyz;             // positions in cell order, atom index | species << 29 in .w
   CellGrid* grids;
-  // internal state for pfc_run_host
+  // internal state for pfc_run_host / pfc_energy_forces_nm
   float4 *h_pos, *h_vel, *h_frc;
   float* h_E;
 };
@@ -79,18 +84,19 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   Buffers t;
   const size_t N = (size_t)s.n_atoms;
   t.species = c.take<int>(N);
-  t.sys_id = c.take<int>(N);
   t.sys_off = c.take<int>((size_t)s.n_systems + 1);
   t.row_of_atom = c.take<int>(N);
-  t.sys_is_cell = c.take<unsigned char>((size_t)s.n_systems);
   t.xs = c.take<float4>(N);
   t.xsl = c.take<float4>(N);
+  t.items = c.take<int4>((size_t)s.n_items);
+  t.row_beg = c.take<int>(N + 1);
+  t.nbr = c.take<uint32_t>((size_t)s.cap_r);
   t.cnt = c.take<int2>(N);
   t.block_tot = c.take<int2>((size_t)s.n_scan_blocks);
   t.r_off = c.take<int>(N + 1);
   t.a_off = c.take<int>(N + 1);
   t.r_idx = c.take<int>((size_t)s.cap_r);
-  t.a_idx = c.take<int>((size_t)s.cap_a);
+  t.a_idx = c.take<int>((size_t)s.cap_r);
   t.aev = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.g = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.e_row = c.take<float>((size_t)s.n_rows);
@@ -99,6 +105,7 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.xlo = c.take<float4>(N);
   t.status = c.take<uint32_t>(64);
   t.sp = c.take<StepParams>(1);
+  t.work = c.take<unsigned long long>(8);
   t.weights = c.take<float>((size_t)NSPEC * DEV_W_PER_ELEM);
   t.wtc = c.take<uint8_t>((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
   t.bias_tc = c.take<float>((size_t)NSPEC * TC_BIAS_LEN);
@@ -122,17 +129,18 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
 }
 
 inline int cells_for(int n_sys_atoms) { return n_sys_atoms + 64 + 1; }
+constexpr int ROW_CAP = 192;                  // neighbour-row capacity of an atom: min(ROW_CAP, N_sys - 1); bulk at 0.1 / A^3 has 59
+constexpr int K1_MIN_BLOCK = 8, K1_MAX_BLOCK = 64;   // atoms per K1 brute-force work item
 
 // worst case over all species / system layouts with these totals
 Sizes worst_case_sizes(int n_atoms, int n_systems) {
   Sizes s{};
   s.n_atoms = n_atoms; s.n_systems = n_systems;
   s.n_rows = (n_atoms + ROW_PAD - 1) / ROW_PAD * ROW_PAD + NSPEC * ROW_PAD;
-  long long per_r = n_atoms - 1 < 128 ? n_atoms - 1 : 128;
-  long long per_a = n_atoms - 1 < 48 ? n_atoms - 1 : 48;
-  long long cr = (long long)n_atoms * (per_r > 1 ? per_r : 1), ca = (long long)n_atoms * (per_a > 1 ? per_a : 1);
+  long long per_r = n_atoms - 1 < ROW_CAP ? n_atoms - 1 : ROW_CAP;      // one system holding every atom
+  long long cr = (long long)n_atoms * (per_r > 1 ? per_r : 1);
   s.cap_r = (int)(cr > 2000000000LL ? 2000000000LL : cr);
-  s.cap_a = (int)(ca > 2000000000LL ? 2000000000LL : ca);
+  s.n_items = n_atoms / K1_MIN_BLOCK + n_systems + 1;
   s.n_scan_blocks = (n_atoms + SCAN_BLOCK - 1) / SCAN_BLOCK;
   s.n_cell_sys = n_atoms / (BRUTE_MAX + 1) + 1;
   if (s.n_cell_sys > n_systems) s.n_cell_sys = n_systems;
@@ -143,30 +151,48 @@ Sizes worst_case_sizes(int n_atoms, int n_systems) {
 
 }  // namespace
 
+constexpr int EF_CACHE = 4;                    // pfc_energy_forces graphs kept (most recently used buffer triples)
+
+struct EfGraph {                               // one captured force evaluation: K1 .. energy sum
+  const float4* pos = nullptr;
+  float* E = nullptr;
+  float4* F = nullptr;
+  bool with_xlo = false;                       // captured with the bound state's low position words
+  cudaGraphExec_t exec = nullptr;
+  unsigned long long last_use = 0;
+};
+
 struct pfc_ctx {
   Sizes sz;
   Buffers b;
   MlpParams mlp;
   TcParams tcp;
+  int device = 0;               // the CUDA device the handle was created on
   int mlp_path;
   int mlp_tm = 128;             // FFMA K3 tile height
   bool mlp_deep = false;        // FFMA K3 staging: 8-stage mbarrier ring (few tiles per SM) or two buffers
   int n_sms = 148;
   int n_cell_sys, n_cell_atoms;
+  int n_items = 0;              // K1 brute-force work items
+  size_t k1_smem = 0;           // bytes: positions of the largest brute-force system
+  long long brute_tests = 0;    // distance tests per evaluation (work counts)
   int launches_ef, launches_step;
+  int steps_per_graph = 16;
   // bound MD state
   float4 *pos = nullptr, *vel = nullptr, *frc = nullptr;
   float* E = nullptr;
   cudaStream_t stream = nullptr, cap_stream = nullptr;
   bool bound = false, forces_stale = true;
   float cur_dt = -1.0f;
-  cudaGraphExec_t g_forces = nullptr, g_step = nullptr, g_lstep = nullptr;   // forces; Verlet step; Langevin step
+  // graphs of the bound state: forces; one Verlet / Langevin step; steps_per_graph of them
+  cudaGraphExec_t g_forces = nullptr, g_step = nullptr, g_lstep = nullptr, g_stepk = nullptr, g_lstepk = nullptr;
+  EfGraph ef[EF_CACHE];         // pfc_energy_forces: graphs keyed on the caller's buffers
+  unsigned long long ef_clock = 0;
   float4* frames = nullptr;     // caller's frame buffer (pfc_set_frames)
   int frame_stride = 0, frame_cap = 0, frames_written = 0;
   long long steps_total = 0;    // steps since pfc_set_state (frame cadence)
   float lg_gamma = -1.f, lg_T = -1.f, lg_dt = -1.f;
   unsigned long long lg_seed = 0;
-  int launches_lstep = 0;
   int launch_counter = 0;
 };
 
@@ -180,9 +206,14 @@ namespace {
 
 inline int cdiv(int a, int b) { return (a + b - 1) / b; }
 
+inline bool on_device(const pfc_ctx* c) {      // every call must run with the handle's device current
+  int dev = -1;
+  return cudaGetDevice(&dev) == cudaSuccess && dev == c->device;
+}
+
 // K1..K4 + energy sum on `st`
 // `ev` (optional): PFC_N_STAGES+1 events recorded at the stage boundaries K1|K2|K3|K4a|K4b|E-sum
-void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStream_t st,
+void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool with_xlo, cudaStream_t st,
                     cudaEvent_t* ev = nullptr) {
   auto mark = [&](int k) { if (ev) cudaEventRecord(ev[k], st); };
   mark(0);
@@ -190,9 +221,10 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
   const Buffers& b = c->b;
   const int N = s.n_atoms;
   // the low position words belong to the bound MD state only
-  const float4* xlo = (c->bound && pos == c->pos) ? b.xlo : nullptr;
-  LAUNCH(c, k1_brute_kernel<false>, cdiv(N, K1_WARPS), K1_WARPS * 32, 0, st, N, pos, b.species, b.sys_id,
-         b.sys_off, b.sys_is_cell, xlo, b.xs, b.xsl, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
+  const float4* xlo = with_xlo ? b.xlo : nullptr;
+  if (c->n_items > 0)
+    LAUNCH(c, k1_brute_kernel, c->n_items, K1_WARPS * 32, c->k1_smem, st, b.items, pos, b.species, xlo, b.xs, b.xsl,
+           b.row_beg, b.nbr, b.cnt, b.status);
   if (c->n_cell_sys > 0) {
     const int nca = c->n_cell_atoms;
     LAUNCH(c, k1_cell_grid_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.sys_off, b.cell_cap_base,
@@ -202,25 +234,13 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
     LAUNCH(c, k1_cell_scan_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.cell_slot_base, b.grids,
            b.cell_count, b.cell_start, b.cell_cursor);
     LAUNCH(c, k1_cell_fill_kernel, cdiv(nca, 256), 256, 0, st, nca, b.cell_atom_list, b.atom_cell,
-           pos, b.cell_cursor, b.cell_xyz);
-    LAUNCH(c, k1_cell_rows_kernel<false>, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
-           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_xyz, b.cnt, b.r_off, b.a_off,
-           b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
-  }
-  if (s.n_scan_blocks > 1)
-    LAUNCH(c, k1_scan_totals_kernel, s.n_scan_blocks, SCAN_THREADS, 0, st, N, b.cnt, b.block_tot);
-  LAUNCH(c, k1_scan_kernel, s.n_scan_blocks, SCAN_THREADS, 0, st, N, b.cnt, b.block_tot, b.r_off, b.a_off,
-         s.cap_r, s.cap_a, b.status);
-  LAUNCH(c, k1_brute_kernel<true>, cdiv(N, K1_WARPS), K1_WARPS * 32, 0, st, N, pos, b.species, b.sys_id,
-         b.sys_off, b.sys_is_cell, xlo, b.xs, b.xsl, b.cnt, b.r_off, b.a_off, b.r_idx, b.a_idx, s.cap_r, s.cap_a);
-  if (c->n_cell_sys > 0) {
-    const int nca = c->n_cell_atoms;
-    LAUNCH(c, k1_cell_rows_kernel<true>, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
-           b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_xyz, b.cnt, b.r_off, b.a_off,
-           b.r_idx, b.a_idx, s.cap_r, s.cap_a, b.status);
+           pos, b.species, b.cell_cursor, b.cell_xyz);
+    LAUNCH(c, k1_cell_rows_kernel, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
+           b.atom_cell_sys, b.atom_cell, pos, b.species, xlo, b.grids, b.cell_start, b.cell_xyz, b.xs, b.xsl,
+           b.row_beg, b.nbr, b.cnt, b.status);
   }
   mark(1);
-  LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.r_off, b.r_idx, s.cap_r,
+  LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
          b.row_of_atom, b.aev, b.status);
   mark(2);
   if (c->mlp_path == PFC_MLP_FP32) {
@@ -246,10 +266,10 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, cudaStre
       LAUNCH(c, k3_mlp_tc_kernel<1>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, b.aev, b.g, b.e_row);
   }
   mark(3);
-  LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.r_off, b.r_idx, s.cap_r,
+  LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
          b.row_of_atom, b.g, b.edge, b.self);
   mark(4);
-  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.r_off, b.r_idx, s.cap_r, b.edge, b.self,
+  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.row_beg, b.nbr, b.cnt, b.edge, b.self,
          b.row_of_atom, b.e_row, F);
   mark(5);
   if (c->n_cell_sys > 0) LAUNCH(c, k_energy_sum_kernel<1024>, s.n_systems, 1024, 0, st, b.sys_off, F, E, b.status);
@@ -263,33 +283,35 @@ void enqueue_verlet(pfc_ctx* c, cudaStream_t st) {
          c->b.species, c->frc, c->pos, c->vel, c->b.xlo);
 }
 
-void drop_graphs(pfc_ctx* c) {
-  if (c->g_forces) cudaGraphExecDestroy(c->g_forces);
-  if (c->g_step) cudaGraphExecDestroy(c->g_step);
-  if (c->g_lstep) cudaGraphExecDestroy(c->g_lstep);
-  c->g_forces = c->g_step = c->g_lstep = nullptr;
-}
-
-// capture {optional fused Verlet kernel, forces} for the bound state
 template <int MODE>
 void enqueue_langevin(pfc_ctx* c, cudaStream_t st) {
   LAUNCH(c, k5_langevin_kernel<MODE>, cdiv(c->sz.n_atoms, K5_THREADS), K5_THREADS, 0, st, c->sz.n_atoms, c->b.sp,
          c->b.species, c->frc, c->pos, c->vel, c->b.xlo);
 }
 
-// kind 0: forces only; 1: fused Verlet kernel + forces; 2: fused Langevin kernel + forces
-int capture(pfc_ctx* c, int kind, cudaGraphExec_t* out, int* n_launches) {
-  // capture on a private stream (the caller's may be the legacy stream, which cannot
-  // capture); the instantiated graph is launched on the caller's stream.
+void drop_state_graphs(pfc_ctx* c) {
+  cudaGraphExec_t* gs[] = {&c->g_forces, &c->g_step, &c->g_lstep, &c->g_stepk, &c->g_lstepk};
+  for (cudaGraphExec_t* g : gs) {
+    if (*g) cudaGraphExecDestroy(*g);
+    *g = nullptr;
+  }
+}
+
+// Captures `n_rep` repetitions of {optional fused integrator kernel, forces} on the private capture
+// stream (the caller's may be the legacy stream, which cannot capture); the instantiated graph is
+// launched on the caller's stream.  kind 0: forces only; 1: fused Verlet kernel + forces;
+// 2: fused Langevin kernel + forces.
+int capture(pfc_ctx* c, int kind, int n_rep, const float4* pos, float* E, float4* F, bool with_xlo,
+            cudaGraphExec_t* out) {
   cudaGraph_t graph = nullptr;
   if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess)
     return PFC_ERR_CAPTURE;
   if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) return PFC_ERR_CAPTURE;
-  c->launch_counter = 0;
-  if (kind == 1) enqueue_verlet<2>(c, c->cap_stream);
-  if (kind == 2) enqueue_langevin<2>(c, c->cap_stream);
-  enqueue_forces(c, c->pos, c->E, c->frc, c->cap_stream);
-  *n_launches = c->launch_counter;
+  for (int r = 0; r < n_rep; ++r) {
+    if (kind == 1) enqueue_verlet<2>(c, c->cap_stream);
+    if (kind == 2) enqueue_langevin<2>(c, c->cap_stream);
+    enqueue_forces(c, pos, E, F, with_xlo, c->cap_stream);
+  }
   cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
   if (e != cudaSuccess || !graph) { cudaGetLastError(); return PFC_ERR_CAPTURE; }
   e = cudaGraphInstantiate(out, graph, 0);
@@ -326,8 +348,19 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (!d->workspace || ((uintptr_t)d->workspace % ALIGN) != 0) return PFC_ERR_WORKSPACE;
   if (d->workspace_bytes < pfc_workspace_bytes(N, NS)) return PFC_ERR_WORKSPACE;
 
+  pfc_tuning_t tun{};                                   // zero = every default
+  if (d->tuning) tun = *d->tuning;
+  if (tun.k3_tile_rows != 0 && tun.k3_tile_rows != 16 && tun.k3_tile_rows != 32 && tun.k3_tile_rows != 64 &&
+      tun.k3_tile_rows != 128)
+    return PFC_ERR_ARG;
+  if (tun.k3_deep_ring < 0 || tun.k3_deep_ring > 2 || tun.steps_per_graph < 0 || tun.steps_per_graph > 256 ||
+      tun.reserved[0] != 0 || tun.reserved[1] != 0)
+    return PFC_ERR_ARG;
+
   pfc_ctx* c = new (std::nothrow) pfc_ctx();
   if (!c) return PFC_ERR_ARG;
+  if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
+  if (tun.steps_per_graph > 0) c->steps_per_graph = tun.steps_per_graph;
   // AUTO: the tensor-core MLP pays from about 4,000 atoms on, where its 128-row tiles start to fill the
   // SMs.  Measured ms/step, FFMA vs tensor, replicas of config 1: 2,200 atoms 0.108 / 0.111, 3,960
   // 0.113 / 0.115, 4,840 0.136 / 0.121, 5,632 0.139 / 0.124; of config 4: 3,758 atoms 0.143 / 0.145,
@@ -339,26 +372,45 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   row_start[0] = 0;
   for (int e = 0; e < NSPEC; ++e) row_start[e + 1] = row_start[e] + (count[e] + ROW_PAD - 1) / ROW_PAD * ROW_PAD;
   c->sz.n_rows = row_start[NSPEC];
-  std::vector<int> row_of_atom(N), sys_id(N);
+  std::vector<int> row_of_atom(N), row_beg(N + 1);
   {
     int next[NSPEC];
     for (int e = 0; e < NSPEC; ++e) next[e] = row_start[e];
     for (int i = 0; i < N; ++i) row_of_atom[i] = next[d->species[i]]++;
   }
-  // systems above BRUTE_MAX atoms go through the cell list
-  std::vector<unsigned char> is_cell(NS, 0);
+  // systems above BRUTE_MAX atoms go through the cell list; the others are cut into K1 work items
+  // (system, block of its atoms): enough items to give every SM a few CTAs, 8..64 atoms each
   std::vector<int> cell_sys, cell_cap_base(1, 0), cell_slot_base, cell_atom_list, atom_cell_sys;
+  std::vector<int4> items;
+  long long n_brute = 0;
+  int max_brute_sys = 1;
   for (int s = 0; s < NS; ++s) {
-    const int b0 = d->sys_offsets[s], e0 = d->sys_offsets[s + 1];
-    for (int i = b0; i < e0; ++i) sys_id[i] = s;
-    if (e0 - b0 > BRUTE_MAX) {
-      is_cell[s] = 1;
-      cell_slot_base.push_back((int)cell_atom_list.size());
-      for (int i = b0; i < e0; ++i) { cell_atom_list.push_back(i); atom_cell_sys.push_back((int)cell_sys.size()); }
-      cell_sys.push_back(s);
-      cell_cap_base.push_back(cell_cap_base.back() + cells_for(e0 - b0));
-    }
+    const int n = d->sys_offsets[s + 1] - d->sys_offsets[s];
+    if (n <= BRUTE_MAX) { n_brute += n; if (n > max_brute_sys) max_brute_sys = n; }
   }
+  int k1_block = (int)((n_brute / (4LL * 148) + 7) / 8 * 8);
+  k1_block = k1_block < K1_MIN_BLOCK ? K1_MIN_BLOCK : k1_block > K1_MAX_BLOCK ? K1_MAX_BLOCK : k1_block;
+  {
+    long long beg = 0;
+    for (int s = 0; s < NS; ++s) {
+      const int b0 = d->sys_offsets[s], e0 = d->sys_offsets[s + 1], n = e0 - b0;
+      const int cap = n - 1 < ROW_CAP ? (n - 1 > 1 ? n - 1 : 1) : ROW_CAP;
+      for (int i = b0; i < e0; ++i) { row_beg[i] = (int)beg; beg += cap; }
+      if (n > BRUTE_MAX) {
+        cell_slot_base.push_back((int)cell_atom_list.size());
+        for (int i = b0; i < e0; ++i) { cell_atom_list.push_back(i); atom_cell_sys.push_back((int)cell_sys.size()); }
+        cell_sys.push_back(s);
+        cell_cap_base.push_back(cell_cap_base.back() + cells_for(n));
+      } else {
+        for (int a0 = b0; a0 < e0; a0 += k1_block)
+          items.push_back(make_int4(b0, e0, a0, a0 + k1_block < e0 ? a0 + k1_block : e0));
+        c->brute_tests += (long long)n * (n - 1);
+      }
+    }
+    row_beg[N] = (int)beg;                              // <= cap_r: sum of n*min(128, n-1) over systems
+  }
+  c->n_items = (int)items.size();
+  c->k1_smem = sizeof(float4) * (size_t)max_brute_sys;
   c->n_cell_sys = (int)cell_sys.size();
   c->n_cell_atoms = (int)cell_atom_list.size();
   carve(c->sz, d->workspace, &c->b);
@@ -451,44 +503,32 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   c->tcp.n_tiles = c->sz.n_rows / TC_TM;
   {
     // truncation steps of the main accumulator chain per phase (K/8, x3 where the three split terms
-    // share one accumulator); PFC_TC_COMP_F / _B scale the forward / backward compensation (experiment)
+    // share one accumulator); pfc_tuning_t.tc_comp_* scale the forward / backward compensation
     const int ntr[6] = {48, 60, 16, 36, 48, 60};
-    const float lf = getenv("PFC_TC_COMP_F") ? (float)atof(getenv("PFC_TC_COMP_F")) : 0.9f;
-    const float lb = getenv("PFC_TC_COMP_B") ? (float)atof(getenv("PFC_TC_COMP_B")) : 0.73f;
+    const float lf = tun.tc_comp_override ? tun.tc_comp_forward : 0.9f;
+    const float lb = tun.tc_comp_override ? tun.tc_comp_backward : 0.73f;
     for (int q = 0; q < 6; ++q) c->tcp.comp[q] = (q < 3 ? lf : lb) * (float)ntr[q] * 2.15e-8f;
   }
 
-  ModelTables tab;
+  StepParams sp0{};
   {
-    // S2/S3: the constants are the fp32 roundings of the decimal values
-    const double shf_r[NSHF_R] = {0.9, 1.16875, 1.4375, 1.70625, 1.975, 2.24375, 2.5125, 2.78125,
-                                  3.05, 3.31875, 3.5875, 3.85625, 4.125, 4.39375, 4.6625, 4.93125};
-    const double shf_a[NSHF_A] = {0.9, 1.55, 2.2, 2.85};
-    const double shf_z[NSHF_Z] = {0.19634954, 0.58904862, 0.98174770, 1.37444679,
-                                  1.76714587, 2.15984495, 2.55254403, 2.94524311};
-    for (int k = 0; k < NSHF_R; ++k) tab.shf_r[k] = (float)shf_r[k];
-    for (int a = 0; a < NSHF_A; ++a) tab.shf_a[a] = (float)shf_a[a];
-    for (int z = 0; z < NSHF_Z; ++z) {
-      const double th = (double)(float)shf_z[z];
-      tab.cos_z[z] = (float)cos(th);
-      tab.sin_z[z] = (float)sin(th);
-    }
     const double mass_default[NSPEC] = {1.008, 12.011, 14.007, 15.999};
     for (int e = 0; e < NSPEC; ++e) {
       const double m = d->masses_amu ? (double)d->masses_amu[e] : mass_default[e];
-      tab.inv_mass_acc[e] = (float)(9.648533216e-3 / m);
+      if (!(m > 0.0)) { delete c; return PFC_ERR_ARG; }
+      sp0.inv_mass_acc[e] = (float)(9.648533216e-3 / m);
     }
   }
   bool ok = true;
   auto up = [&](void* dst, const void* src, size_t bytes) {
     if (bytes && cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess) ok = false;
   };
-  if (cudaMemcpyToSymbol(c_tab, &tab, sizeof(tab)) != cudaSuccess) ok = false;
   up(b.species, d->species, sizeof(int) * N);
-  up(b.sys_id, sys_id.data(), sizeof(int) * N);
+  up(b.sp, &sp0, sizeof(sp0));
+  up(b.row_beg, row_beg.data(), sizeof(int) * (N + 1));
+  up(b.items, items.data(), sizeof(int4) * items.size());
   up(b.sys_off, d->sys_offsets, sizeof(int) * (NS + 1));
   up(b.row_of_atom, row_of_atom.data(), sizeof(int) * N);
-  up(b.sys_is_cell, is_cell.data(), NS);
   up(b.weights, w.data(), sizeof(float) * w.size());
   up(b.wtc, wtc.data(), wtc.size());
   up(b.bias_tc, bias_tc.data(), sizeof(float) * bias_tc.size());
@@ -500,6 +540,10 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   // padded AEV rows are never written by K2: zero everything once
   if (cudaMemset(b.aev, 0, sizeof(float) * (size_t)c->sz.n_rows * AEV_LEN) != cudaSuccess) ok = false;
   if (cudaMemset(b.status, 0, 256) != cudaSuccess) ok = false;
+  if (cudaMemset(b.work, 0, 64) != cudaSuccess) ok = false;
+  if (c->k1_smem > 48 * 1024 &&
+      cudaFuncSetAttribute(k1_brute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->k1_smem) != cudaSuccess)
+    ok = false;
   if (cudaMemset(b.xlo, 0, sizeof(float4) * N) != cudaSuccess) ok = false;
 #define K3_SMEM_ATTR(TM_, DEEP_)                                                                       \
   if (cudaFuncSetAttribute(k3_mlp_fp32_kernel<TM_, DEEP_>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
@@ -512,9 +556,8 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (cudaFuncSetAttribute(k3_mlp_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)TC_SMEM_BYTES) != cudaSuccess) ok = false;
   {
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && sms > 0)
       c->n_sms = sms;
   }
   {
@@ -524,59 +567,86 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
     // quantise the grid finest.  A batch that cannot give every SM a 32-row tile uses 16-row tiles
     // with the deep staging ring (config 0: 47 -> 43 us, config 2: 49 -> 45 us against two buffers;
     // with several CTAs per SM the ring is slower: config 4 2.52 ms, config 3 0.27 ms).
-    // PFC_K3_TM / PFC_K3_DEEP override (tuning only).
+    // pfc_tuning_t.k3_tile_rows / k3_deep_ring override (tests reach every variant through them).
     auto tiles = [&](int tm) { int n = 0; for (int e = 0; e < NSPEC; ++e) n += (count[e] + tm - 1) / tm; return n; };
     // (16-row tiles only when they spread the batch over clearly more SMs than 32-row tiles would:
     // config 2, 95 vs 48 tiles, 47 vs 53 us; config 0 has 4 tiles either way and the packed 32-row
     // kernel takes 37 us against 45 us)
     c->mlp_tm = (tiles(32) >= c->n_sms || 2 * tiles(16) < 3 * tiles(32)) ? 32 : 16;
     c->mlp_deep = c->mlp_tm == 16;
-    if (const char* ov = getenv("PFC_K3_TM")) {
-      const int v = atoi(ov);
-      if (v == 16 || v == 32 || v == 64 || v == 128) c->mlp_tm = v;
-    }
-    if (const char* ov = getenv("PFC_K3_DEEP")) c->mlp_deep = atoi(ov) != 0 && c->mlp_tm <= 32;
+    if (tun.k3_tile_rows) { c->mlp_tm = tun.k3_tile_rows; c->mlp_deep = false; }
+    if (tun.k3_deep_ring) c->mlp_deep = tun.k3_deep_ring == 2;
+    if (c->mlp_tm > 32) c->mlp_deep = false;            // the ring exists for tiles of <= 32 rows
   }
   if (cudaDeviceSynchronize() != cudaSuccess) ok = false;
   if (!ok) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
   // launch counts (static: depends only on the configuration)
-  c->launches_ef = 8 + (c->sz.n_scan_blocks > 1 ? 1 : 0) + (c->n_cell_sys > 0 ? 6 : 0);
+  c->launches_ef = 5 + (c->n_items > 0 ? 1 : 0) + (c->n_cell_sys > 0 ? 5 : 0);
   c->launches_step = c->launches_ef + 1;
   *out = c;
   return PFC_OK;
 }
 
+// the cached graph of this buffer triple, captured on first sight (least recently used slot evicted)
+static int ef_graph(pfc_ctx* c, const float4* pos, float* E, float4* F, bool with_xlo, cudaGraphExec_t* out) {
+  EfGraph* slot = &c->ef[0];
+  for (EfGraph& g : c->ef) {
+    if (g.exec && g.pos == pos && g.E == E && g.F == F && g.with_xlo == with_xlo) {
+      g.last_use = ++c->ef_clock;
+      *out = g.exec;
+      return PFC_OK;
+    }
+    if (!g.exec) { if (slot->exec) slot = &g; }
+    else if (slot->exec && g.last_use < slot->last_use) slot = &g;
+  }
+  if (slot->exec) { cudaGraphExecDestroy(slot->exec); slot->exec = nullptr; }
+  const int rc = capture(c, 0, 1, pos, E, F, with_xlo, &slot->exec);
+  if (rc != PFC_OK) return rc;
+  slot->pos = pos; slot->E = E; slot->F = F; slot->with_xlo = with_xlo;
+  slot->last_use = ++c->ef_clock;
+  *out = slot->exec;
+  return PFC_OK;
+}
+
 int pfc_energy_forces(pfc_t* c, const float* pos, float* E, float* F, void* stream) {
   if (!c || !pos || !E || !F) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
   cudaStream_t st = (cudaStream_t)stream;
-  c->launch_counter = 0;
-  enqueue_forces(c, (const float4*)pos, E, (float4*)F, st);
+  // the low position words belong to the bound MD state only
+  const bool with_xlo = c->bound && (const float4*)pos == c->pos;
+  cudaGraphExec_t g = nullptr;
+  const int rc = ef_graph(c, (const float4*)pos, E, (float4*)F, with_xlo, &g);
+  if (rc != PFC_OK) return rc;
+  if (cudaGraphLaunch(g, st) != cudaSuccess) { cudaGetLastError(); return PFC_ERR_CUDA; }
   if (!c->bound) c->stream = st;
-  return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+  return PFC_OK;
 }
 
 int pfc_energy_forces_nm(pfc_t* c, const float* pos_nm, float* E_kj, float* F_kj_nm, void* stream) {
   if (!c || !pos_nm || !E_kj) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
   if (c->bound && (c->pos == c->b.h_pos)) return PFC_ERR_STATE;   // the staging buffers hold a pfc_run_host state
   cudaStream_t st = (cudaStream_t)stream;
   const int N = c->sz.n_atoms, NS = c->sz.n_systems;
   Buffers& b = c->b;
-  c->launch_counter = 0;
-  LAUNCH(c, k0_pack_nm_kernel, cdiv(N, K0_THREADS), K0_THREADS, 0, st, N, pos_nm, b.h_pos);
-  enqueue_forces(c, b.h_pos, b.h_E, b.h_frc, st);
-  LAUNCH(c, k0_unpack_kj_kernel, cdiv(N > NS ? N : NS, K0_THREADS), K0_THREADS, 0, st, N, NS, b.h_frc, b.h_E,
-         F_kj_nm, E_kj);
+  k0_pack_nm_kernel<<<cdiv(N, K0_THREADS), K0_THREADS, 0, st>>>(N, pos_nm, b.h_pos);
+  cudaGraphExec_t g = nullptr;
+  const int rc = ef_graph(c, b.h_pos, b.h_E, b.h_frc, false, &g);
+  if (rc != PFC_OK) return rc;
+  if (cudaGraphLaunch(g, st) != cudaSuccess) { cudaGetLastError(); return PFC_ERR_CUDA; }
+  k0_unpack_kj_kernel<<<cdiv(N > NS ? N : NS, K0_THREADS), K0_THREADS, 0, st>>>(N, NS, b.h_frc, b.h_E, F_kj_nm, E_kj);
   if (!c->bound) c->stream = st;
   return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
 }
 
 int pfc_profile_stages(pfc_t* c, const float* pos, float* E, float* F, void* stream, float* ms) {
   if (!c || !pos || !E || !F || !ms) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
   cudaStream_t st = (cudaStream_t)stream;
   cudaEvent_t ev[PFC_N_STAGES + 1];
   for (int k = 0; k <= PFC_N_STAGES; ++k)
     if (cudaEventCreate(&ev[k]) != cudaSuccess) return PFC_ERR_CUDA;
-  enqueue_forces(c, (const float4*)pos, E, (float4*)F, st, ev);
+  enqueue_forces(c, (const float4*)pos, E, (float4*)F, c->bound && (const float4*)pos == c->pos, st, ev);
   int rc = cudaStreamSynchronize(st) == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
   for (int k = 0; k < PFC_N_STAGES && rc == PFC_OK; ++k)
     if (cudaEventElapsedTime(&ms[k], ev[k], ev[k + 1]) != cudaSuccess) rc = PFC_ERR_CUDA;
@@ -584,12 +654,41 @@ int pfc_profile_stages(pfc_t* c, const float* pos, float* E, float* F, void* str
   return rc;
 }
 
+// sums the row counts of the last evaluation: {radial entries, angular entries, triples}
+__global__ void k_work_counts_kernel(int n_atoms, const int2* __restrict__ cnt, unsigned long long* __restrict__ out) {
+  unsigned long long r = 0, a = 0, t = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_atoms; i += gridDim.x * blockDim.x) {
+    const int2 c = cnt[i];
+    r += (unsigned long long)c.x; a += (unsigned long long)c.y;
+    t += (unsigned long long)((long long)c.y * (c.y - 1) / 2);
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    r += __shfl_xor_sync(0xffffffffu, r, o); a += __shfl_xor_sync(0xffffffffu, a, o); t += __shfl_xor_sync(0xffffffffu, t, o);
+  }
+  if ((threadIdx.x & 31) == 0) { atomicAdd(out, r); atomicAdd(out + 1, a); atomicAdd(out + 2, t); }
+}
+
+int pfc_work_counts(pfc_t* c, int64_t* counts) {
+  if (!c || !counts) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
+  cudaStream_t st = c->stream;
+  if (cudaMemsetAsync(c->b.work, 0, 64, st) != cudaSuccess) return PFC_ERR_CUDA;
+  k_work_counts_kernel<<<148, 256, 0, st>>>(c->sz.n_atoms, c->b.cnt, c->b.work);
+  unsigned long long h[3];
+  if (cudaMemcpyAsync(h, c->b.work, sizeof(h), cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return PFC_ERR_CUDA;
+  counts[0] = (int64_t)h[0]; counts[1] = (int64_t)h[1]; counts[2] = (int64_t)h[2];
+  counts[3] = (int64_t)c->brute_tests;
+  return PFC_OK;
+}
+
 int pfc_set_state(pfc_t* c, float* pos, float* vel, float* E, float* F, void* stream) {
   if (!c || !pos || !vel || !E || !F) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
   cudaStream_t st = (cudaStream_t)stream;
   const bool same = c->bound && c->pos == (float4*)pos && c->vel == (float4*)vel && c->E == E &&
                     c->frc == (float4*)F;
-  if (!same) drop_graphs(c);                       // pointers are baked into the graphs
+  if (!same) drop_state_graphs(c);                 // pointers are baked into the graphs
   c->pos = (float4*)pos; c->vel = (float4*)vel; c->E = E; c->frc = (float4*)F;
   c->stream = st;
   c->bound = true;
@@ -614,12 +713,22 @@ static int maybe_store_frame(pfc_ctx* c, cudaStream_t st) {
   return PFC_OK;
 }
 
+// steps until (and including) the next one after which a frame is due; a huge number if none
+static long long steps_to_next_frame(const pfc_ctx* c) {
+  if (!c->frames || c->frame_stride <= 0 || c->frames_written >= c->frame_cap) return 1LL << 60;
+  return c->frame_stride - (c->steps_total % c->frame_stride);
+}
+
 static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
   cudaStream_t st = c->stream;
   int rc;
-  if (!c->g_forces && (rc = capture(c, 0, &c->g_forces, &c->launches_ef)) != PFC_OK) return rc;
-  cudaGraphExec_t* gs = langevin ? &c->g_lstep : &c->g_step;
-  if (!*gs && (rc = capture(c, langevin ? 2 : 1, gs, langevin ? &c->launches_lstep : &c->launches_step)) != PFC_OK)
+  const int kind = langevin ? 2 : 1;
+  if (!c->g_forces && (rc = capture(c, 0, 1, c->pos, c->E, c->frc, true, &c->g_forces)) != PFC_OK) return rc;
+  cudaGraphExec_t* g1 = langevin ? &c->g_lstep : &c->g_step;
+  cudaGraphExec_t* gk = langevin ? &c->g_lstepk : &c->g_stepk;
+  if (!*g1 && (rc = capture(c, kind, 1, c->pos, c->E, c->frc, true, g1)) != PFC_OK) return rc;
+  const int K = c->steps_per_graph;
+  if (K > 1 && n_steps - 1 >= K && !*gk && (rc = capture(c, kind, K, c->pos, c->E, c->frc, true, gk)) != PFC_OK)
     return rc;
   if (dt_fs != c->cur_dt) {
     k5_set_params_kernel<<<1, 1, 0, st>>>(c->b.sp, dt_fs);
@@ -630,14 +739,24 @@ static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
     c->forces_stale = false;
   }
   if (n_steps == 0) return PFC_OK;
-  // step 1: half kick + drift, forces.  steps 2..n: one graph each = fused
-  // (trailing half kick + leading half kick + drift), forces.  Then the last half kick.
+  // step 1: half kick + drift, forces.  steps 2..n: fused (trailing half kick + leading half kick +
+  // drift), forces -- K of them per graph launch while no frame falls inside the span, else one per
+  // launch.  Then the last half kick.
   if (langevin) enqueue_langevin<1>(c, st); else enqueue_verlet<1>(c, st);
   if (cudaGraphLaunch(c->g_forces, st) != cudaSuccess) return PFC_ERR_CUDA;
   if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
-  for (int s = 1; s < n_steps; ++s) {
-    if (cudaGraphLaunch(*gs, st) != cudaSuccess) return PFC_ERR_CUDA;
-    if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
+  int left = n_steps - 1;
+  while (left > 0) {
+    if (*gk && left >= K && steps_to_next_frame(c) >= K) {
+      if (cudaGraphLaunch(*gk, st) != cudaSuccess) return PFC_ERR_CUDA;
+      c->steps_total += K - 1;                       // (no frame is due inside the span)
+      if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
+      left -= K;
+    } else {
+      if (cudaGraphLaunch(*g1, st) != cudaSuccess) return PFC_ERR_CUDA;
+      if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
+      --left;
+    }
   }
   enqueue_verlet<0>(c, st);
   return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
@@ -645,7 +764,7 @@ static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
 
 int pfc_step(pfc_t* c, int32_t n_steps, float dt_fs) {
   if (!c || n_steps < 0 || !(dt_fs > 0.0f)) return PFC_ERR_ARG;
-  if (!c->bound) return PFC_ERR_STATE;
+  if (!c->bound || !on_device(c)) return PFC_ERR_STATE;
   return run_steps(c, n_steps, dt_fs, false);
 }
 
@@ -653,7 +772,7 @@ int pfc_step_langevin(pfc_t* c, int32_t n_steps, float dt_fs, float friction_per
                       uint64_t seed) {
   if (!c || n_steps < 0 || !(dt_fs > 0.0f) || !(friction_per_fs >= 0.0f) || !(temperature_K >= 0.0f))
     return PFC_ERR_ARG;
-  if (!c->bound) return PFC_ERR_STATE;
+  if (!c->bound || !on_device(c)) return PFC_ERR_STATE;
   if (friction_per_fs != c->lg_gamma || temperature_K != c->lg_T || dt_fs != c->lg_dt || seed != c->lg_seed) {
     const double c1 = exp(-(double)friction_per_fs * (double)dt_fs), c2 = sqrt(1.0 - c1 * c1);
     k5_set_langevin_kernel<<<1, 1, 0, c->stream>>>(c->b.sp, (float)c1, (float)c2,
@@ -682,6 +801,7 @@ int pfc_frames_written(pfc_t* c, int32_t* n) {
 static int run_host_impl(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, float dt_fs, float* E_h,
                          float* F_h, void* stream, bool forces_in) {
   if (!c || !pos_h || !vel_h || !E_h || (forces_in && !F_h)) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
   cudaStream_t st = (cudaStream_t)stream;
   const size_t nb = sizeof(float4) * (size_t)c->sz.n_atoms;
   Buffers& b = c->b;
@@ -713,10 +833,20 @@ int pfc_run_host_resume(pfc_t* c, float* pos_h, float* vel_h, float* F_h, int32_
 int pfc_get_neighbors(pfc_t* c, const int32_t** r_off, const int32_t** r_idx, const int32_t** a_off,
                       const int32_t** a_idx) {
   if (!c) return PFC_ERR_ARG;
-  if (r_off) *r_off = c->b.r_off;
-  if (r_idx) *r_idx = c->b.r_idx;
-  if (a_off) *a_off = c->b.a_off;
-  if (a_idx) *a_idx = c->b.a_idx;
+  if (!on_device(c)) return PFC_ERR_STATE;
+  // export the step path's fixed-capacity rows into the canonical CSR (reading S7)
+  const Sizes& s = c->sz;
+  const Buffers& b = c->b;
+  cudaStream_t st = c->stream;
+  if (s.n_scan_blocks > 1) k1_scan_totals_kernel<<<s.n_scan_blocks, SCAN_THREADS, 0, st>>>(s.n_atoms, b.cnt, b.block_tot);
+  k1_scan_kernel<<<s.n_scan_blocks, SCAN_THREADS, 0, st>>>(s.n_atoms, b.cnt, b.block_tot, b.r_off, b.a_off);
+  k1_export_csr_kernel<<<cdiv(s.n_atoms, K1_WARPS), K1_WARPS * 32, 0, st>>>(s.n_atoms, b.row_beg, b.nbr, b.cnt, b.r_off,
+                                                                          b.a_off, b.r_idx, b.a_idx);
+  if (cudaGetLastError() != cudaSuccess) return PFC_ERR_CUDA;
+  if (r_off) *r_off = b.r_off;
+  if (r_idx) *r_idx = b.r_idx;
+  if (a_off) *a_off = b.a_off;
+  if (a_idx) *a_idx = b.a_idx;
   return PFC_OK;
 }
 
@@ -730,13 +860,6 @@ int pfc_get_intermediates(pfc_t* c, const float** aev, const float** g, const in
   return PFC_OK;
 }
 
-int pfc_get_capacities(pfc_t* c, int32_t* cap_r, int32_t* cap_a) {
-  if (!c) return PFC_ERR_ARG;
-  if (cap_r) *cap_r = c->sz.cap_r;
-  if (cap_a) *cap_a = c->sz.cap_a;
-  return PFC_OK;
-}
-
 int pfc_copy_to_host(const void* src, void* dst, size_t bytes) {
   if (!src || !dst) return PFC_ERR_ARG;
   return cudaMemcpy(dst, src, bytes, cudaMemcpyDeviceToHost) == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
@@ -744,6 +867,7 @@ int pfc_copy_to_host(const void* src, void* dst, size_t bytes) {
 
 int pfc_status(pfc_t* c, uint32_t* bits) {
   if (!c || !bits) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
   if (cudaStreamSynchronize(c->stream) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpy(bits, c->b.status, sizeof(uint32_t), cudaMemcpyDeviceToHost) != cudaSuccess) return PFC_ERR_CUDA;
   return PFC_OK;
@@ -755,16 +879,19 @@ int pfc_mlp_path(pfc_t* c, int32_t* path) {
   return PFC_OK;
 }
 
-int pfc_launch_counts(pfc_t* c, int32_t* per_ef, int32_t* per_step) {
+int pfc_launch_counts(pfc_t* c, int32_t* per_ef, int32_t* per_step, int32_t* steps_per_graph) {
   if (!c) return PFC_ERR_ARG;
   if (per_ef) *per_ef = c->launches_ef;
   if (per_step) *per_step = c->launches_step;
+  if (steps_per_graph) *steps_per_graph = c->steps_per_graph;
   return PFC_OK;
 }
 
 int pfc_destroy(pfc_t* c) {
   if (!c) return PFC_ERR_ARG;
-  drop_graphs(c);
+  drop_state_graphs(c);
+  for (EfGraph& g : c->ef)
+    if (g.exec) cudaGraphExecDestroy(g.exec);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   delete c;
   return PFC_OK;
@@ -778,7 +905,7 @@ const char* pfc_error_string(int code) {
     case PFC_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
     case PFC_ERR_CUDA: return "CUDA runtime error";
     case PFC_ERR_CAPTURE: return "CUDA graph capture failed";
-    case PFC_ERR_STATE: return "pfc_step called before pfc_set_state";
+    case PFC_ERR_STATE: return "no MD state bound (pfc_set_state), or the handle's CUDA device is not current";
     default: return "unknown pfc error";
   }
 }

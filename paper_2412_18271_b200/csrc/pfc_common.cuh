@@ -34,20 +34,38 @@ constexpr float ACC_F = 9.648533216e-3f;           // (A/fs^2) per (eV/A/amu)
 constexpr uint32_t ST_RADIAL_OVERFLOW = 1u, ST_ANGULAR_OVERFLOW = 2u, ST_ANGULAR_ROW = 4u,
                    ST_NONFINITE = 8u, ST_CELL_OVERFLOW = 16u;
 
-// Tables in constant memory, filled by pfc_create.
+// Model tables in constant memory: compile-time constants, identical for every handle (nothing
+// per-handle lives in constant memory; the masses are in StepParams).
+//   shf_r[k] = (float)(0.9 + k*0.26875)  (S2);  shf_a = 0.9, 1.55, 2.2, 2.85  (S3);
+//   cos_z[b], sin_z[b] = (float)cos / sin of (double)(float)SHF_Z[b], SHF_Z = 0.19634954 + b*pi/8 as
+//   the fp32 literals of DESIGN.md (S3, S8).
 struct ModelTables {
-  float shf_r[NSHF_R];   // 0.9 + k*0.26875           (S2)
-  float shf_a[NSHF_A];   // 0.9, 1.55, 2.2, 2.85      (S3)
-  float cos_z[NSHF_Z];   // cos(SHF_Z[b]),  SHF_Z[b] = (float)(pi/16 + b*pi/8)  (S3)
+  float shf_r[NSHF_R];
+  float shf_a[NSHF_A];
+  float cos_z[NSHF_Z];
   float sin_z[NSHF_Z];
-  float inv_mass_acc[NSPEC];  // ACC / m_s
 };
-__constant__ ModelTables c_tab;
+__constant__ ModelTables c_tab = {
+    {0.9f, 1.16875f, 1.4375f, 1.70625f, 1.975f, 2.24375f, 2.5125f, 2.78125f,
+     3.05f, 3.31875f, 3.5875f, 3.85625f, 4.125f, 4.39375f, 4.6625f, 4.93125f},
+    {0.9f, 1.55f, 2.2f, 2.85f},
+    {0.9807852506637573f, 0.8314695954322815f, 0.5555702447891235f, 0.19509035348892212f,
+     -0.19509032368659973f, -0.5555701851844788f, -0.8314696550369263f, -0.9807853102684021f},
+    {0.19509032368659973f, 0.5555702447891235f, 0.8314695954322815f, 0.9807852506637573f,
+     0.9807852506637573f, 0.8314696550369263f, 0.5555701851844788f, 0.19509030878543854f}};
+
+// Neighbour-row entry word (internal format of K1's rows): bits 0..28 neighbour index j,
+// bits 29..30 species of j, bit 31 set when j is also an angular neighbour (d2 < RC2_A).
+constexpr uint32_t NBR_IDX_MASK = 0x1FFFFFFFu;
+__device__ __forceinline__ int nbr_index(uint32_t w) { return (int)(w & NBR_IDX_MASK); }
+__device__ __forceinline__ int nbr_species(uint32_t w) { return (int)((w >> 29) & 3u); }
+__device__ __forceinline__ bool nbr_angular(uint32_t w) { return (w >> 31) != 0u; }
 
 // Step parameters live in device memory so a captured graph is reusable for any dt.
 struct StepParams {
   float dt;        // fs
   float half_dt;   // dt/2
+  float inv_mass_acc[NSPEC];  // ACC / m_s of THIS handle (pfc_desc_t.masses_amu)
   // Langevin (O9): v <- c1 v + sigma[species] xi,  sigma_s = c2 sqrt(kB T ACC / m_s)
   float c1;
   float sigma[NSPEC];

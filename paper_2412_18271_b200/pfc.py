@@ -32,13 +32,23 @@ STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
 N_STAGES = 6
 STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum")
 
-EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy_forces_nm", "pfc_profile_stages", "pfc_set_state", "pfc_step",
-           "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host", "pfc_run_host_resume", "pfc_get_neighbors", "pfc_get_capacities", "pfc_get_intermediates", "pfc_status",
-           "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts", "pfc_destroy", "pfc_error_string")
+# include/pfc.h (the provider boundary) and include/pfc_debug.h (measurement / parity helpers)
+EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy_forces_nm", "pfc_set_state",
+           "pfc_step", "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host",
+           "pfc_run_host_resume", "pfc_get_neighbors", "pfc_get_intermediates", "pfc_status", "pfc_destroy",
+           "pfc_error_string")
+DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts")
 
 
 class PfcError(RuntimeError):
     pass
+
+
+class Tuning(ctypes.Structure):
+    """pfc_tuning_t (include/pfc.h): a zero-filled struct is "all defaults"."""
+    _fields_ = [("k3_tile_rows", c_int32), ("k3_deep_ring", c_int32), ("tc_comp_override", c_int32),
+                ("tc_comp_forward", c_float), ("tc_comp_backward", c_float), ("steps_per_graph", c_int32),
+                ("reserved", c_int32 * 2)]
 
 
 class _Desc(ctypes.Structure):
@@ -46,7 +56,7 @@ class _Desc(ctypes.Structure):
                 ("species", POINTER(c_int32)), ("sys_offsets", POINTER(c_int32)),
                 ("weights", POINTER(c_float)), ("masses_amu", POINTER(c_float)),
                 ("workspace", c_void_p), ("workspace_bytes", c_size_t),
-                ("mlp_path", c_int32)]
+                ("mlp_path", c_int32), ("tuning", POINTER(Tuning))]
 
 
 _lib = None
@@ -77,16 +87,16 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_run_host.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p, c_void_p]
     lib.pfc_run_host_resume.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p]
     lib.pfc_get_neighbors.argtypes = [c_void_p, pp_i32, pp_i32, pp_i32, pp_i32]
-    lib.pfc_get_capacities.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32)]
+    lib.pfc_work_counts.argtypes = [c_void_p, POINTER(ctypes.c_int64)]
     lib.pfc_get_intermediates.argtypes = [c_void_p, pp_f, pp_f, pp_i32, POINTER(c_int32)]
     lib.pfc_copy_to_host.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.pfc_status.argtypes = [c_void_p, POINTER(c_uint32)]
     lib.pfc_mlp_path.argtypes = [c_void_p, POINTER(c_int32)]
-    lib.pfc_launch_counts.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32)]
+    lib.pfc_launch_counts.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32)]
     lib.pfc_destroy.argtypes = [c_void_p]
     lib.pfc_error_string.argtypes = [c_int]
     lib.pfc_error_string.restype = c_char_p
-    for name in EXPORTS:
+    for name in EXPORTS + DEBUG_EXPORTS:
         if name not in ("pfc_workspace_bytes", "pfc_error_string"):
             getattr(lib, name).restype = c_int
     _lib = lib
@@ -108,11 +118,24 @@ def _stream_ptr(stream) -> int:
     return int(s.cuda_stream)
 
 
+def _on_device(method):
+    """Run a Pfc method with the handle's CUDA device current (the library checks it: a handle is
+    bound to the device it was created on), so that a handle on cuda:1 works while cuda:0 is current."""
+    import functools
+
+    @functools.wraps(method)
+    def wrapper(self, *args, **kwargs):
+        import torch
+        with torch.cuda.device(self.device):
+            return method(self, *args, **kwargs)
+    return wrapper
+
+
 class Pfc:
     """One handle = one set of systems + one potential (pfc_create .. pfc_destroy)."""
 
     def __init__(self, species, sys_offsets, weights, masses_amu=None, mlp_path: int = MLP_AUTO,
-                 device="cuda:0"):
+                 device="cuda:0", tuning: "Tuning | None" = None):
         import torch
         if not torch.cuda.is_available():
             raise PfcError("pfc needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -136,13 +159,15 @@ class Pfc:
                       species.ctypes.data_as(POINTER(c_int32)), sys_offsets.ctypes.data_as(POINTER(c_int32)),
                       weights.ctypes.data_as(POINTER(c_float)),
                       None if masses is None else masses.ctypes.data_as(POINTER(c_float)),
-                      c_void_p(base), c_size_t(nbytes), int(mlp_path))
+                      c_void_p(base), c_size_t(nbytes), int(mlp_path),
+                      None if tuning is None else ctypes.pointer(tuning))
             h = c_void_p()
             _check(self._lib.pfc_create(byref(d), byref(h)), "pfc_create")
         self._h = h
         self._bound = None
 
     # -- pfc_energy_forces ------------------------------------------------------
+    @_on_device
     def energy_forces(self, pos, E=None, F=None, stream=None):
         """pos: cuda float32 [N,4].  Returns (E [n_systems], F [N,4] = {Fx,Fy,Fz,e_i}); enqueues only."""
         import torch
@@ -157,6 +182,7 @@ class Pfc:
                                            _stream_ptr(stream)), "pfc_energy_forces")
         return E, F
 
+    @_on_device
     def profile_stages(self, pos, E, F, stream=None):
         """Per-stage device times (ms) of one energy_forces pass; synchronises."""
         ms = (c_float * N_STAGES)()
@@ -165,6 +191,7 @@ class Pfc:
         return [float(x) for x in ms]
 
     # -- pfc_set_state / pfc_step -------------------------------------------------
+    @_on_device
     def set_state(self, pos, vel, E=None, F=None, stream=None):
         import torch
         self._expect(pos, (self.n_atoms, 4))
@@ -180,9 +207,11 @@ class Pfc:
         self._bound = (pos, vel, E, F)          # keep the tensors alive while bound
         return E, F
 
+    @_on_device
     def step(self, n_steps: int, dt_fs: float = 0.5):
         _check(self._lib.pfc_step(self._h, int(n_steps), float(dt_fs)), "pfc_step")
 
+    @_on_device
     def energy_forces_nm(self, pos_nm, want_forces: bool = True, stream=None):
         """Provider call in the paper's units: pos_nm cuda [N,3] float32 (nm) -> (E kJ/mol [n_systems],
         F kJ/mol/nm [N,3] or None).  Marshalling only; the conversion runs in the library's kernels."""
@@ -195,10 +224,12 @@ class Pfc:
                "pfc_energy_forces_nm")
         return E, F
 
+    @_on_device
     def step_langevin(self, n_steps: int, dt_fs: float, friction_per_fs: float, temperature_K: float, seed: int):
         _check(self._lib.pfc_step_langevin(self._h, int(n_steps), float(dt_fs), float(friction_per_fs),
                                            float(temperature_K), int(seed)), "pfc_step_langevin")
 
+    @_on_device
     def set_frames(self, frames, stride: int):
         """frames: device tensor [max_frames, N, 4] float32 (None unbinds)."""
         if frames is None:
@@ -215,6 +246,7 @@ class Pfc:
         return int(n.value)
 
     # -- pfc_run_host -------------------------------------------------------------
+    @_on_device
     def run_host(self, pos_host, vel_host, n_steps: int, dt_fs: float, E_host, F_host=None, stream=None):
         """Host tensors/arrays [N,4] float32 (pinned for async copies), updated in place."""
         def ptr(a):
@@ -224,6 +256,7 @@ class Pfc:
         _check(self._lib.pfc_run_host(self._h, ptr(pos_host), ptr(vel_host), int(n_steps), float(dt_fs),
                                       ptr(E_host), ptr(F_host), _stream_ptr(stream)), "pfc_run_host")
 
+    @_on_device
     def run_host_resume(self, pos_host, vel_host, F_host, n_steps: int, dt_fs: float, E_host, stream=None):
         """As run_host, with F_host [N,4] holding the forces at pos_host on entry (uploaded, not recomputed)."""
         def ptr(a):
@@ -238,6 +271,7 @@ class Pfc:
         _check(self._lib.pfc_mlp_path(self._h, byref(v)), "pfc_mlp_path")
         return int(v.value)
 
+    @_on_device
     def status(self) -> int:
         bits = c_uint32()
         _check(self._lib.pfc_status(self._h, byref(bits)), "pfc_status")
@@ -249,24 +283,38 @@ class Pfc:
             raise PfcError("device status: " + ", ".join(v for k, v in STATUS_BITS.items() if bits & k))
 
     def launch_counts(self):
-        a, b = c_int32(), c_int32()
-        _check(self._lib.pfc_launch_counts(self._h, byref(a), byref(b)), "pfc_launch_counts")
+        """(kernel launches per energy/forces evaluation, per steady-state MD step)."""
+        a, b, k = c_int32(), c_int32(), c_int32()
+        _check(self._lib.pfc_launch_counts(self._h, byref(a), byref(b), byref(k)), "pfc_launch_counts")
         return int(a.value), int(b.value)
 
+    def steps_per_graph(self) -> int:
+        a, b, k = c_int32(), c_int32(), c_int32()
+        _check(self._lib.pfc_launch_counts(self._h, byref(a), byref(b), byref(k)), "pfc_launch_counts")
+        return int(k.value)
+
+    @_on_device
+    def work_counts(self):
+        """Row totals of the last evaluation: dict(radial, angular, triples, brute_tests); synchronises."""
+        v = (ctypes.c_int64 * 4)()
+        _check(self._lib.pfc_work_counts(self._h, v), "pfc_work_counts")
+        return {"radial": int(v[0]), "angular": int(v[1]), "triples": int(v[2]), "brute_tests": int(v[3])}
+
+    @_on_device
     def neighbors(self):
-        """Copies the CSR lists of the last evaluation to host numpy arrays (synchronises)."""
+        """The neighbour lists of the last evaluation as int32 CSR (r_off, r_idx, a_off, a_idx), copied
+        to host numpy arrays (pfc_get_neighbors exports the step path's rows; synchronises)."""
         import torch
         p = [POINTER(c_int32)() for _ in range(4)]
         _check(self._lib.pfc_get_neighbors(self._h, *[byref(x) for x in p]), "pfc_get_neighbors")
         torch.cuda.synchronize(self.device)
         r_off = self._copy(p[0], self.n_atoms + 1, np.int32)
         a_off = self._copy(p[2], self.n_atoms + 1, np.int32)
-        cr, ca = c_int32(), c_int32()
-        _check(self._lib.pfc_get_capacities(self._h, byref(cr), byref(ca)), "pfc_get_capacities")
-        r_idx = self._copy(p[1], min(int(r_off[-1]), cr.value), np.int32)   # rows past the capacity
-        a_idx = self._copy(p[3], min(int(a_off[-1]), ca.value), np.int32)   # were never written
+        r_idx = self._copy(p[1], int(r_off[-1]), np.int32)
+        a_idx = self._copy(p[3], int(a_off[-1]), np.int32)
         return r_off, r_idx, a_off, a_idx
 
+    @_on_device
     def intermediates(self):
         """(aev [N,384], g [N,384]) of the last evaluation in ATOM order (host copies)."""
         import torch
@@ -293,6 +341,7 @@ class Pfc:
                 and tuple(t.shape) == tuple(shape) and t.is_contiguous()):
             raise PfcError(f"expected a contiguous cuda float32 tensor of shape {shape}")
 
+    @_on_device
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
             self._lib.pfc_destroy(self._h)

@@ -1,5 +1,6 @@
-"""The C-ABI library loads without a GPU and exports every entry point include/pfc.h declares; the
-Python binding lists exactly the same names (no compute calls here)."""
+"""The C-ABI library loads without a GPU and exports every entry point include/*.h declares; the
+Python binding lists exactly the same names (no compute calls here); the library reads no
+environment variable."""
 import ctypes
 import os
 import re
@@ -7,8 +8,8 @@ import re
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared():
-    text = open(os.path.join(ROOT, "include", "pfc.h")).read()
+def _declared(header="pfc.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return set(re.findall(r"\b(pfc_[a-z0-9_]+)\s*\(", text))
 
@@ -17,11 +18,23 @@ def test_library_exports_every_declared_symbol():
     from paper_2412_18271_b200 import build, pfc
     build.build_libpfc()
     lib = ctypes.CDLL(pfc.LIB_PATH)
-    names = _declared()
+    names, debug = _declared("pfc.h"), _declared("pfc_debug.h")
     assert {"pfc_create", "pfc_energy_forces", "pfc_step", "pfc_destroy"} <= names      # the north_star four
-    missing = [n for n in sorted(names) if not hasattr(lib, n)]
+    missing = [n for n in sorted(names | debug) if not hasattr(lib, n)]
     assert not missing, missing
     assert set(pfc.EXPORTS) == names
+    assert set(pfc.DEBUG_EXPORTS) == debug
+    assert len(names) <= 16                                    # "keep them few"
+
+
+def test_library_reads_no_environment_variable():
+    """SURVEY.md section 5 / north_star: no env-var dispatch.  Tuning goes through pfc_tuning_t."""
+    csrc = os.path.join(ROOT, "paper_2412_18271_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+    from paper_2412_18271_b200 import pfc
+    import ctypes as C
+    assert C.sizeof(pfc.Tuning) == 32                          # mirrors pfc_tuning_t
 
 
 def test_host_only_entry_points_work_without_a_device():

@@ -118,13 +118,12 @@ def test_tf32x3_trajectory_config1(pfc, weights):
     _trajectory(pfc, weights, W.make_config(1), 100)
 
 
-def test_uncompensated_tf32x3_misses_the_trajectory_bar(pfc, weights, monkeypatch):
-    """Evidence for the compensation: switched off (PFC_TC_COMP_F/B = 0, experiment overrides) the
-    worst replica of config 1 leaves the 1e-4 A bar while all the others keep it."""
-    monkeypatch.setenv("PFC_TC_COMP_F", "0")
-    monkeypatch.setenv("PFC_TC_COMP_B", "0")
+def test_uncompensated_tf32x3_misses_the_trajectory_bar(pfc, weights):
+    """Evidence for the compensation: switched off (pfc_tuning_t.tc_comp_override with both factors 0)
+    the worst replica of config 1 leaves the 1e-4 A bar while all the others keep it."""
     wl = W.make_config(1)
-    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TF32X3)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TF32X3,
+                tuning=pfc.Tuning(tc_comp_override=1, tc_comp_forward=0.0, tc_comp_backward=0.0))
     pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
     p.set_state(pos, vel)
     p.step(100, wl.dt_fs)
