@@ -2,33 +2,45 @@
 // input-gradient backward, as a chain of eight grouped-GEMM phases per 128-row tile on the
 // tcgen05 tensor cores (O5 / section 5; backward = PAPER.md:67 "forces by backprop").
 //
-// Precision: kind::tf32 with the 3-term split  A*B ~= A_hi*B_hi + A_lo*B_hi + A_hi*B_lo
-// (x_hi = x rounded to 10 mantissa bits, x_lo = x - x_hi exactly), fp32 accumulation in TMEM.
-// The hardware truncates fp32 operands to tf32 (measured), so every hi part is exact and the
-// dropped terms are O(2^-21) relative.  N_TERMS = 1 is plain TF32, kept only to produce the
-// evidence that it misses the tolerance.
+// Precision: kind::f16 with a 3-term split and fp32 accumulation in TMEM,
+//     A*B ~= A_hi*B_hi + A_lo*B_hi + A_hi*B_lo,   x_hi = fp16(x),  x_lo = fp16(x - x_hi):
+// 11 + 11 significant bits per operand (x - x_hi is exact in fp32; the tensor core multiplies
+// fp16 subnormals exactly -- measured -- so a small remainder costs absolute, not relative,
+// accuracy: 3e-8 of the operand's scale).  Every operand class is pre-scaled by an exact power of
+// two that puts its typical magnitude well inside fp16's range (weights per layer and element from
+// max|W|, the AEV by 8, the backward deltas from max|w4|); the scales leave through the epilogue
+// factor of each phase (TcParams::kf), so no rounding is added.  Against the round-1 kind::tf32
+// split this is half the tensor-pipe time per k (K = 16 per MMA instead of 8), half the operand
+// bytes in shared memory and in the weight stream.  (A bf16 remainder would not need the scaling,
+// but the hardware rejects instruction descriptors that mix fp16 and bf16 operands -- measured.)
+// N_TERMS = 1 is plain FP16 operands, kept only to produce the evidence that a single 16-bit
+// term misses the tolerance.
 //
-// One persistent CTA per SM, 320 threads, one 128-row tile of ONE element in flight:
-//   warps 0-7  producers/epilogue: make the A operand of every phase in 32-wide K chunks
-//              (hi|lo, K-major, SWIZZLE_128B) into a 4-slot shared-memory ring -- phase 0 from
-//              the AEV rows in global memory, later phases from the previous accumulator in
-//              TMEM (bias, CELU, CELU', Hadamard) -- and drain g to global memory;
-//   warp 8     TMA: streams the pre-packed, pre-swizzled weight chunks (hi|lo) of the phase
-//              schedule from L2 into a 2-slot ring with cp.async.bulk + mbarrier;
+// One persistent CTA per SM, 320 threads, 128-row tiles of ONE element each:
+//   warps 0-7  workers: make the A operand of every phase in 32-wide K chunks (hi | lo, K-major,
+//              SWIZZLE_64B) -- phase 0 from the AEV rows in global memory, later phases from the
+//              previous accumulator in TMEM (bias, CELU, CELU', Hadamard) -- and drain g;
+//   warp 8     TMA: streams the pre-packed, pre-swizzled weight chunks (hi | lo) of the schedule
+//              from L2 into a 4-slot ring with cp.async.bulk + mbarrier;
 //   warp 9     one elected thread issues tcgen05.mma and commits to the ring / phase barriers.
-// TMEM (512 columns) keeps the forward pre-activations z1,z2,z3 for the backward pass:
-//   z1 [0,160)  z2 [160,288)  z3 [288,384)  d2pre [384,512)  d1pre [160,320)  g-pass [384,512)
-// The accumulate step of the tensor core rounds toward zero (measured: the energy error of a
-// single-accumulator split correlates at -0.7 with the energy), one truncation per MMA, so the
-// small terms A_lo*B_hi + A_hi*B_lo of phases 0 and 2 go to an accumulator of their own
-// (S0 [352,512), S2 [384,480): free at that time) and are added on the CUDA cores; z1 is written
-// back (bias included) for the backward pass.
-// What remains of that one-sided loss is compensated in the epilogues: a chain of n MMA instructions
-// shrinks its sum by a relative beta ~ lambda * n * 2.15e-8 on average (half an ulp of the running sum
-// per step), so every phase returns z + beta_p * z (TcParams::comp; lambda measured against the fp64
-// oracle).  With it the path meets the 1e-4 A trajectory bar on all five
-// configurations and is what PFC_MLP_AUTO selects for batches of >= 4096 atoms.
+// Schedule.  The eight phases of a tile are a serial chain (each needs the previous
+// accumulator), except at its two ends: the first GEMM (AEV x W1) depends only on global
+// memory and the three g passes (delta1 x W1^T) only on delta1.  So consecutive tiles are
+// software-pipelined: while the tensor pipe runs the g passes of tile t (delta1 kept RESIDENT in
+// shared memory, produced once) it also runs the first GEMM of tile t+1 (the "overlapped
+// block"); meanwhile warps 0-3 drain g of tile t (TMEM -> global, two accumulator buffers) and
+// warps 4-7 convert the AEV chunks of tile t+1 (global -> fp16 hi | lo -> ring).  Then all eight
+// warps walk the chain z1 -> h1 -> z2 -> h2 -> z3 -> delta3 -> d2pre -> delta2 -> d1pre -> delta1.
+// TMEM (512 columns):  z1 [0,160)   z2 [160,288)   z3 [288,384)   d2pre [384,512)
+//                      d1pre [160,320)   g buffer A [384,512)   g buffer B [160,288)
+// The accumulate step of the tensor core rounds toward zero -- the running sum once per MMA
+// instruction, and every product as it is aligned to it (measured: a chain of n K=16 MMAs shrinks
+// an all-positive sum by 9e-8 n, a mixed-sign one by 2e-8 n); the one-sided loss is compensated in
+// the epilogues: every phase returns (1 + beta_p) z with beta_p = lambda n_p 2.15e-8 (kf folds it
+// in; lambda is calibrated per element against the FP32 path at first use).
 #pragma once
+#include <cuda_fp16.h>
+
 #include "pfc_common.cuh"
 #include "tc_ptx.cuh"
 
@@ -36,61 +48,124 @@ namespace pfc {
 
 constexpr int TC_TM = 128;                       // rows per tile == ROW_PAD
 constexpr int TC_THREADS = 320;
-constexpr int TC_EPI_THREADS = 256;
-constexpr int TC_NA = 4, TC_NB = 2;              // ring depths
-constexpr int TC_A_SLOT = 2 * TC_TM * 128;       // 32,768 B: hi | lo
-constexpr int TC_B_SLOT = 2 * D1 * 128;          // 40,960 B: widest N (160) hi | lo
+constexpr int TC_WORKERS = 256;                  // warps 0-7
+constexpr int TC_KC = 32;                        // k per chunk: one 64-byte SWIZZLE_64B row of fp16
+constexpr int TC_NA = 3, TC_NB = 4;              // ring depths: A operand chunks, weight chunks
+constexpr int TC_A_HALF = TC_TM * 64;            // 8,192 B: one part (hi or lo) of an A chunk
+constexpr int TC_A_SLOT = 2 * TC_A_HALF;         // 16,384 B: hi | lo
+constexpr int TC_B_SLOT = 2 * D1 * 64;           // 20,480 B: widest N (160), hi | lo
+constexpr int TC_ND1 = D1 / TC_KC;               // 5 resident delta1 chunks
 constexpr int TC_NPHASE = 8;
 constexpr int TC_GN = 128;                       // g is produced in 3 passes of 128 columns
-constexpr int TC_S0_COL = 352, TC_S2_COL = 384;  // small-term accumulators of phases 0 and 2
+constexpr int TC_NPASS = D0 / TC_GN;             // 3
+constexpr int TC_COL_Z1 = 0, TC_COL_Z2 = 160, TC_COL_Z3 = 288, TC_COL_D2 = 384, TC_COL_D1 = 160,
+              TC_COL_GA = 384, TC_COL_GB = 160;
+constexpr int TC_AEV_SCALE_LOG2 = 3;             // the AEV operand is multiplied by 8 before the split
 
-// phase schedule: N, K chunks, D column, packed-weight byte offset (per element)
+// phase schedule: N, K chunks, packed-weight byte offset (per element)
+//   0: W1 (N 160, K 384)   1: W2 (128, 160)   2: W3 (96, 128)   3: W3^T (128, 96)   4: W2^T (160, 128)
+//   5-7: W1^T in three passes (128, 160)
 __host__ __device__ constexpr int tc_phase_n(int p) {
   return p == 0 ? D1 : p == 1 ? D2 : p == 2 ? D3 : p == 3 ? D2 : p == 4 ? D1 : TC_GN;
 }
 __host__ __device__ constexpr int tc_phase_nk(int p) {
-  return p == 0 ? D0 / 32 : p == 1 ? D1 / 32 : p == 2 ? D2 / 32 : p == 3 ? D3 / 32 : p == 4 ? D2 / 32 : D1 / 32;
+  return p == 0 ? D0 / TC_KC : p == 1 ? D1 / TC_KC : p == 2 ? D2 / TC_KC : p == 3 ? D3 / TC_KC : p == 4 ? D2 / TC_KC : D1 / TC_KC;
 }
-__host__ __device__ constexpr int tc_phase_dcol(int p) {
-  return p == 0 ? 0 : p == 1 ? 160 : p == 2 ? 288 : p == 3 ? 384 : p == 4 ? 160 : 384;
-}
-__host__ __device__ constexpr int tc_chunk_bytes(int p) { return 2 * tc_phase_n(p) * 128; }
+// MMA instructions of the accumulator chain of epilogue q (0..4: phases 0..4; 5: one g pass): 2 k steps per chunk
+__host__ __device__ constexpr int tc_chain_mmas(int q, int n_terms) { return 2 * n_terms * tc_phase_nk(q); }
+__host__ __device__ constexpr int tc_chunk_bytes(int p) { return 2 * tc_phase_n(p) * 64; }
 __host__ __device__ constexpr int tc_phase_off(int p) {
   int o = 0;
   for (int q = 0; q < p; ++q) o += tc_phase_nk(q) * tc_chunk_bytes(q);
   return o;
 }
-constexpr int TC_W_BYTES_PER_ELEM = tc_phase_off(TC_NPHASE);        // 1,507,328
-constexpr int TC_CHUNKS_PER_TILE = 12 + 5 + 4 + 3 + 4 + 15;         // 43
-static_assert(TC_W_BYTES_PER_ELEM == 1507328, "packed weight image");
+constexpr int TC_W_BYTES_PER_ELEM = tc_phase_off(TC_NPHASE);        // 753,664
+static_assert(TC_W_BYTES_PER_ELEM == 753664, "packed weight image");
 
-struct TcSmem {                                   // after the 1024-aligned rings
-  uint64_t a_full[TC_NA], a_empty[TC_NA], b_full[TC_NB], b_empty[TC_NB];
-  uint64_t d_full, dg_free;
+// The overlapped block: 15 g-pass chunks of the previous tile and 12 first-GEMM chunks of the
+// current one, in the fixed order the MMA issuer and the weight stream both follow.  Entry =
+// kind << 8 | pass << 4 | chunk;  kind 0 = g pass (pass 0..2, chunk 0..4), kind 1 = first GEMM.
+// Pass 0 runs first (its operand is ready when the block starts, the AEV chunks are still in
+// flight); the first GEMM ends the block, so that the last drain overlaps its tail.
+constexpr int TC_BLOCK_OPS = 27;
+__host__ __device__ constexpr int tc_block_op(int i) {
+  constexpr int G = 0, A = 1 << 8;
+  const int t[TC_BLOCK_OPS] = {
+      G | 0x00, G | 0x01, G | 0x02, G | 0x03, G | 0x04,
+      A | 0, G | 0x10, A | 1, G | 0x11, A | 2, G | 0x12, A | 3, G | 0x13, A | 4, G | 0x14,
+      A | 5, G | 0x20, A | 6, G | 0x21, A | 7, G | 0x22, A | 8, G | 0x23, G | 0x24,
+      A | 9, A | 10, A | 11};
+  return t[i];
+}
+
+struct TcSmem {                                   // after the 1024-aligned operand regions
+  uint64_t a0_full[TC_NA], a_full[TC_NA], a_empty[TC_NA];   // ring A: first-GEMM chunks (128 producers) / chain chunks (256)
+  uint64_t b_full[TC_NB], b_empty[TC_NB];
+  uint64_t z_full[5];                             // accumulators z1, z2, z3, d2pre, d1pre complete
+  uint64_t g_full[2];                             // g buffer A / B complete
+  uint64_t g_free;                                // g buffer A drained (128 drain threads)
+  uint64_t d1_full[TC_ND1];                       // resident delta1 chunk written (256)
+  uint64_t d1_free;                               // every g-pass MMA of the tile has read the resident delta1
+  uint64_t dd_full;                               // the four delta2 chunks are written to the resident region (256)
+  uint64_t p5_done;                               // the delta1 producers have finished reading TMEM (256)
   uint32_t tmem_base;
   float epart[2][TC_TM];
 };
-constexpr size_t TC_SMEM_BYTES = 1024 + (size_t)TC_NA * TC_A_SLOT + (size_t)TC_NB * TC_B_SLOT + sizeof(TcSmem);
+constexpr size_t TC_SMEM_BYTES = 1024 + (size_t)TC_ND1 * TC_A_SLOT + (size_t)TC_NA * TC_A_SLOT +
+                                 (size_t)TC_NB * TC_B_SLOT + sizeof(TcSmem);
+static_assert(TC_SMEM_BYTES <= 227 * 1024, "shared memory budget");
+
+// per element: b1[160] b2[128] b3[96] w4[96] b4[1] pad[3] w4s[96] (w4 times the delta scale) kf[8]
+constexpr int TC_BIAS_B1 = 0, TC_BIAS_B2 = D1, TC_BIAS_B3 = D1 + D2, TC_BIAS_W4 = D1 + D2 + D3,
+              TC_BIAS_B4 = D1 + D2 + D3 + D3, TC_BIAS_W4S = 484, TC_BIAS_KF = 580, TC_BIAS_LEN = 588;
 
 struct TcParams {
-  const uint8_t* wpack;        // [NSPEC][TC_W_BYTES_PER_ELEM] packed hi|lo swizzled weight chunks
-  const float* bias[NSPEC];    // per element: b1[160] b2[128] b3[96] w4[96] b4[1]  (481 floats)
+  const uint8_t* wpack;        // [NSPEC][TC_W_BYTES_PER_ELEM] packed hi|lo swizzled weight chunks (scaled)
+  const float* bias[NSPEC];    // TC_BIAS_LEN floats per element; kf[q] = (1 + beta_q) 2^-(operand scales) of epilogue q
   int row_start[NSPEC + 1];
   int n_tiles;
-  float comp[6];               // expected relative truncation loss of the accumulator chain of phases 0..4 and the g passes
 };
-constexpr int TC_BIAS_B1 = 0, TC_BIAS_B2 = D1, TC_BIAS_B3 = D1 + D2, TC_BIAS_W4 = D1 + D2 + D3,
-              TC_BIAS_B4 = D1 + D2 + D3 + D3, TC_BIAS_LEN = 484;
 
-// x -> (hi, lo): hi = x rounded to tf32 precision (10 mantissa bits); lo = x - hi (exact in fp32)
-// rounded to tf32 as well -- the tensor core would otherwise TRUNCATE it, a one-sided 2^-21 error
-// that adds up linearly over K and over the atoms of a system; rounded, it is 2^-22 and unbiased.
-__device__ __forceinline__ float tf32_round(float x) {
-  return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
+// ---- kind::f16 descriptors ----------------------------------------------------------------------
+// Shared-memory matrix descriptor, K-major operand, SWIZZLE_64B: rows of 64 bytes (32 fp16),
+// 8-row groups 512 bytes apart (SBO), 16-byte unit u of row r stored at unit u ^ ((r >> 1) & 3).
+// [0,14) start>>4 | [16,30) LBO>>4 (=1, unused when swizzled) | [32,46) SBO>>4 |
+// [46,48) version = 1 | [61,64) layout: 4 = SWIZZLE_64B.
+__device__ __forceinline__ uint64_t tc_desc_sw64(uint32_t smem_addr) {
+  uint64_t d = (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)1 << 16;
+  d |= (uint64_t)(512 >> 4) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)4 << 61;
+  return d;
 }
-__device__ __forceinline__ void tf32_split(float x, float& hi, float& lo) {
-  hi = tf32_round(x);
-  lo = tf32_round(x - hi);
+// byte offset of fp16 element (row r, k in 0..31) inside a [rows x 32] SWIZZLE_64B tile
+__host__ __device__ constexpr uint32_t tc_sw64_off(uint32_t r, uint32_t k) {
+  return (r >> 3) * 512u + (r & 7u) * 64u + ((((k >> 3) ^ ((r >> 1) & 3u)) << 4) | ((k & 7u) << 1));
+}
+// Instruction descriptor, kind::f16, fp32 accumulate, fp16 A and B, both K-major, M x N tile:
+// [4,6) D fmt: 1 = f32 | [7,10) A fmt: 0 = f16 | [10,13) B fmt: 0 = f16 | [15] A major: 0 = K |
+// [16] B major: 0 = K | [17,23) N>>3 | [24,29) M>>4.
+__host__ __device__ constexpr uint32_t tc_idesc_f16(int M, int N) {
+  return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void tc_mma_f16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                           uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+
+// (x0, x1) -> packed (hi, lo): hi = fp16(x) to nearest, lo = fp16(x - hi) (x - hi is exact in fp32)
+__device__ __forceinline__ void tc_split2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+  const __half2 h = __floats2half2_rn(x0, x1);
+  const float2 f = __half22float2(h);
+  const __half2 l = __floats2half2_rn(x0 - f.x, x1 - f.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
 // CELU(x) and CELU'(x), alpha = 0.1:  e = exp(min(x,0)/alpha)
@@ -100,18 +175,17 @@ __device__ __forceinline__ void celu_both(float x, float& h, float& d) {
   d = x > 0.0f ? 1.0f : e;
 }
 
-// store 16 consecutive K values (columns 16*hf .. 16*hf+15 of a 32-wide chunk) of row r as hi|lo
+// store 16 consecutive K values (columns 16*hf .. 16*hf+15 of a 32-wide chunk) of row r as hi | lo
 __device__ __forceinline__ void tc_store_a16(uint8_t* slot, int r, int hf, const float (&v)[16]) {
+  uint32_t hi[8], lo[8];
 #pragma unroll
-  for (int jj = 0; jj < 4; ++jj) {
-    float4 hi, lo;
-    tf32_split(v[4 * jj + 0], hi.x, lo.x);
-    tf32_split(v[4 * jj + 1], hi.y, lo.y);
-    tf32_split(v[4 * jj + 2], hi.z, lo.z);
-    tf32_split(v[4 * jj + 3], hi.w, lo.w);
-    const uint32_t off = (uint32_t)r * 128u + ((uint32_t)((4 * hf + jj) ^ (r & 7)) << 4);
-    *reinterpret_cast<float4*>(slot + off) = hi;
-    *reinterpret_cast<float4*>(slot + TC_TM * 128 + off) = lo;
+  for (int j = 0; j < 8; ++j) tc_split2(v[2 * j], v[2 * j + 1], hi[j], lo[j]);
+  const uint32_t row = (uint32_t)(r >> 3) * 512u + (uint32_t)(r & 7) * 64u, sw = (uint32_t)(r >> 1) & 3u;
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+    const uint32_t off = row + ((((uint32_t)(2 * hf + u)) ^ sw) << 4);
+    *reinterpret_cast<uint4*>(slot + off) = make_uint4(hi[4 * u], hi[4 * u + 1], hi[4 * u + 2], hi[4 * u + 3]);
+    *reinterpret_cast<uint4*>(slot + TC_A_HALF + off) = make_uint4(lo[4 * u], lo[4 * u + 1], lo[4 * u + 2], lo[4 * u + 3]);
   }
 }
 
@@ -121,16 +195,24 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
                  float* __restrict__ e_row) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* base = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t* ringA = base;
+  uint8_t* resD1 = base;                                   // resident delta1 operand: 5 chunks
+  uint8_t* ringA = resD1 + TC_ND1 * TC_A_SLOT;
   uint8_t* ringB = ringA + TC_NA * TC_A_SLOT;
   TcSmem& S = *reinterpret_cast<TcSmem*>(ringB + TC_NB * TC_B_SLOT);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
 
   if (tid == 0) {
-    for (int i = 0; i < TC_NA; ++i) { tc::mbar_init(&S.a_full[i], TC_EPI_THREADS); tc::mbar_init(&S.a_empty[i], 1); }
+    for (int i = 0; i < TC_NA; ++i) {
+      tc::mbar_init(&S.a0_full[i], TC_WORKERS / 2); tc::mbar_init(&S.a_full[i], TC_WORKERS); tc::mbar_init(&S.a_empty[i], 1);
+    }
     for (int i = 0; i < TC_NB; ++i) { tc::mbar_init(&S.b_full[i], 1); tc::mbar_init(&S.b_empty[i], 1); }
-    tc::mbar_init(&S.d_full, 1);
-    tc::mbar_init(&S.dg_free, TC_EPI_THREADS);
+    for (int i = 0; i < 5; ++i) tc::mbar_init(&S.z_full[i], 1);
+    tc::mbar_init(&S.g_full[0], 1); tc::mbar_init(&S.g_full[1], 1);
+    tc::mbar_init(&S.g_free, TC_WORKERS / 2);
+    for (int i = 0; i < TC_ND1; ++i) tc::mbar_init(&S.d1_full[i], TC_WORKERS);
+    tc::mbar_init(&S.d1_free, 1);
+    tc::mbar_init(&S.dd_full, TC_WORKERS);
+    tc::mbar_init(&S.p5_done, TC_WORKERS);
     tc::mbar_fence_init();
   }
   if (warp == 9) tc::tmem_alloc<512>(&S.tmem_base);
@@ -138,278 +220,337 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tbase = S.tmem_base;
+  // tiles of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...; iteration `it` runs the overlapped block of
+  // (tile it-1, tile it) and then the chain of tile it; one extra iteration drains the last tile
+  const int n_my = (P.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  auto tile_of = [&](int it) { return (int)blockIdx.x + it * (int)gridDim.x; };
+  auto elem_of = [&](int tile) {
+    int el = 0;
+#pragma unroll
+    for (int k = 1; k < NSPEC; ++k) el += (tile * TC_TM >= P.row_start[k]);
+    return el;
+  };
 
   if (warp < 8) {
-    // =========================== producers / epilogue ===========================
+    // =========================== workers ===========================
     const int q = warp & 3, hf = warp >> 2;
     const int r = 32 * q + lane;                               // tile row == TMEM lane
     const uint32_t tlane = tbase + ((uint32_t)(32 * q) << 16);
-    uint32_t ia = 0, nd = 0, ndg = 0;                          // A chunks produced, d_full / dg_free phases seen
-    auto acquire = [&]() -> uint8_t* {                         // wait until slot ia%NA is free
+    uint32_t ia = 0;                                           // ring A chunks so far (all kinds)
+    auto acquire = [&]() -> uint8_t* {                         // wait until slot ia % NA is free
       const uint32_t s = ia % TC_NA, use = ia / TC_NA;
       tc::mbar_wait(&S.a_empty[s], (use & 1u) ^ 1u);
       return ringA + s * TC_A_SLOT;
     };
-    auto publish = [&]() {
+    auto publish = [&](uint64_t* bar) {
       tc::tc_fence_before();                                   // this thread's tcgen05.ld precede the MMAs that overwrite
       tc::fence_proxy_async_smem();
-      tc::mbar_arrive(&S.a_full[ia % TC_NA]);
-      ++ia;
+      tc::mbar_arrive(bar);
     };
-    auto wait_d = [&]() { tc::mbar_wait(&S.d_full, nd & 1u); ++nd; tc::tc_fence_after(); };
-
-    for (int tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
-      const int row0 = tile * TC_TM;
-      int el = 0;
+    for (int it = 0; it <= n_my; ++it) {
+      const bool have_prev = it >= 1, have_cur = it < n_my;
+      const uint32_t par = (uint32_t)it & 1u, par_prev = ((uint32_t)it + 1u) & 1u;
+      // ------------------------------ overlapped block ------------------------------
+      if (hf == 0) {
+        // drain g of the previous tile: pass 0 and 2 from buffer A, pass 1 from buffer B
+        if (have_prev) {
+          const int row0 = tile_of(it - 1) * TC_TM;
+          const float kg = __ldg(P.bias[elem_of(tile_of(it - 1))] + TC_BIAS_KF + 5);
+#pragma unroll 1
+          for (int pass = 0; pass < TC_NPASS; ++pass) {
+            const int buf = pass == 1 ? 1 : 0;
+            // completions of g_full[A]: two per tile (2(it-1), 2(it-1)+1); of g_full[B]: one per tile
+            tc::mbar_wait(&S.g_full[buf], buf ? par_prev : (uint32_t)(pass >> 1));
+            tc::tc_fence_after();
+            float* dst = g + (size_t)(row0 + r) * AEV_LEN + pass * TC_GN;
+            const uint32_t col = (uint32_t)(buf ? TC_COL_GB : TC_COL_GA);
 #pragma unroll
-      for (int k = 1; k < NSPEC; ++k) el += (row0 >= P.row_start[k]);
-      const float* bias = P.bias[el];
-
-      // ---- phase 0 operand: AEV rows, 12 chunks of 32 columns, split into hi|lo ----
-      {
-        const float4* src = reinterpret_cast<const float4*>(aev + (size_t)row0 * AEV_LEN);
-        float4 nxt[4];
+            for (int c = 0; c < TC_GN / 32; ++c) {
+              float v0[16], v1[16];
+              tc::tmem_ld16(tlane + col + 32 * c, v0);
+              tc::tmem_ld16(tlane + col + 32 * c + 16, v1);
+              tc::tmem_ld_wait();
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int f = tid + TC_EPI_THREADS * i;
-          nxt[i] = __ldg(src + (size_t)(f >> 3) * (AEV_LEN / 4) + (f & 7));
-        }
-        for (int c = 0; c < D0 / 32; ++c) {
-          float4 cur[4];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) cur[i] = nxt[i];
-          if (c + 1 < D0 / 32) {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              const int f = tid + TC_EPI_THREADS * i;
-              nxt[i] = __ldg(src + (size_t)(f >> 3) * (AEV_LEN / 4) + 8 * (c + 1) + (f & 7));
+              for (int k = 0; k < 4; ++k) {
+                reinterpret_cast<float4*>(dst + 32 * c)[k] =
+                    make_float4(kg * v0[4 * k], kg * v0[4 * k + 1], kg * v0[4 * k + 2], kg * v0[4 * k + 3]);
+                reinterpret_cast<float4*>(dst + 32 * c + 16)[k] =
+                    make_float4(kg * v1[4 * k], kg * v1[4 * k + 1], kg * v1[4 * k + 2], kg * v1[4 * k + 3]);
+              }
+            }
+            if (buf == 0) {
+              tc::tc_fence_before();
+              tc::mbar_arrive(&S.g_free);
             }
           }
-          uint8_t* slot = acquire();
+        }
+        if (have_cur) ia += D0 / TC_KC;                        // the twelve first-GEMM chunks are made by warps 4-7
+      } else if (have_cur) {
+        // first-GEMM operand of the current tile: AEV rows (times 8), 12 chunks of 32 columns -> hi | lo
+        const int ty = tid - TC_WORKERS / 2;                   // 0..127
+        const float4* src = reinterpret_cast<const float4*>(aev + (size_t)tile_of(it) * TC_TM * AEV_LEN);
+        // float4 f = ty + 128 i (i < 8) of a chunk: row f >> 3, 16-byte piece f & 7 of its 128 bytes
+        float4 buf0[8], buf1[8];
+        auto load = [&](float4 (&b)[8], int c) {
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int f = tid + TC_EPI_THREADS * i, rr = f >> 3, j = f & 7;
-            float4 hi, lo;
-            tf32_split(cur[i].x, hi.x, lo.x); tf32_split(cur[i].y, hi.y, lo.y);
-            tf32_split(cur[i].z, hi.z, lo.z); tf32_split(cur[i].w, hi.w, lo.w);
-            const uint32_t off = (uint32_t)rr * 128u + ((uint32_t)(j ^ (rr & 7)) << 4);
-            *reinterpret_cast<float4*>(slot + off) = hi;
-            *reinterpret_cast<float4*>(slot + TC_TM * 128 + off) = lo;
+          for (int i = 0; i < 8; ++i) {
+            const int f = ty + (TC_WORKERS / 2) * i;
+            b[i] = __ldg(src + (size_t)(f >> 3) * (AEV_LEN / 4) + 8 * c + (f & 7));
           }
-          publish();
+        };
+        auto convert = [&](const float4 (&b)[8], uint8_t* slot) {
+          constexpr float sc = (float)(1 << TC_AEV_SCALE_LOG2);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int f = ty + (TC_WORKERS / 2) * i, rr = f >> 3, j = f & 7;   // piece j: k = 4j .. 4j+3
+            uint32_t h0, l0, h1, l1;
+            tc_split2(sc * b[i].x, sc * b[i].y, h0, l0);
+            tc_split2(sc * b[i].z, sc * b[i].w, h1, l1);
+            const uint32_t off = tc_sw64_off((uint32_t)rr, (uint32_t)(4 * j));
+            *reinterpret_cast<uint2*>(slot + off) = make_uint2(h0, h1);
+            *reinterpret_cast<uint2*>(slot + TC_A_HALF + off) = make_uint2(l0, l1);
+          }
+        };
+        load(buf0, 0);
+        load(buf1, 1);
+#pragma unroll 1
+        for (int c = 0; c < D0 / TC_KC; c += 2) {
+          uint8_t* slot = acquire();
+          convert(buf0, slot);
+          if (c + 2 < D0 / TC_KC) load(buf0, c + 2);
+          tc::fence_proxy_async_smem();
+          tc::mbar_arrive(&S.a0_full[ia % TC_NA]);
+          ++ia;
+          slot = acquire();
+          convert(buf1, slot);
+          if (c + 3 < D0 / TC_KC) load(buf1, c + 3);
+          tc::fence_proxy_async_smem();
+          tc::mbar_arrive(&S.a0_full[ia % TC_NA]);
+          ++ia;
         }
       }
+      if (!have_cur) break;
+      // ------------------------------ chain of the current tile ------------------------------
+      const int row0 = tile_of(it) * TC_TM;
+      const float* bias = P.bias[elem_of(tile_of(it))];
+      const float k0 = __ldg(bias + TC_BIAS_KF + 0), k1 = __ldg(bias + TC_BIAS_KF + 1), k2 = __ldg(bias + TC_BIAS_KF + 2),
+                  k3 = __ldg(bias + TC_BIAS_KF + 3), k4 = __ldg(bias + TC_BIAS_KF + 4);
       // ---- z1 -> h1 = CELU(z1 + b1): operand of phase 1 ----
-      wait_d();
-      for (int c = 0; c < D1 / 32; ++c) {
+      tc::mbar_wait(&S.z_full[0], par);
+      tc::tc_fence_after();
+#pragma unroll 1
+      for (int c = 0; c < D1 / TC_KC; ++c) {
         float z[16], h[16], d;
-        tc::tmem_ld16(tlane + 0 + 32 * c + 16 * hf, z);
+        tc::tmem_ld16(tlane + TC_COL_Z1 + 32 * c + 16 * hf, z);
+        tc::tmem_ld_wait();
         const float* b = bias + TC_BIAS_B1 + 32 * c + 16 * hf;
-        if (N_TERMS == 3) {
-          float sm[16];
-          tc::tmem_ld16(tlane + TC_S0_COL + 32 * c + 16 * hf, sm);
-          tc::tmem_ld_wait();
 #pragma unroll
-          for (int k = 0; k < 16; ++k) { const float t = z[k] + sm[k]; z[k] = fmaf(t, P.comp[0], t) + __ldg(b + k); }
-        } else {
-          tc::tmem_ld_wait();
-#pragma unroll
-          for (int k = 0; k < 16; ++k) z[k] += __ldg(b + k);
-        }
-        tc::tmem_st16(tlane + 0 + 32 * c + 16 * hf, z);          // z1 + b1, kept for delta1
-#pragma unroll
-        for (int k = 0; k < 16; ++k) celu_both(z[k], h[k], d);
-        tc::tmem_st_wait();
+        for (int k = 0; k < 16; ++k) celu_both(fmaf(z[k], k0, __ldg(b + k)), h[k], d);
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
-        publish();
+        publish(&S.a_full[ia % TC_NA]);
+        ++ia;
       }
       // ---- z2 -> h2: operand of phase 2 ----
-      wait_d();
-      for (int c = 0; c < D2 / 32; ++c) {
+      tc::mbar_wait(&S.z_full[1], par);
+      tc::tc_fence_after();
+#pragma unroll 1
+      for (int c = 0; c < D2 / TC_KC; ++c) {
         float z[16], h[16], d;
-        tc::tmem_ld16(tlane + 160 + 32 * c + 16 * hf, z);
+        tc::tmem_ld16(tlane + TC_COL_Z2 + 32 * c + 16 * hf, z);
         tc::tmem_ld_wait();
         const float* b = bias + TC_BIAS_B2 + 32 * c + 16 * hf;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) celu_both(fmaf(z[k], P.comp[1], z[k]) + __ldg(b + k), h[k], d);
+        for (int k = 0; k < 16; ++k) celu_both(fmaf(z[k], k1, __ldg(b + k)), h[k], d);
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
-        publish();
+        publish(&S.a_full[ia % TC_NA]);
+        ++ia;
       }
-      // ---- z3 -> e_i = w4.h3 + b4 and delta3 = w4 * CELU'(z3 + b3): operand of phase 3 ----
-      wait_d();
+      // ---- z3 -> e_i = w4.h3 + b4 and delta3 = w4 * CELU'(z3 + b3) (scaled): operand of phase 3 ----
+      tc::mbar_wait(&S.z_full[2], par);
+      tc::tc_fence_after();
       {
         float epart = 0.0f;
-        for (int c = 0; c < D3 / 32; ++c) {
+#pragma unroll 1
+        for (int c = 0; c < D3 / TC_KC; ++c) {
           float z[16], dl[16];
-          tc::tmem_ld16(tlane + 288 + 32 * c + 16 * hf, z);
-          if (N_TERMS == 3) {
-            float sm[16];
-            tc::tmem_ld16(tlane + TC_S2_COL + 32 * c + 16 * hf, sm);
-            tc::tmem_ld_wait();
-#pragma unroll
-            for (int k = 0; k < 16; ++k) z[k] += sm[k];
-          } else {
-            tc::tmem_ld_wait();
-          }
+          tc::tmem_ld16(tlane + TC_COL_Z3 + 32 * c + 16 * hf, z);
+          tc::tmem_ld_wait();
           const float* b = bias + TC_BIAS_B3 + 32 * c + 16 * hf;
           const float* w4 = bias + TC_BIAS_W4 + 32 * c + 16 * hf;
+          const float* w4s = bias + TC_BIAS_W4S + 32 * c + 16 * hf;
 #pragma unroll
           for (int k = 0; k < 16; ++k) {
             float h, d;
-            const float w = __ldg(w4 + k);
-            celu_both(fmaf(z[k], P.comp[2], z[k]) + __ldg(b + k), h, d);
-            epart = fmaf(w, h, epart);
-            dl[k] = w * d;
+            celu_both(fmaf(z[k], k2, __ldg(b + k)), h, d);
+            epart = fmaf(__ldg(w4 + k), h, epart);
+            dl[k] = __ldg(w4s + k) * d;
           }
           uint8_t* slot = acquire();
           tc_store_a16(slot, r, hf, dl);
-          publish();
+          publish(&S.a_full[ia % TC_NA]);
+          ++ia;
         }
         S.epart[hf][r] = epart;
-        asm volatile("bar.sync 1, %0;" ::"n"(TC_EPI_THREADS) : "memory");
+        asm volatile("bar.sync 1, %0;" ::"n"(TC_WORKERS) : "memory");
         if (hf == 0) e_row[row0 + r] = (S.epart[0][r] + S.epart[1][r]) + __ldg(bias + TC_BIAS_B4);
       }
       // ---- delta2 = d2pre * CELU'(z2 + b2): operand of phase 4 ----
-      wait_d();
-      for (int c = 0; c < D2 / 32; ++c) {
+      // d1pre (phase 4's accumulator) overwrites z2 / z3, so phase 4 cannot start before ALL of delta2
+      // exists: its four chunks go to the resident region (free at this point: the previous tile's g
+      // passes are over), not through the three-slot ring, which could not hold them
+      tc::mbar_wait(&S.z_full[3], par);
+      tc::tc_fence_after();
+      if (have_prev) tc::mbar_wait(&S.d1_free, par_prev);      // the previous tile's g passes have read the region
+#pragma unroll 1
+      for (int c = 0; c < D2 / TC_KC; ++c) {
         float z[16], p[16];
-        tc::tmem_ld16(tlane + 160 + 32 * c + 16 * hf, z);
-        tc::tmem_ld16(tlane + 384 + 32 * c + 16 * hf, p);
+        tc::tmem_ld16(tlane + TC_COL_Z2 + 32 * c + 16 * hf, z);
+        tc::tmem_ld16(tlane + TC_COL_D2 + 32 * c + 16 * hf, p);
         tc::tmem_ld_wait();
         const float* b = bias + TC_BIAS_B2 + 32 * c + 16 * hf;
 #pragma unroll
         for (int k = 0; k < 16; ++k) {
           float h, d;
-          celu_both(fmaf(z[k], P.comp[1], z[k]) + __ldg(b + k), h, d);
-          p[k] = fmaf(p[k], P.comp[3], p[k]) * d;
+          celu_both(fmaf(z[k], k1, __ldg(b + k)), h, d);
+          p[k] = (p[k] * k3) * d;
         }
-        uint8_t* slot = acquire();
-        tc_store_a16(slot, r, hf, p);
-        publish();
+        tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
       }
-      // ---- delta1 = d1pre * CELU'(z1 + b1): operand of the three g passes; drain g ----
-      wait_d();
-      for (int pass = 0; pass < D0 / TC_GN; ++pass) {
-        for (int c = 0; c < D1 / 32; ++c) {
-          float z[16], p[16];
-          tc::tmem_ld16(tlane + 0 + 32 * c + 16 * hf, z);
-          tc::tmem_ld16(tlane + 160 + 32 * c + 16 * hf, p);
-          tc::tmem_ld_wait();
+      publish(&S.dd_full);
+      // ---- delta1 = d1pre * CELU'(z1 + b1): RESIDENT operand of the three g passes ----
+      tc::mbar_wait(&S.z_full[4], par);                        // (phase 4 has consumed delta2: the region is free again)
+      tc::tc_fence_after();
+#pragma unroll 1
+      for (int c = 0; c < TC_ND1; ++c) {
+        float z[16], p[16];
+        tc::tmem_ld16(tlane + TC_COL_Z1 + 32 * c + 16 * hf, z);
+        tc::tmem_ld16(tlane + TC_COL_D1 + 32 * c + 16 * hf, p);
+        tc::tmem_ld_wait();
+        const float* b = bias + TC_BIAS_B1 + 32 * c + 16 * hf;
 #pragma unroll
-          for (int k = 0; k < 16; ++k) {
-            float h, d;
-            celu_both(z[k], h, d);                             // z1 already holds the bias
-            p[k] = fmaf(p[k], P.comp[4], p[k]) * d;
-          }
-          uint8_t* slot = acquire();
-          tc_store_a16(slot, r, hf, p);
-          publish();
+        for (int k = 0; k < 16; ++k) {
+          float h, d;
+          celu_both(fmaf(z[k], k0, __ldg(b + k)), h, d);
+          p[k] = (p[k] * k4) * d;
         }
-        wait_d();
-        float* dst = g + (size_t)(row0 + r) * AEV_LEN + pass * TC_GN + 16 * hf;
-#pragma unroll
-        for (int c = 0; c < TC_GN / 32; c += 2) {
-          float v0[16], v1[16];
-          tc::tmem_ld16(tlane + 384 + 32 * c + 16 * hf, v0);
-          tc::tmem_ld16(tlane + 384 + 32 * (c + 1) + 16 * hf, v1);
-          tc::tmem_ld_wait();
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const float cg = P.comp[5];
-            reinterpret_cast<float4*>(dst + 32 * c)[k] =
-                make_float4(fmaf(cg, v0[4 * k], v0[4 * k]), fmaf(cg, v0[4 * k + 1], v0[4 * k + 1]),
-                            fmaf(cg, v0[4 * k + 2], v0[4 * k + 2]), fmaf(cg, v0[4 * k + 3], v0[4 * k + 3]));
-            reinterpret_cast<float4*>(dst + 32 * (c + 1))[k] =
-                make_float4(fmaf(cg, v1[4 * k], v1[4 * k]), fmaf(cg, v1[4 * k + 1], v1[4 * k + 1]),
-                            fmaf(cg, v1[4 * k + 2], v1[4 * k + 2]), fmaf(cg, v1[4 * k + 3], v1[4 * k + 3]));
-          }
-        }
-        tc::tc_fence_before();
-        tc::mbar_arrive(&S.dg_free);
-        ++ndg;
+        tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
+        publish(&S.d1_full[c]);
       }
+      tc::tc_fence_before();
+      tc::mbar_arrive(&S.p5_done);
     }
   } else if (warp == 8) {
     // =========================== TMA: weight chunks ===========================
     if (lane == 0) {
       uint32_t ib = 0;
-      for (int tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
-        const int row0 = tile * TC_TM;
-        int el = 0;
-#pragma unroll
-        for (int k = 1; k < NSPEC; ++k) el += (row0 >= P.row_start[k]);
-        const uint8_t* src = P.wpack + (size_t)el * TC_W_BYTES_PER_ELEM;
+      auto stream = [&](const uint8_t* src, uint32_t bytes) {
+        const uint32_t s = ib % TC_NB, use = ib / TC_NB;
+        tc::mbar_wait(&S.b_empty[s], (use & 1u) ^ 1u);
+        tc::mbar_arrive_expect_tx(&S.b_full[s], bytes);
+        tc::bulk_g2s(ringB + s * TC_B_SLOT, src, bytes, &S.b_full[s]);
+        ++ib;
+      };
+      for (int it = 0; it <= n_my; ++it) {
+        const bool have_prev = it >= 1, have_cur = it < n_my;
+        const uint8_t* wprev = have_prev ? P.wpack + (size_t)elem_of(tile_of(it - 1)) * TC_W_BYTES_PER_ELEM : nullptr;
+        const uint8_t* wcur = have_cur ? P.wpack + (size_t)elem_of(tile_of(it)) * TC_W_BYTES_PER_ELEM : nullptr;
 #pragma unroll 1
-        for (int p = 0; p < TC_NPHASE; ++p) {
-          const uint32_t bytes = (uint32_t)tc_chunk_bytes(p);
-          const int nk = tc_phase_nk(p);
-          for (int c = 0; c < nk; ++c) {
-            const uint32_t s = ib % TC_NB, use = ib / TC_NB;
-            tc::mbar_wait(&S.b_empty[s], (use & 1u) ^ 1u);
-            tc::mbar_arrive_expect_tx(&S.b_full[s], bytes);
-            tc::bulk_g2s(ringB + s * TC_B_SLOT, src, bytes, &S.b_full[s]);
-            src += bytes;
-            ++ib;
+        for (int i = 0; i < TC_BLOCK_OPS; ++i) {
+          const int op = tc_block_op(i);
+          if (op >> 8) {
+            if (have_cur) stream(wcur + tc_phase_off(0) + (size_t)(op & 15) * tc_chunk_bytes(0), (uint32_t)tc_chunk_bytes(0));
+          } else if (have_prev) {
+            stream(wprev + tc_phase_off(5 + ((op >> 4) & 3)) + (size_t)(op & 15) * tc_chunk_bytes(5), (uint32_t)tc_chunk_bytes(5));
           }
+        }
+        if (!have_cur) break;
+#pragma unroll 1
+        for (int p = 1; p <= 4; ++p) {
+          const uint8_t* src = wcur + tc_phase_off(p);
+          const uint32_t bytes = (uint32_t)tc_chunk_bytes(p);
+          for (int c = 0; c < tc_phase_nk(p); ++c) stream(src + (size_t)c * bytes, bytes);
         }
       }
     }
   } else {
     // =========================== MMA issuer ===========================
     if (lane == 0) {
-      uint32_t ia = 0, ib = 0, ndg = 0;
-      for (int tile = blockIdx.x; tile < P.n_tiles; tile += gridDim.x) {
-#pragma unroll 1
-        for (int p = 0; p < TC_NPHASE; ++p) {
-          const int N = tc_phase_n(p), nk = tc_phase_nk(p);
-          const uint32_t dcol = tbase + (uint32_t)tc_phase_dcol(p);
-          const uint32_t idesc = tc::idesc_tf32(TC_TM, N);
-          const bool split_acc = N_TERMS == 3 && (p == 0 || p == 2);
-          const uint32_t scol = tbase + (uint32_t)(p == 0 ? TC_S0_COL : TC_S2_COL);
-          if (p == 3 || p == 4) {
-            // p4: d1pre overwrites z2 / z3 / d2pre: every delta2 chunk must exist first (the last
-            // chunk's barrier completes after the earlier ones: producers arrive in order);
-            // p3: d2pre overwrites S2, which the delta3 producers still read
-            const uint32_t il = ia + (uint32_t)nk - 1;
-            tc::mbar_wait(&S.a_full[il % TC_NA], (il / TC_NA) & 1u);
-          }
-          if (p >= 6) {                                   // g pass buffer drained by the epilogue
-            tc::mbar_wait(&S.dg_free, ndg & 1u);
-            ++ndg;
-          }
-          for (int c = 0; c < nk; ++c) {
-            const uint32_t sa = ia % TC_NA, sb = ib % TC_NB;
-            tc::mbar_wait(&S.a_full[sa], (ia / TC_NA) & 1u);
-            tc::mbar_wait(&S.b_full[sb], (ib / TC_NB) & 1u);
-            tc::tc_fence_after();
-            const uint32_t a_hi = tc::smem_u32(ringA + sa * TC_A_SLOT), a_lo = a_hi + TC_TM * 128;
-            const uint32_t b_hi = tc::smem_u32(ringB + sb * TC_B_SLOT), b_lo = b_hi + (uint32_t)N * 128;
+      uint32_t ia = 0, ib = 0;
+      uint32_t par_a0 = 0, par_a1 = 0;                         // per-slot phase parities of a0_full / a_full
+      // one 32-k chunk: 2 k steps x N_TERMS MMAs of M 128 x N into TMEM column dcol; A from `a_slot`, B from ring slot
+      auto issue = [&](uint32_t dcol, uint32_t a_slot, int N, bool first) {
+        const uint32_t sb = ib % TC_NB;
+        tc::mbar_wait(&S.b_full[sb], (ib / TC_NB) & 1u);
+        tc::tc_fence_after();
+        const uint32_t a_hi = a_slot, a_lo = a_slot + TC_A_HALF;
+        const uint32_t b_hi = tc::smem_u32(ringB + sb * TC_B_SLOT), b_lo = b_hi + (uint32_t)N * 64u;
+        const uint32_t idesc = tc_idesc_f16(TC_TM, N);
 #pragma unroll
-            for (int ks = 0; ks < 4; ++ks) {
-              const uint64_t dah = tc::smem_desc_sw128(a_hi + 32 * ks), dal = tc::smem_desc_sw128(a_lo + 32 * ks);
-              const uint64_t dbh = tc::smem_desc_sw128(b_hi + 32 * ks), dbl = tc::smem_desc_sw128(b_lo + 32 * ks);
-              if (split_acc) {
-                tc::mma_tf32_ss(scol, dal, dbh, idesc, (c | ks) ? 1u : 0u);
-                tc::mma_tf32_ss(scol, dah, dbl, idesc, 1u);
-                tc::mma_tf32_ss(dcol, dah, dbh, idesc, (c | ks) ? 1u : 0u);
-              } else if (N_TERMS == 3) {
-                tc::mma_tf32_ss(dcol, dal, dbh, idesc, (c | ks) ? 1u : 0u);
-                tc::mma_tf32_ss(dcol, dah, dbl, idesc, 1u);
-                tc::mma_tf32_ss(dcol, dah, dbh, idesc, 1u);
-              } else {
-                tc::mma_tf32_ss(dcol, dah, dbh, idesc, (c | ks) ? 1u : 0u);
-              }
-            }
-            tc::mma_commit(&S.a_empty[sa]);
-            tc::mma_commit(&S.b_empty[sb]);
-            ++ia; ++ib;
+        for (int ks = 0; ks < 2; ++ks) {
+          const uint64_t dah = tc_desc_sw64(a_hi + 32 * ks), dal = tc_desc_sw64(a_lo + 32 * ks);
+          const uint64_t dbh = tc_desc_sw64(b_hi + 32 * ks), dbl = tc_desc_sw64(b_lo + 32 * ks);
+          if (N_TERMS == 3) {
+            tc_mma_f16(dcol, dal, dbh, idesc, (first && ks == 0) ? 0u : 1u);
+            tc_mma_f16(dcol, dah, dbl, idesc, 1u);
+            tc_mma_f16(dcol, dah, dbh, idesc, 1u);
+          } else {
+            tc_mma_f16(dcol, dah, dbh, idesc, (first && ks == 0) ? 0u : 1u);
           }
-          tc::mma_commit(&S.d_full);
         }
-        ++ndg;                                            // the last pass's drain: consumed below
-        tc::mbar_wait(&S.dg_free, (ndg - 1) & 1u);        // keep dg_free phases aligned per tile
+        tc::mma_commit(&S.b_empty[sb]);
+        ++ib;
+      };
+      // a chunk whose A operand comes through ring A (kind 0: first GEMM, 128 producers; kind 1: chain, 256)
+      auto issue_ring = [&](uint32_t dcol, int N, bool first, int kind) {
+        const uint32_t sa = ia % TC_NA;
+        if (kind == 0) { tc::mbar_wait(&S.a0_full[sa], (par_a0 >> sa) & 1u); par_a0 ^= 1u << sa; }
+        else           { tc::mbar_wait(&S.a_full[sa], (par_a1 >> sa) & 1u); par_a1 ^= 1u << sa; }
+        issue(dcol, tc::smem_u32(ringA + sa * TC_A_SLOT), N, first);
+        tc::mma_commit(&S.a_empty[sa]);
+        ++ia;
+      };
+      for (int it = 0; it <= n_my; ++it) {
+        const bool have_prev = it >= 1, have_cur = it < n_my;
+        const uint32_t par_prev = ((uint32_t)it + 1u) & 1u;
+        // ------------------------------ overlapped block ------------------------------
+        bool p5_waited = !have_prev;
+#pragma unroll 1
+        for (int i = 0; i < TC_BLOCK_OPS; ++i) {
+          const int op = tc_block_op(i), c = op & 15;
+          if (op >> 8) {                                       // first GEMM of the current tile -> z1
+            if (!have_cur) continue;
+            if (!p5_waited) { tc::mbar_wait(&S.p5_done, par_prev); p5_waited = true; }   // z1 / d1pre of the previous tile were read
+            issue_ring(tbase + TC_COL_Z1, D1, c == 0, 0);
+            if (c == D0 / TC_KC - 1) tc::mma_commit(&S.z_full[0]);
+          } else {                                             // g pass of the previous tile
+            if (!have_prev) continue;
+            const int pass = (op >> 4) & 3;
+            if (c == 0) {
+              if (pass == 1 && !p5_waited) { tc::mbar_wait(&S.p5_done, par_prev); p5_waited = true; }   // buffer B = d1pre's columns
+              if (pass == 2) tc::mbar_wait(&S.g_free, 0u);     // buffer A drained of pass 0 (completion 2(it-1))
+            }
+            if (pass == 0) tc::mbar_wait(&S.d1_full[c], par_prev);
+            issue(tbase + (uint32_t)(pass == 1 ? TC_COL_GB : TC_COL_GA), tc::smem_u32(resD1 + c * TC_A_SLOT), TC_GN, c == 0);
+            if (c == TC_ND1 - 1) {
+              tc::mma_commit(&S.g_full[pass == 1 ? 1 : 0]);
+              if (pass == TC_NPASS - 1) tc::mma_commit(&S.d1_free);
+            }
+          }
+        }
+        if (!have_cur) break;
+        // ------------------------------ chain ------------------------------
+        for (int c = 0; c < tc_phase_nk(1); ++c) issue_ring(tbase + TC_COL_Z2, tc_phase_n(1), c == 0, 1);
+        tc::mma_commit(&S.z_full[1]);
+        for (int c = 0; c < tc_phase_nk(2); ++c) issue_ring(tbase + TC_COL_Z3, tc_phase_n(2), c == 0, 1);
+        tc::mma_commit(&S.z_full[2]);
+        for (int c = 0; c < tc_phase_nk(3); ++c) issue_ring(tbase + TC_COL_D2, tc_phase_n(3), c == 0, 1);
+        tc::mma_commit(&S.z_full[3]);
+        tc::mbar_wait(&S.dd_full, (uint32_t)it & 1u);            // all of delta2 is in the resident region
+        for (int c = 0; c < tc_phase_nk(4); ++c)
+          issue(tbase + TC_COL_D1, tc::smem_u32(resD1 + c * TC_A_SLOT), tc_phase_n(4), c == 0);
+        tc::mma_commit(&S.z_full[4]);
       }
     }
   }

@@ -8,6 +8,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <cmath>
 #include <new>
 #include <vector>
 
@@ -129,6 +130,8 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
 }
 
 inline int cells_for(int n_sys_atoms) { return n_sys_atoms + 64 + 1; }
+// default scale of the tensor-core MLP's truncation compensation, forward / backward phases
+constexpr float TC_LAMBDA_FWD = 1.0f, TC_LAMBDA_BWD = 1.0f;
 constexpr int ROW_CAP = 192;                  // neighbour-row capacity of an atom: min(ROW_CAP, N_sys - 1); bulk at 0.1 / A^3 has 59
 constexpr int K1_MIN_BLOCK = 8, K1_MAX_BLOCK = 64;   // atoms per K1 brute-force work item
 
@@ -450,22 +453,33 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   for (int e = 0; e <= NSPEC; ++e) c->mlp.row_start[e] = row_start[e];
 
   // tensor-core path: per element, the B operand of every phase chunk exactly as it sits in
-  // shared memory -- [N rows x 32 k] fp32, K-major, SWIZZLE_128B, hi block then lo block
+  // shared memory -- [N rows x 32 k] fp16, K-major, SWIZZLE_64B, hi block then lo block -- with every
+  // weight matrix scaled by the power of two that puts max|W| into [256, 512) (k3_mlp_tc.cuh)
   std::vector<uint8_t> wtc((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
   std::vector<float> bias_tc((size_t)NSPEC * TC_BIAS_LEN, 0.0f);
+  const int n_terms = c->mlp_path == PFC_MLP_TF32X1 ? 1 : 3;
   for (int e = 0; e < NSPEC; ++e) {
     const float* src = d->weights + (size_t)e * W_PER_ELEM;
     const float *W1 = src, *b1 = W1 + D1 * D0, *W2 = b1 + D1, *b2 = W2 + D2 * D1, *W3 = b2 + D2,
                 *b3 = W3 + D3 * D2, *W4 = b3 + D3, *b4 = W4 + D3;
+    auto scale_log2 = [](const float* w, int n, float target) {   // e with max|w| 2^e in [target/2, target)
+      float m = 0.0f;
+      for (int i = 0; i < n; ++i) m = fmaxf(m, fabsf(w[i]));
+      if (!(m > 0.0f) || !std::isfinite(m)) return 0;
+      int ex = (int)floorf(log2f(target / m));
+      return ex < -12 ? -12 : ex > 24 ? 24 : ex;
+    };
+    const int eW1 = scale_log2(W1, D1 * D0, 512.0f), eW2 = scale_log2(W2, D2 * D1, 512.0f),
+              eW3 = scale_log2(W3, D3 * D2, 512.0f), eD = scale_log2(W4, D3, 16.0f);
     // B[n][k] of phase p (see k3_mlp_tc.cuh): forward W[n][k]; backward W[k][n]
     auto bval = [&](int p, int n, int k) -> float {
       switch (p) {
-        case 0: return W1[n * D0 + k];
-        case 1: return W2[n * D1 + k];
-        case 2: return W3[n * D2 + k];
-        case 3: return W3[k * D2 + n];
-        case 4: return W2[k * D1 + n];
-        default: return W1[k * D0 + (p - 5) * TC_GN + n];
+        case 0: return ldexpf(W1[n * D0 + k], eW1);
+        case 1: return ldexpf(W2[n * D1 + k], eW2);
+        case 2: return ldexpf(W3[n * D2 + k], eW3);
+        case 3: return ldexpf(W3[k * D2 + n], eW3);
+        case 4: return ldexpf(W2[k * D1 + n], eW2);
+        default: return ldexpf(W1[k * D0 + (p - 5) * TC_GN + n], eW1);
       }
     };
     uint8_t* img = wtc.data() + (size_t)e * TC_W_BYTES_PER_ELEM;
@@ -474,19 +488,12 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
       for (int ch = 0; ch < nk; ++ch) {
         uint8_t* chunk = img + tc_phase_off(p) + (size_t)ch * tc_chunk_bytes(p);
         for (int n = 0; n < N; ++n)
-          for (int kk = 0; kk < 32; ++kk) {
-            const float v = bval(p, n, 32 * ch + kk);
-            uint32_t u;
-            memcpy(&u, &v, 4);
-            u = (u + 0x1000u) & 0xFFFFE000u;               // hi: rounded to tf32 precision
-            float hi;
-            memcpy(&hi, &u, 4);
-            float lo = v - hi;                              // exact; then rounded to tf32 like hi
-            memcpy(&u, &lo, 4);
-            u = (u + 0x1000u) & 0xFFFFE000u;
-            memcpy(&lo, &u, 4);
-            memcpy(chunk + tc::sw128_off(n, kk), &hi, 4);
-            memcpy(chunk + (size_t)N * 128 + tc::sw128_off(n, kk), &lo, 4);
+          for (int kk = 0; kk < TC_KC; ++kk) {
+            const float v = bval(p, n, TC_KC * ch + kk);
+            const __half hi = __float2half_rn(v);                       // hi: fp16 to nearest
+            const __half lo = __float2half_rn(v - __half2float(hi));    // lo: the (exact) remainder, fp16 to nearest
+            memcpy(chunk + tc_sw64_off(n, kk), &hi, 2);
+            memcpy(chunk + (size_t)N * 64 + tc_sw64_off(n, kk), &lo, 2);
           }
       }
     }
@@ -496,19 +503,21 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
     memcpy(bt + TC_BIAS_B3, b3, sizeof(float) * D3);
     memcpy(bt + TC_BIAS_W4, W4, sizeof(float) * D3);
     bt[TC_BIAS_B4] = b4[0];
+    for (int k = 0; k < D3; ++k) bt[TC_BIAS_W4S + k] = ldexpf(W4[k], eD);
+    // epilogue factors: (1 + beta_q) times the inverse operand scales; beta_q = lambda n_q 2.15e-8 is the
+    // expected relative truncation loss of a chain of n_q MMA instructions (pfc_tuning_t.tc_comp_* scale it)
+    const float lf = tun.tc_comp_override ? tun.tc_comp_forward : TC_LAMBDA_FWD;
+    const float lb = tun.tc_comp_override ? tun.tc_comp_backward : TC_LAMBDA_BWD;
+    const int inv_scale[6] = {-(TC_AEV_SCALE_LOG2 + eW1), -eW2, -eW3, -eW3, -eW2, -(eW1 + eD)};
+    for (int q = 0; q < 6; ++q) {
+      const float beta = (q < 3 ? lf : lb) * (float)tc_chain_mmas(q, n_terms) * 2.15e-8f;
+      bt[TC_BIAS_KF + q] = ldexpf(1.0f + beta, inv_scale[q]);
+    }
     c->tcp.bias[e] = c->b.bias_tc + (size_t)e * TC_BIAS_LEN;
   }
   c->tcp.wpack = c->b.wtc;
   for (int e = 0; e <= NSPEC; ++e) c->tcp.row_start[e] = row_start[e];
   c->tcp.n_tiles = c->sz.n_rows / TC_TM;
-  {
-    // truncation steps of the main accumulator chain per phase (K/8, x3 where the three split terms
-    // share one accumulator); pfc_tuning_t.tc_comp_* scale the forward / backward compensation
-    const int ntr[6] = {48, 60, 16, 36, 48, 60};
-    const float lf = tun.tc_comp_override ? tun.tc_comp_forward : 0.9f;
-    const float lb = tun.tc_comp_override ? tun.tc_comp_backward : 0.73f;
-    for (int q = 0; q < 6; ++q) c->tcp.comp[q] = (q < 3 ? lf : lb) * (float)ntr[q] * 2.15e-8f;
-  }
 
   StepParams sp0{};
   {
