@@ -328,14 +328,14 @@ def run_pfc(args):
         # the burst bf16 peak when the clock record shows the run was never power-capped, else the sustained one
         capped = bool(clocks and "sw_power_cap" in (clocks.get("reasons") or []))
         bf16 = peaks["bf16_tflops_sustained"] if capped else peaks["bf16_tflops"]
-        tensor_peak = 0.5 * bf16
+        tensor_peak = bf16                                       # kind::f16 operands: the bf16 / fp16 dense rate
         if mlp == pfc.MLP_FP32:
             roof = {"bound": "alu", "achieved": flops / k3_s / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "peak_source": "148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz (guide unit counts and max SM clock)"}
         else:
             roof = {"bound": "tensor", "achieved": flops / k3_s / 1e12, "peak": tensor_peak, "unit": "TFLOP/s",
                     "peak_source": f"{peak_src} bf16 {'sustained (sw_power_cap seen)' if capped else 'burst (no power cap seen)'} "
-                                   "x 0.5 (tf32:bf16 nominal ratio); achieved counts algorithmic flops once, the "
+                                   "(kind::f16 runs at the bf16 rate); achieved counts algorithmic flops once, the "
                                    "3-term split issues 3x"}
         k3_name = "K3_fp32" if mlp == pfc.MLP_FP32 else "K3_tc"
         traffic, traffic_src = _traffic(k3_name, args.config)
@@ -394,11 +394,11 @@ def run_pfc(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32" if mlp == 0 else "tf32x3",    # MLP contractions as a 3-term tf32 split, fp32 accumulate; all else f32
+            "dtype": "f32" if mlp == 0 else "f16x3",     # MLP contractions as a 3-term fp16 hi|lo split, fp32 accumulate; all else f32
             "data": "synthetic",
             "config": _config_dict(args, wl),
-            "path": {"mlp_path": "fp32_ffma" if mlp == 0 else "tf32x3_tcgen05",
-                     "mlp_path_requested": {0: "fp32", 1: "tf32x3", 2: "tf32x1", 3: "auto"}[args.mlp],
+            "path": {"mlp_path": "fp32_ffma" if mlp == 0 else "f16x3_tcgen05",
+                     "mlp_path_requested": {0: "fp32", 1: "tensor", 2: "tensor_1term", 3: "auto"}[args.mlp],
                      "steps_per_graph": p.steps_per_graph()},
             "ns_per_day_per_replica": steps_per_s * DT_FS * 1e-6 * 86400,
             "ns_per_day_aggregate": steps_per_s * DT_FS * 1e-6 * 86400 * wl.n_systems * world,
@@ -444,7 +444,7 @@ def main():
     ap.add_argument("--integrator", default="verlet", choices=["verlet", "langevin"],
                     help="langevin = the paper's timing protocol (friction 0.1 ps^-1, 10 frames), PAPER.md:94")
     ap.add_argument("--mlp", type=int, default=3, choices=[0, 1, 3],
-                    help="3 = auto (library default: tensor-core MLP from 4096 atoms on), 0 = FP32 FFMA, 1 = tcgen05 TF32x3")
+                    help="3 = auto (library default: tensor-core MLP from 4096 atoms on), 0 = FP32 FFMA, 1 = tcgen05 fp16 split")
     ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (100 steps each)")
     args = ap.parse_args()
     INTEGRATOR["kind"] = args.integrator

@@ -67,9 +67,9 @@ extern "C" {
 #define PFC_MAX_ANGULAR 96              /* angular neighbours one atom may have  */
 
 #define PFC_MLP_FP32 0                  /* FP32 FFMA grouped MLP                 */
-#define PFC_MLP_TF32X3 1                /* tcgen05 kind::tf32, 3-term split      */
-#define PFC_MLP_TF32X1 2                /* tcgen05 plain TF32: tolerance evidence only (fails it) */
-#define PFC_MLP_AUTO 3                  /* TF32X3 for batches of >= 4096 atoms, FP32 below */
+#define PFC_MLP_TENSOR 1                /* tcgen05 kind::f16, fp16 hi|lo 3-term split, fp32 accumulate */
+#define PFC_MLP_TENSOR_1TERM 2          /* tcgen05 plain fp16 operands: tolerance evidence only (fails it) */
+#define PFC_MLP_AUTO 3                  /* TENSOR for batches of >= 4096 atoms, FP32 below */
 
 /* Optional tuning knobs, passed explicitly through pfc_desc_t.tuning (HOST pointer, NULL = all
  * defaults; a zero-filled struct is also "all defaults").  The library reads no environment
@@ -102,7 +102,7 @@ typedef struct {
   const float *masses_amu;       /* HOST [4] or NULL -> {1.008,12.011,14.007,15.999} */
   void *workspace;               /* DEVICE, 256-byte aligned, >= pfc_workspace_bytes() */
   size_t workspace_bytes;
-  int32_t mlp_path;              /* PFC_MLP_AUTO (recommended), PFC_MLP_FP32, PFC_MLP_TF32X3 (or PFC_MLP_TF32X1) */
+  int32_t mlp_path;              /* PFC_MLP_AUTO (recommended), PFC_MLP_FP32, PFC_MLP_TENSOR (or PFC_MLP_TENSOR_1TERM) */
   const pfc_tuning_t *tuning;    /* HOST or NULL (defaults)                         */
 } pfc_desc_t;
 
@@ -192,7 +192,9 @@ int pfc_run_host_resume(pfc_t *ctx, float *pos_host, float *vel_host, float *F_h
 int pfc_get_neighbors(pfc_t *ctx, const int32_t **r_off, const int32_t **r_idx,
                       const int32_t **a_off, const int32_t **a_idx);
 /* aev, g: [n_rows][384] in element-sorted padded row order; row_of_atom
- * DEVICE [n_atoms] gives each atom's row. */
+ * DEVICE [n_atoms] gives each atom's row.  (On the tensor-core MLP path K2 writes the AEV as the
+ * MLP's packed fp16 hi|lo operand image; the call then enqueues its unpacking into fp32 rows on the
+ * handle's stream: synchronise before reading.) */
 int pfc_get_intermediates(pfc_t *ctx, const float **aev, const float **g,
                           const int32_t **row_of_atom, int32_t *n_rows);
 

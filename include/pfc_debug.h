@@ -23,6 +23,12 @@ int pfc_profile_stages(pfc_t *ctx, const float *pos, float *E, float *F, void *s
  * neighbours), brute-force distance tests per evaluation}.  Synchronises the handle's stream. */
 int pfc_work_counts(pfc_t *ctx, int64_t *counts);
 
+/* Timeline of the tensor-core MLP kernel (one relaunch of K3 on the AEV rows of the last evaluation; the
+ * outputs it rewrites are unchanged): SM clock values recorded by the first CTA at the scheduling events of
+ * its first 8 tile iterations, 128 slots per iteration (slot meaning: TC_TRACE comment in csrc/k3_mlp_tc.cuh);
+ * 0 = event not reached.  cycles HOST [n], n <= 1024.  PFC_ERR_STATE on the FP32 path.  Synchronises. */
+int pfc_k3_timeline(pfc_t *ctx, int64_t *cycles, int32_t n);
+
 /* Parity helper: synchronous cudaMemcpy of `bytes` from a DEVICE pointer returned by the
  * getters of pfc.h into HOST memory. */
 int pfc_copy_to_host(const void *device_src, void *host_dst, size_t bytes);

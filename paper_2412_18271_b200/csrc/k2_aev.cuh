@@ -23,8 +23,15 @@
 //             results are bit-reproducible.
 // theta is never formed: cos(theta - theta_b) = c cos(theta_b) + sqrt(1-c^2) sin(theta_b)
 // with c = 0.95 cos(phi); the power 32 is five squarings.
-// Rows are written in element-sorted padded order (row_of_atom) so K3's tiles are contiguous.
+// Rows are written in element-sorted padded order (row_of_atom) so K3's tiles are contiguous --
+// as fp32 rows aev[row][384] for the FP32 MLP, or (PACK16) directly as the A operand image of the
+// tensor-core MLP's first GEMM: per 128-row tile and 32-column chunk one 16 KB block, the values
+// times 8 split into fp16 hi | lo, K-major SWIZZLE_64B (k3_mlp_tc.cuh) -- the AEV -> MLP fusion of
+// SURVEY.md 8(f) item 4 on the operand side: K3 brings a chunk in with one bulk copy and no warp
+// touches it again.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "aev_common.cuh"
 
 namespace pfc {
@@ -42,6 +49,10 @@ struct AevFwdSmem {
   int pre4[NPAIR + 1];           // first 4-slot group of each species-pair block
 };
 
+constexpr int K2_PACK_CHUNK_BYTES = 2 * 128 * 64;     // == TC_A_SLOT: hi block then lo block of one [128 x 32] chunk
+constexpr float K2_PACK_SCALE = 8.0f;                // == 2^TC_AEV_SCALE_LOG2
+
+template <bool PACK16>
 __global__ void __launch_bounds__(AEV_WARPS * 32, 8)
 k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __restrict__ xsl,
                   const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr, const int2* __restrict__ cnt,
@@ -56,7 +67,27 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __re
   const float4 xi = xs[i], li = xsl[i];
   const int rb = row_beg[i];
   const int re = rb + cnt[i].x;
-  float* dst = aev + (size_t)row_of_atom[i] * AEV_LEN;
+  const int row = row_of_atom[i];
+  float* dst = aev + (size_t)row * AEV_LEN;
+  // one 32-column chunk of my row: lane <-> column.  PACK16: my fp16 element of the chunk image (the 32
+  // lanes fill one 64-byte row of the hi block and one of the lo block)
+  uint8_t* pk = nullptr;
+  if (PACK16) {
+    const uint32_t r = (uint32_t)row & 127u, k = lane;
+    pk = reinterpret_cast<uint8_t*>(aev) + (size_t)(row >> 7) * (AEV_LEN / 32) * K2_PACK_CHUNK_BYTES +
+         (r >> 3) * 512u + (r & 7u) * 64u + ((((k >> 3) ^ ((r >> 1) & 3u)) << 4) | ((k & 7u) << 1));
+  }
+  auto emit = [&](int c, float v) {
+    if (!PACK16) {
+      dst[32 * c + (int)lane] = v;
+    } else {
+      const float sv = K2_PACK_SCALE * v;
+      const __half h = __float2half_rn(sv);
+      const __half l = __float2half_rn(sv - __half2float(h));
+      *reinterpret_cast<__half*>(pk + (size_t)c * K2_PACK_CHUNK_BYTES) = h;
+      *reinterpret_cast<__half*>(pk + (size_t)c * K2_PACK_CHUNK_BYTES + K2_PACK_CHUNK_BYTES / 2) = l;
+    }
+  };
   int m = 0;
   uint32_t na = 0;                                // angular neighbours per species, one byte each
   float acc[NSPEC] = {0.f, 0.f, 0.f, 0.f};
@@ -112,8 +143,8 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __re
   // radial part of the row: lanes 0-15 hold shell k of species 0 / 2, lanes 16-31 of species 1 / 3
 #pragma unroll
   for (int z = 0; z < NSPEC; ++z) acc[z] += __shfl_xor_sync(0xffffffffu, acc[z], 16);
-  dst[lane] = 0.25f * (half ? acc[1] : acc[0]);
-  dst[32 + lane] = 0.25f * (half ? acc[3] : acc[2]);
+  emit(0, 0.25f * (half ? acc[1] : acc[0]));
+  emit(1, 0.25f * (half ? acc[3] : acc[2]));
   if (m > MAX_ANG) {                              // outputs unspecified (S25); keep every index in range
     if (lane == 0) atomicOr(status, ST_ANGULAR_ROW);
     m = 0; na = 0;
@@ -221,7 +252,20 @@ k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __re
     __syncwarp();
   }
 #pragma unroll
-  for (int p = 0; p < NPAIR; ++p) dst[RAD_LEN + 32 * p + (int)lane] = out[p];
+  for (int p = 0; p < NPAIR; ++p) emit(2 + p, out[p]);
+}
+
+// pfc_get_intermediates on the tensor path: the packed operand image back to fp32 rows
+// (aev = (hi + lo) / 8: the value the tensor core multiplies, within 2^-23 of K2's fp32 sum)
+__global__ void k2_unpack16_kernel(int n_rows, const uint8_t* __restrict__ packed, float* __restrict__ aev) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_rows * AEV_LEN) return;
+  const uint32_t row = (uint32_t)(idx / AEV_LEN), col = (uint32_t)(idx % AEV_LEN), r = row & 127u, k = col & 31u;
+  const uint8_t* blk = packed + ((size_t)(row >> 7) * (AEV_LEN / 32) + (size_t)(col >> 5)) * K2_PACK_CHUNK_BYTES +
+                       (r >> 3) * 512u + (r & 7u) * 64u + ((((k >> 3) ^ ((r >> 1) & 3u)) << 4) | ((k & 7u) << 1));
+  const float hi = __half2float(*reinterpret_cast<const __half*>(blk));
+  const float lo = __half2float(*reinterpret_cast<const __half*>(blk + K2_PACK_CHUNK_BYTES / 2));
+  aev[idx] = (hi + lo) * (1.0f / K2_PACK_SCALE);
 }
 
 }  // namespace pfc

@@ -17,20 +17,21 @@
 // term misses the tolerance.
 //
 // One persistent CTA per SM, 320 threads, 128-row tiles of ONE element each:
-//   warps 0-7  workers: make the A operand of every phase in 32-wide K chunks (hi | lo, K-major,
-//              SWIZZLE_64B) -- phase 0 from the AEV rows in global memory, later phases from the
-//              previous accumulator in TMEM (bias, CELU, CELU', Hadamard) -- and drain g;
+//   warps 0-7  workers: make the A operand of phases 1-7 in 32-wide K chunks (hi | lo, K-major,
+//              SWIZZLE_64B) from the previous accumulator in TMEM (bias, CELU, CELU', Hadamard), and
+//              drain g;
 //   warp 8     TMA: streams the pre-packed, pre-swizzled weight chunks (hi | lo) of the schedule
-//              from L2 into a 4-slot ring with cp.async.bulk + mbarrier;
+//              from L2 into a 4-slot ring with cp.async.bulk + mbarrier -- and the A operand of
+//              phase 0, which K2 writes in exactly the chunk image the tensor core reads (AEV times 8,
+//              fp16 hi | lo, SWIZZLE_64B; one contiguous 16 KB block per tile and chunk), into ring A;
 //   warp 9     one elected thread issues tcgen05.mma and commits to the ring / phase barriers.
 // Schedule.  The eight phases of a tile are a serial chain (each needs the previous
 // accumulator), except at its two ends: the first GEMM (AEV x W1) depends only on global
 // memory and the three g passes (delta1 x W1^T) only on delta1.  So consecutive tiles are
 // software-pipelined: while the tensor pipe runs the g passes of tile t (delta1 kept RESIDENT in
 // shared memory, produced once) it also runs the first GEMM of tile t+1 (the "overlapped
-// block"); meanwhile warps 0-3 drain g of tile t (TMEM -> global, two accumulator buffers) and
-// warps 4-7 convert the AEV chunks of tile t+1 (global -> fp16 hi | lo -> ring).  Then all eight
-// warps walk the chain z1 -> h1 -> z2 -> h2 -> z3 -> delta3 -> d2pre -> delta2 -> d1pre -> delta1.
+// block"); meanwhile warps 0-3 drain g of tile t (TMEM -> global, two accumulator buffers).  Then all
+// eight warps walk the chain z1 -> h1 -> z2 -> h2 -> z3 -> delta3 -> d2pre -> delta2 -> d1pre -> delta1.
 // TMEM (512 columns):  z1 [0,160)   z2 [160,288)   z3 [288,384)   d2pre [384,512)
 //                      d1pre [160,320)   g buffer A [384,512)   g buffer B [160,288)
 // The accumulate step of the tensor core rounds toward zero -- the running sum once per MMA
@@ -99,7 +100,7 @@ __host__ __device__ constexpr int tc_block_op(int i) {
 }
 
 struct TcSmem {                                   // after the 1024-aligned operand regions
-  uint64_t a0_full[TC_NA], a_full[TC_NA], a_empty[TC_NA];   // ring A: first-GEMM chunks (128 producers) / chain chunks (256)
+  uint64_t a0_full[TC_NA], a_full[TC_NA], a_empty[TC_NA];   // ring A: first-GEMM chunks (bulk copy) / chain chunks (256 producers)
   uint64_t b_full[TC_NB], b_empty[TC_NB];
   uint64_t z_full[5];                             // accumulators z1, z2, z3, d2pre, d1pre complete
   uint64_t g_full[2];                             // g buffer A / B complete
@@ -110,6 +111,7 @@ struct TcSmem {                                   // after the 1024-aligned oper
   uint64_t p5_done;                               // the delta1 producers have finished reading TMEM (256)
   uint32_t tmem_base;
   float epart[2][TC_TM];
+  float4 stage[4][32 * 8];                        // per drain warp: 32 rows x 32 columns of g, 16-byte units XOR-swizzled by row
 };
 constexpr size_t TC_SMEM_BYTES = 1024 + (size_t)TC_ND1 * TC_A_SLOT + (size_t)TC_NA * TC_A_SLOT +
                                  (size_t)TC_NB * TC_B_SLOT + sizeof(TcSmem);
@@ -124,6 +126,7 @@ struct TcParams {
   const float* bias[NSPEC];    // TC_BIAS_LEN floats per element; kf[q] = (1 + beta_q) 2^-(operand scales) of epilogue q
   int row_start[NSPEC + 1];
   int n_tiles;
+  long long* trace;            // DEVICE or NULL: pfc_k3_timeline (CTA 0 records clock64 at the events of TC_TRACE_*)
 };
 
 // ---- kind::f16 descriptors ----------------------------------------------------------------------
@@ -168,11 +171,22 @@ __device__ __forceinline__ void tc_split2(float x0, float x1, uint32_t& hi, uint
   lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
-// CELU(x) and CELU'(x), alpha = 0.1:  e = exp(min(x,0)/alpha)
+// CELU(x) and CELU'(x), alpha = 0.1, branch-free:  e = exp(min(x,0)/alpha) is exactly 1 for x >= 0, so
+//   CELU'(x) = e   and   CELU(x) = max(x,0) + alpha (e - 1)
+__device__ __forceinline__ float celu_d(float x) { return ex2_approx(fminf(x, 0.0f) * (LOG2E / CELU_ALPHA)); }
+__device__ __forceinline__ float celu_h(float x) { return fmaxf(x, 0.0f) + fmaf(CELU_ALPHA, celu_d(x), -CELU_ALPHA); }
 __device__ __forceinline__ void celu_both(float x, float& h, float& d) {
-  const float e = ex2_approx(fminf(x, 0.0f) * (LOG2E / CELU_ALPHA));
-  h = x > 0.0f ? x : CELU_ALPHA * (e - 1.0f);
-  d = x > 0.0f ? 1.0f : e;
+  d = celu_d(x);
+  h = fmaxf(x, 0.0f) + fmaf(CELU_ALPHA, d, -CELU_ALPHA);
+}
+
+// 16 consecutive floats of a 64-byte aligned table (biases, w4) through the read-only path, four 16-byte loads
+__device__ __forceinline__ void tc_ld16(const float* p, float (&v)[16]) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float4 t = __ldg(reinterpret_cast<const float4*>(p) + j);
+    v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
+  }
 }
 
 // store 16 consecutive K values (columns 16*hf .. 16*hf+15 of a 32-wide chunk) of row r as hi | lo
@@ -189,9 +203,19 @@ __device__ __forceinline__ void tc_store_a16(uint8_t* slot, int r, int hf, const
   }
 }
 
+// pfc_k3_timeline: 64 slots per tile iteration of CTA 0.  MMA issuer: 0 iteration start, 1..27 after block op i,
+// 28..31 after the chain GEMMs 1..4 are issued.  Worker thread 0 (drain group): 32 block start, 33..35 after drain
+// pass 0..2, then 36/37 .. 44/45 = accumulator seen / operand written for h1, h2, delta3, delta2, delta1.  Worker
+// (slots 48.. unused).
+constexpr int TC_TRACE_STRIDE = 128, TC_TRACE_ITERS = 8;
+#define TC_TRACE(slot)                                                                              \
+  do {                                                                                              \
+    if (P.trace != nullptr && blockIdx.x == 0 && it < TC_TRACE_ITERS) P.trace[it * TC_TRACE_STRIDE + (slot)] = clock64(); \
+  } while (0)
+
 template <int N_TERMS>
 __global__ void __launch_bounds__(TC_THREADS, 1)
-k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ aev, float* __restrict__ g,
+k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__ aev16, float* __restrict__ g,
                  float* __restrict__ e_row) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* base = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -203,7 +227,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
 
   if (tid == 0) {
     for (int i = 0; i < TC_NA; ++i) {
-      tc::mbar_init(&S.a0_full[i], TC_WORKERS / 2); tc::mbar_init(&S.a_full[i], TC_WORKERS); tc::mbar_init(&S.a_empty[i], 1);
+      tc::mbar_init(&S.a0_full[i], 1); tc::mbar_init(&S.a_full[i], TC_WORKERS); tc::mbar_init(&S.a_empty[i], 1);
     }
     for (int i = 0; i < TC_NB; ++i) { tc::mbar_init(&S.b_full[i], 1); tc::mbar_init(&S.b_empty[i], 1); }
     for (int i = 0; i < 5; ++i) tc::mbar_init(&S.z_full[i], 1);
@@ -250,6 +274,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
     for (int it = 0; it <= n_my; ++it) {
       const bool have_prev = it >= 1, have_cur = it < n_my;
       const uint32_t par = (uint32_t)it & 1u, par_prev = ((uint32_t)it + 1u) & 1u;
+      if (tid == 0) TC_TRACE(32);
       // ------------------------------ overlapped block ------------------------------
       if (hf == 0) {
         // drain g of the previous tile: pass 0 and 2 from buffer A, pass 1 from buffer B
@@ -262,9 +287,12 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
             // completions of g_full[A]: two per tile (2(it-1), 2(it-1)+1); of g_full[B]: one per tile
             tc::mbar_wait(&S.g_full[buf], buf ? par_prev : (uint32_t)(pass >> 1));
             tc::tc_fence_after();
-            float* dst = g + (size_t)(row0 + r) * AEV_LEN + pass * TC_GN;
             const uint32_t col = (uint32_t)(buf ? TC_COL_GB : TC_COL_GA);
-#pragma unroll
+            // 32 x 32 blocks: TMEM gives every lane its own row; the block is transposed through shared
+            // memory so that each store instruction writes four complete 128-byte row segments (a lane
+            // storing its own row touched 32 different lines per instruction: 3.7 us per pass, measured)
+            float4* stg = S.stage[q];
+#pragma unroll 1
             for (int c = 0; c < TC_GN / 32; ++c) {
               float v0[16], v1[16];
               tc::tmem_ld16(tlane + col + 32 * c, v0);
@@ -272,63 +300,27 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
               tc::tmem_ld_wait();
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
-                reinterpret_cast<float4*>(dst + 32 * c)[k] =
-                    make_float4(kg * v0[4 * k], kg * v0[4 * k + 1], kg * v0[4 * k + 2], kg * v0[4 * k + 3]);
-                reinterpret_cast<float4*>(dst + 32 * c + 16)[k] =
-                    make_float4(kg * v1[4 * k], kg * v1[4 * k + 1], kg * v1[4 * k + 2], kg * v1[4 * k + 3]);
+                stg[lane * 8 + (k ^ (lane & 7))] = make_float4(kg * v0[4 * k], kg * v0[4 * k + 1], kg * v0[4 * k + 2], kg * v0[4 * k + 3]);
+                stg[lane * 8 + ((4 + k) ^ (lane & 7))] = make_float4(kg * v1[4 * k], kg * v1[4 * k + 1], kg * v1[4 * k + 2], kg * v1[4 * k + 3]);
               }
+              __syncwarp();
+              float* blk = g + (size_t)(row0 + 32 * q) * AEV_LEN + pass * TC_GN + 32 * c;
+#pragma unroll
+              for (int i = 0; i < 8; ++i) {
+                const int rr = 4 * i + (lane >> 3), u = lane & 7;
+                *reinterpret_cast<float4*>(blk + (size_t)rr * AEV_LEN + 4 * u) = stg[rr * 8 + (u ^ (rr & 7))];
+              }
+              __syncwarp();
             }
             if (buf == 0) {
               tc::tc_fence_before();
               tc::mbar_arrive(&S.g_free);
             }
+            if (tid == 0) TC_TRACE(33 + pass);
           }
-        }
-        if (have_cur) ia += D0 / TC_KC;                        // the twelve first-GEMM chunks are made by warps 4-7
-      } else if (have_cur) {
-        // first-GEMM operand of the current tile: AEV rows (times 8), 12 chunks of 32 columns -> hi | lo
-        const int ty = tid - TC_WORKERS / 2;                   // 0..127
-        const float4* src = reinterpret_cast<const float4*>(aev + (size_t)tile_of(it) * TC_TM * AEV_LEN);
-        // float4 f = ty + 128 i (i < 8) of a chunk: row f >> 3, 16-byte piece f & 7 of its 128 bytes
-        float4 buf0[8], buf1[8];
-        auto load = [&](float4 (&b)[8], int c) {
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const int f = ty + (TC_WORKERS / 2) * i;
-            b[i] = __ldg(src + (size_t)(f >> 3) * (AEV_LEN / 4) + 8 * c + (f & 7));
-          }
-        };
-        auto convert = [&](const float4 (&b)[8], uint8_t* slot) {
-          constexpr float sc = (float)(1 << TC_AEV_SCALE_LOG2);
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const int f = ty + (TC_WORKERS / 2) * i, rr = f >> 3, j = f & 7;   // piece j: k = 4j .. 4j+3
-            uint32_t h0, l0, h1, l1;
-            tc_split2(sc * b[i].x, sc * b[i].y, h0, l0);
-            tc_split2(sc * b[i].z, sc * b[i].w, h1, l1);
-            const uint32_t off = tc_sw64_off((uint32_t)rr, (uint32_t)(4 * j));
-            *reinterpret_cast<uint2*>(slot + off) = make_uint2(h0, h1);
-            *reinterpret_cast<uint2*>(slot + TC_A_HALF + off) = make_uint2(l0, l1);
-          }
-        };
-        load(buf0, 0);
-        load(buf1, 1);
-#pragma unroll 1
-        for (int c = 0; c < D0 / TC_KC; c += 2) {
-          uint8_t* slot = acquire();
-          convert(buf0, slot);
-          if (c + 2 < D0 / TC_KC) load(buf0, c + 2);
-          tc::fence_proxy_async_smem();
-          tc::mbar_arrive(&S.a0_full[ia % TC_NA]);
-          ++ia;
-          slot = acquire();
-          convert(buf1, slot);
-          if (c + 3 < D0 / TC_KC) load(buf1, c + 3);
-          tc::fence_proxy_async_smem();
-          tc::mbar_arrive(&S.a0_full[ia % TC_NA]);
-          ++ia;
         }
       }
+      if (have_cur) ia += D0 / TC_KC;                          // the twelve first-GEMM chunks come by bulk copy (warp 8)
       if (!have_cur) break;
       // ------------------------------ chain of the current tile ------------------------------
       const int row0 = tile_of(it) * TC_TM;
@@ -338,38 +330,45 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
       // ---- z1 -> h1 = CELU(z1 + b1): operand of phase 1 ----
       tc::mbar_wait(&S.z_full[0], par);
       tc::tc_fence_after();
+      if (tid == 0) TC_TRACE(36);
 #pragma unroll 1
       for (int c = 0; c < D1 / TC_KC; ++c) {
-        float z[16], h[16], d;
+        float z[16], h[16];
         tc::tmem_ld16(tlane + TC_COL_Z1 + 32 * c + 16 * hf, z);
         tc::tmem_ld_wait();
-        const float* b = bias + TC_BIAS_B1 + 32 * c + 16 * hf;
+        float bb[16];
+        tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) celu_both(fmaf(z[k], k0, __ldg(b + k)), h[k], d);
+        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k0, bb[k]));
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
         ++ia;
       }
+      if (tid == 0) TC_TRACE(37);
       // ---- z2 -> h2: operand of phase 2 ----
       tc::mbar_wait(&S.z_full[1], par);
       tc::tc_fence_after();
+      if (tid == 0) TC_TRACE(38);
 #pragma unroll 1
       for (int c = 0; c < D2 / TC_KC; ++c) {
-        float z[16], h[16], d;
+        float z[16], h[16];
         tc::tmem_ld16(tlane + TC_COL_Z2 + 32 * c + 16 * hf, z);
         tc::tmem_ld_wait();
-        const float* b = bias + TC_BIAS_B2 + 32 * c + 16 * hf;
+        float bb[16];
+        tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) celu_both(fmaf(z[k], k1, __ldg(b + k)), h[k], d);
+        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k1, bb[k]));
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
         ++ia;
       }
+      if (tid == 0) TC_TRACE(39);
       // ---- z3 -> e_i = w4.h3 + b4 and delta3 = w4 * CELU'(z3 + b3) (scaled): operand of phase 3 ----
       tc::mbar_wait(&S.z_full[2], par);
       tc::tc_fence_after();
+      if (tid == 0) TC_TRACE(40);
       {
         float epart = 0.0f;
 #pragma unroll 1
@@ -377,15 +376,16 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           float z[16], dl[16];
           tc::tmem_ld16(tlane + TC_COL_Z3 + 32 * c + 16 * hf, z);
           tc::tmem_ld_wait();
-          const float* b = bias + TC_BIAS_B3 + 32 * c + 16 * hf;
-          const float* w4 = bias + TC_BIAS_W4 + 32 * c + 16 * hf;
-          const float* w4s = bias + TC_BIAS_W4S + 32 * c + 16 * hf;
+          float bb[16], w4[16], w4s[16];
+          tc_ld16(bias + TC_BIAS_B3 + 32 * c + 16 * hf, bb);
+          tc_ld16(bias + TC_BIAS_W4 + 32 * c + 16 * hf, w4);
+          tc_ld16(bias + TC_BIAS_W4S + 32 * c + 16 * hf, w4s);
 #pragma unroll
           for (int k = 0; k < 16; ++k) {
             float h, d;
-            celu_both(fmaf(z[k], k2, __ldg(b + k)), h, d);
-            epart = fmaf(__ldg(w4 + k), h, epart);
-            dl[k] = __ldg(w4s + k) * d;
+            celu_both(fmaf(z[k], k2, bb[k]), h, d);
+            epart = fmaf(w4[k], h, epart);
+            dl[k] = w4s[k] * d;
           }
           uint8_t* slot = acquire();
           tc_store_a16(slot, r, hf, dl);
@@ -396,12 +396,14 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
         asm volatile("bar.sync 1, %0;" ::"n"(TC_WORKERS) : "memory");
         if (hf == 0) e_row[row0 + r] = (S.epart[0][r] + S.epart[1][r]) + __ldg(bias + TC_BIAS_B4);
       }
+      if (tid == 0) TC_TRACE(41);
       // ---- delta2 = d2pre * CELU'(z2 + b2): operand of phase 4 ----
       // d1pre (phase 4's accumulator) overwrites z2 / z3, so phase 4 cannot start before ALL of delta2
       // exists: its four chunks go to the resident region (free at this point: the previous tile's g
       // passes are over), not through the three-slot ring, which could not hold them
       tc::mbar_wait(&S.z_full[3], par);
       tc::tc_fence_after();
+      if (tid == 0) TC_TRACE(42);
       if (have_prev) tc::mbar_wait(&S.d1_free, par_prev);      // the previous tile's g passes have read the region
 #pragma unroll 1
       for (int c = 0; c < D2 / TC_KC; ++c) {
@@ -409,42 +411,46 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
         tc::tmem_ld16(tlane + TC_COL_Z2 + 32 * c + 16 * hf, z);
         tc::tmem_ld16(tlane + TC_COL_D2 + 32 * c + 16 * hf, p);
         tc::tmem_ld_wait();
-        const float* b = bias + TC_BIAS_B2 + 32 * c + 16 * hf;
+        float bb[16];
+        tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
-          float h, d;
-          celu_both(fmaf(z[k], k1, __ldg(b + k)), h, d);
-          p[k] = (p[k] * k3) * d;
-        }
+        for (int k = 0; k < 16; ++k) p[k] = (p[k] * k3) * celu_d(fmaf(z[k], k1, bb[k]));
         tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
       }
       publish(&S.dd_full);
+      if (tid == 0) TC_TRACE(43);
       // ---- delta1 = d1pre * CELU'(z1 + b1): RESIDENT operand of the three g passes ----
       tc::mbar_wait(&S.z_full[4], par);                        // (phase 4 has consumed delta2: the region is free again)
       tc::tc_fence_after();
+      if (tid == 0) TC_TRACE(44);
 #pragma unroll 1
       for (int c = 0; c < TC_ND1; ++c) {
         float z[16], p[16];
         tc::tmem_ld16(tlane + TC_COL_Z1 + 32 * c + 16 * hf, z);
         tc::tmem_ld16(tlane + TC_COL_D1 + 32 * c + 16 * hf, p);
         tc::tmem_ld_wait();
-        const float* b = bias + TC_BIAS_B1 + 32 * c + 16 * hf;
+        float bb[16];
+        tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
-          float h, d;
-          celu_both(fmaf(z[k], k0, __ldg(b + k)), h, d);
-          p[k] = (p[k] * k4) * d;
-        }
+        for (int k = 0; k < 16; ++k) p[k] = (p[k] * k4) * celu_d(fmaf(z[k], k0, bb[k]));
         tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
         publish(&S.d1_full[c]);
       }
       tc::tc_fence_before();
       tc::mbar_arrive(&S.p5_done);
+      if (tid == 0) TC_TRACE(45);
     }
   } else if (warp == 8) {
     // =========================== TMA: weight chunks ===========================
     if (lane == 0) {
-      uint32_t ib = 0;
+      uint32_t ib = 0, ia = 0;
+      auto stream_a = [&](const uint8_t* src) {                // one first-GEMM operand chunk (hi | lo, as K2 wrote it) into ring A
+        const uint32_t s = ia % TC_NA, use = ia / TC_NA;
+        tc::mbar_wait(&S.a_empty[s], (use & 1u) ^ 1u);
+        tc::mbar_arrive_expect_tx(&S.a0_full[s], (uint32_t)TC_A_SLOT);
+        tc::bulk_g2s(ringA + s * TC_A_SLOT, src, (uint32_t)TC_A_SLOT, &S.a0_full[s]);
+        ++ia;
+      };
       auto stream = [&](const uint8_t* src, uint32_t bytes) {
         const uint32_t s = ib % TC_NB, use = ib / TC_NB;
         tc::mbar_wait(&S.b_empty[s], (use & 1u) ^ 1u);
@@ -460,7 +466,10 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
         for (int i = 0; i < TC_BLOCK_OPS; ++i) {
           const int op = tc_block_op(i);
           if (op >> 8) {
-            if (have_cur) stream(wcur + tc_phase_off(0) + (size_t)(op & 15) * tc_chunk_bytes(0), (uint32_t)tc_chunk_bytes(0));
+            if (have_cur) {
+              stream_a(aev16 + ((size_t)tile_of(it) * (D0 / TC_KC) + (size_t)(op & 15)) * TC_A_SLOT);
+              stream(wcur + tc_phase_off(0) + (size_t)(op & 15) * tc_chunk_bytes(0), (uint32_t)tc_chunk_bytes(0));
+            }
           } else if (have_prev) {
             stream(wprev + tc_phase_off(5 + ((op >> 4) & 3)) + (size_t)(op & 15) * tc_chunk_bytes(5), (uint32_t)tc_chunk_bytes(5));
           }
@@ -472,6 +481,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
           const uint32_t bytes = (uint32_t)tc_chunk_bytes(p);
           for (int c = 0; c < tc_phase_nk(p); ++c) stream(src + (size_t)c * bytes, bytes);
         }
+        ia += (uint32_t)(tc_phase_nk(1) + tc_phase_nk(2) + tc_phase_nk(3));   // the chain's ring A chunks are made by the workers
       }
     }
   } else {
@@ -502,7 +512,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
         tc::mma_commit(&S.b_empty[sb]);
         ++ib;
       };
-      // a chunk whose A operand comes through ring A (kind 0: first GEMM, 128 producers; kind 1: chain, 256)
+      // a chunk whose A operand comes through ring A (kind 0: first GEMM, bulk copy; kind 1: chain, 256 producers)
       auto issue_ring = [&](uint32_t dcol, int N, bool first, int kind) {
         const uint32_t sa = ia % TC_NA;
         if (kind == 0) { tc::mbar_wait(&S.a0_full[sa], (par_a0 >> sa) & 1u); par_a0 ^= 1u << sa; }
@@ -514,6 +524,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
       for (int it = 0; it <= n_my; ++it) {
         const bool have_prev = it >= 1, have_cur = it < n_my;
         const uint32_t par_prev = ((uint32_t)it + 1u) & 1u;
+        TC_TRACE(0);
         // ------------------------------ overlapped block ------------------------------
         bool p5_waited = !have_prev;
 #pragma unroll 1
@@ -538,19 +549,24 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const float* __restrict__ a
               if (pass == TC_NPASS - 1) tc::mma_commit(&S.d1_free);
             }
           }
+          TC_TRACE(1 + i);
         }
         if (!have_cur) break;
         // ------------------------------ chain ------------------------------
         for (int c = 0; c < tc_phase_nk(1); ++c) issue_ring(tbase + TC_COL_Z2, tc_phase_n(1), c == 0, 1);
         tc::mma_commit(&S.z_full[1]);
+        TC_TRACE(28);
         for (int c = 0; c < tc_phase_nk(2); ++c) issue_ring(tbase + TC_COL_Z3, tc_phase_n(2), c == 0, 1);
         tc::mma_commit(&S.z_full[2]);
+        TC_TRACE(29);
         for (int c = 0; c < tc_phase_nk(3); ++c) issue_ring(tbase + TC_COL_D2, tc_phase_n(3), c == 0, 1);
         tc::mma_commit(&S.z_full[3]);
+        TC_TRACE(30);
         tc::mbar_wait(&S.dd_full, (uint32_t)it & 1u);            // all of delta2 is in the resident region
         for (int c = 0; c < tc_phase_nk(4); ++c)
           issue(tbase + TC_COL_D1, tc::smem_u32(resD1 + c * TC_A_SLOT), tc_phase_n(4), c == 0);
         tc::mma_commit(&S.z_full[4]);
+        TC_TRACE(31);
       }
     }
   }

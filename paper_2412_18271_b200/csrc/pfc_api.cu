@@ -62,11 +62,13 @@ struct Buffers {
   uint32_t* nbr;                // [cap_r] entry words (k1_neighbors.cuh)
   int2 *cnt, *block_tot;
   int *r_off, *a_off, *r_idx, *a_idx;   // CSR export (pfc_get_neighbors only)
-  float *aev, *g, *e_row;
+  float *aev, *g, *e_row;       // aev: fp32 rows (FP32 MLP) or the packed fp16 operand image (tensor MLP), same bytes
+  float* aev_unpacked;          // pfc_get_intermediates on the tensor path
   float4 *edge, *self, *xlo;
   uint32_t* status;
   StepParams* sp;
   unsigned long long* work;     // pfc_work_counts
+  long long* trace;             // pfc_k3_timeline
   float* weights;
   uint8_t* wtc;                 // tensor-core path: packed hi|lo swizzled weight chunks
   float* bias_tc;
@@ -100,6 +102,7 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.a_idx = c.take<int>((size_t)s.cap_r);
   t.aev = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.g = c.take<float>((size_t)s.n_rows * AEV_LEN);
+  t.aev_unpacked = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.e_row = c.take<float>((size_t)s.n_rows);
   t.edge = c.take<float4>((size_t)s.cap_r);
   t.self = c.take<float4>(N);
@@ -107,6 +110,7 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.status = c.take<uint32_t>(64);
   t.sp = c.take<StepParams>(1);
   t.work = c.take<unsigned long long>(8);
+  t.trace = c.take<long long>((size_t)TC_TRACE_STRIDE * TC_TRACE_ITERS);
   t.weights = c.take<float>((size_t)NSPEC * DEV_W_PER_ELEM);
   t.wtc = c.take<uint8_t>((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
   t.bias_tc = c.take<float>((size_t)NSPEC * TC_BIAS_LEN);
@@ -243,8 +247,12 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool wit
            b.row_beg, b.nbr, b.cnt, b.status);
   }
   mark(1);
-  LAUNCH(c, k2_aev_fwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
-         b.row_of_atom, b.aev, b.status);
+  if (c->mlp_path == PFC_MLP_FP32)
+    LAUNCH(c, k2_aev_fwd_kernel<false>, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
+           b.row_of_atom, b.aev, b.status);
+  else                                                    // the tensor MLP's first operand, as it sits in shared memory
+    LAUNCH(c, k2_aev_fwd_kernel<true>, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
+           b.row_of_atom, b.aev, b.status);
   mark(2);
   if (c->mlp_path == PFC_MLP_FP32) {
 #define K3_LAUNCH(TM_, DEEP_)                                                                          \
@@ -263,10 +271,10 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool wit
 #undef K3_LAUNCH
   } else {
     const int grid = c->tcp.n_tiles < c->n_sms ? c->tcp.n_tiles : c->n_sms;   // persistent: one CTA per SM
-    if (c->mlp_path == PFC_MLP_TF32X3)
-      LAUNCH(c, k3_mlp_tc_kernel<3>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, b.aev, b.g, b.e_row);
+    if (c->mlp_path == PFC_MLP_TENSOR)
+      LAUNCH(c, k3_mlp_tc_kernel<3>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, (const uint8_t*)b.aev, b.g, b.e_row);
     else
-      LAUNCH(c, k3_mlp_tc_kernel<1>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, b.aev, b.g, b.e_row);
+      LAUNCH(c, k3_mlp_tc_kernel<1>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, (const uint8_t*)b.aev, b.g, b.e_row);
   }
   mark(3);
   LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
@@ -336,7 +344,7 @@ size_t pfc_workspace_bytes(int32_t n_atoms, int32_t n_systems) {
 int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (!d || !out || !d->species || !d->sys_offsets || !d->weights) return PFC_ERR_ARG;
   if (d->n_atoms < 1 || d->n_systems < 1 || d->n_systems > d->n_atoms) return PFC_ERR_ARG;
-  if (d->mlp_path != PFC_MLP_FP32 && d->mlp_path != PFC_MLP_TF32X3 && d->mlp_path != PFC_MLP_TF32X1 &&
+  if (d->mlp_path != PFC_MLP_FP32 && d->mlp_path != PFC_MLP_TENSOR && d->mlp_path != PFC_MLP_TENSOR_1TERM &&
       d->mlp_path != PFC_MLP_AUTO)
     return PFC_ERR_ARG;
   const int N = d->n_atoms, NS = d->n_systems;
@@ -368,7 +376,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   // SMs.  Measured ms/step, FFMA vs tensor, replicas of config 1: 2,200 atoms 0.108 / 0.111, 3,960
   // 0.113 / 0.115, 4,840 0.136 / 0.121, 5,632 0.139 / 0.124; of config 4: 3,758 atoms 0.143 / 0.145,
   // 4,749 0.163 / 0.147; config 2 (1,500 atoms) 0.111 / 0.141
-  c->mlp_path = d->mlp_path == PFC_MLP_AUTO ? (d->n_atoms >= 4096 ? PFC_MLP_TF32X3 : PFC_MLP_FP32) : d->mlp_path;
+  c->mlp_path = d->mlp_path == PFC_MLP_AUTO ? (d->n_atoms >= 4096 ? PFC_MLP_TENSOR : PFC_MLP_FP32) : d->mlp_path;
   c->sz = worst_case_sizes(N, NS);                      // capacities are the worst-case ones
   // static element grouping: rows sorted by element, blocks padded to ROW_PAD
   int row_start[NSPEC + 1];
@@ -457,7 +465,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   // weight matrix scaled by the power of two that puts max|W| into [256, 512) (k3_mlp_tc.cuh)
   std::vector<uint8_t> wtc((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
   std::vector<float> bias_tc((size_t)NSPEC * TC_BIAS_LEN, 0.0f);
-  const int n_terms = c->mlp_path == PFC_MLP_TF32X1 ? 1 : 3;
+  const int n_terms = c->mlp_path == PFC_MLP_TENSOR_1TERM ? 1 : 3;
   for (int e = 0; e < NSPEC; ++e) {
     const float* src = d->weights + (size_t)e * W_PER_ELEM;
     const float *W1 = src, *b1 = W1 + D1 * D0, *W2 = b1 + D1, *b2 = W2 + D2 * D1, *W3 = b2 + D2,
@@ -518,6 +526,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   c->tcp.wpack = c->b.wtc;
   for (int e = 0; e <= NSPEC; ++e) c->tcp.row_start[e] = row_start[e];
   c->tcp.n_tiles = c->sz.n_rows / TC_TM;
+  c->tcp.trace = nullptr;
 
   StepParams sp0{};
   {
@@ -675,6 +684,25 @@ __global__ void k_work_counts_kernel(int n_atoms, const int2* __restrict__ cnt, 
     r += __shfl_xor_sync(0xffffffffu, r, o); a += __shfl_xor_sync(0xffffffffu, a, o); t += __shfl_xor_sync(0xffffffffu, t, o);
   }
   if ((threadIdx.x & 31) == 0) { atomicAdd(out, r); atomicAdd(out + 1, a); atomicAdd(out + 2, t); }
+}
+
+int pfc_k3_timeline(pfc_t* c, int64_t* cycles, int32_t n) {
+  if (!c || !cycles || n < 1) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;
+  if (c->mlp_path == PFC_MLP_FP32) return PFC_ERR_STATE;
+  const int total = TC_TRACE_STRIDE * TC_TRACE_ITERS;
+  cudaStream_t st = c->stream;
+  if (cudaMemsetAsync(c->b.trace, 0, sizeof(long long) * total, st) != cudaSuccess) return PFC_ERR_CUDA;
+  TcParams tp = c->tcp;
+  tp.trace = c->b.trace;
+  const int grid = tp.n_tiles < c->n_sms ? tp.n_tiles : c->n_sms;
+  if (c->mlp_path == PFC_MLP_TENSOR) k3_mlp_tc_kernel<3><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(tp, (const uint8_t*)c->b.aev, c->b.g, c->b.e_row);
+  else k3_mlp_tc_kernel<1><<<grid, TC_THREADS, TC_SMEM_BYTES, st>>>(tp, (const uint8_t*)c->b.aev, c->b.g, c->b.e_row);
+  std::vector<long long> h(total);
+  if (cudaMemcpyAsync(h.data(), c->b.trace, sizeof(long long) * total, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return PFC_ERR_CUDA;
+  for (int i = 0; i < n && i < total; ++i) cycles[i] = (int64_t)h[i];
+  return PFC_OK;
 }
 
 int pfc_work_counts(pfc_t* c, int64_t* counts) {
@@ -862,7 +890,17 @@ int pfc_get_neighbors(pfc_t* c, const int32_t** r_off, const int32_t** r_idx, co
 int pfc_get_intermediates(pfc_t* c, const float** aev, const float** g, const int32_t** row_of_atom,
                           int32_t* n_rows) {
   if (!c) return PFC_ERR_ARG;
-  if (aev) *aev = c->b.aev;
+  if (aev) {
+    if (c->mlp_path == PFC_MLP_FP32) {
+      *aev = c->b.aev;
+    } else {                                            // the tensor path keeps the AEV as the packed operand image: unpack it
+      if (!on_device(c)) return PFC_ERR_STATE;
+      const int n = c->sz.n_rows * AEV_LEN;
+      k2_unpack16_kernel<<<cdiv(n, 256), 256, 0, c->stream>>>(c->sz.n_rows, (const uint8_t*)c->b.aev, c->b.aev_unpacked);
+      if (cudaGetLastError() != cudaSuccess) return PFC_ERR_CUDA;
+      *aev = c->b.aev_unpacked;
+    }
+  }
   if (g) *g = c->b.g;
   if (row_of_atom) *row_of_atom = c->b.row_of_atom;
   if (n_rows) *n_rows = c->sz.n_rows;

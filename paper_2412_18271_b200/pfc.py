@@ -21,9 +21,9 @@ LIB_PATH = os.path.join(_HERE, "libpfc.so")
 AEV_LEN = 384
 N_WEIGHTS = 378756
 MLP_FP32 = 0
-MLP_TF32X3 = 1
-MLP_TF32X1 = 2            # plain TF32: tolerance evidence only
-MLP_AUTO = 3              # TF32X3 from 4096 atoms on, FP32 below
+MLP_TENSOR = 1
+MLP_TENSOR_1TERM = 2      # plain fp16 operands: tolerance evidence only
+MLP_AUTO = 3              # MLP_TENSOR from 4096 atoms on, FP32 below
 
 STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
                4: "angular row longer than PFC_MAX_ANGULAR", 8: "non-finite energy",
@@ -37,7 +37,7 @@ EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy
            "pfc_step", "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host",
            "pfc_run_host_resume", "pfc_get_neighbors", "pfc_get_intermediates", "pfc_status", "pfc_destroy",
            "pfc_error_string")
-DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts")
+DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_k3_timeline", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts")
 
 
 class PfcError(RuntimeError):
@@ -88,6 +88,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_run_host_resume.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int32, c_float, c_void_p, c_void_p]
     lib.pfc_get_neighbors.argtypes = [c_void_p, pp_i32, pp_i32, pp_i32, pp_i32]
     lib.pfc_work_counts.argtypes = [c_void_p, POINTER(ctypes.c_int64)]
+    lib.pfc_k3_timeline.argtypes = [c_void_p, POINTER(ctypes.c_int64), c_int32]
     lib.pfc_get_intermediates.argtypes = [c_void_p, pp_f, pp_f, pp_i32, POINTER(c_int32)]
     lib.pfc_copy_to_host.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.pfc_status.argtypes = [c_void_p, POINTER(c_uint32)]
@@ -292,6 +293,13 @@ class Pfc:
         a, b, k = c_int32(), c_int32(), c_int32()
         _check(self._lib.pfc_launch_counts(self._h, byref(a), byref(b), byref(k)), "pfc_launch_counts")
         return int(k.value)
+
+    @_on_device
+    def k3_timeline(self):
+        """SM-clock timeline of the tensor-core MLP kernel's first CTA: int64 array [8, 128] (pfc_k3_timeline)."""
+        v = (ctypes.c_int64 * 1024)()
+        _check(self._lib.pfc_k3_timeline(self._h, v, 1024), "pfc_k3_timeline")
+        return np.array(v[:], dtype=np.int64).reshape(8, 128)
 
     @_on_device
     def work_counts(self):

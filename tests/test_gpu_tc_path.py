@@ -51,7 +51,7 @@ def _errors(pfc, weights, wl, path, cell=False):
 @pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
 def test_tf32x3_step0_energy_forces_full_size(pfc, weights, k):
     wl = W.make_config(k)
-    err = _errors(pfc, weights, wl, pfc.MLP_TF32X3, cell=(k == 3))
+    err = _errors(pfc, weights, wl, pfc.MLP_TENSOR, cell=(k == 3))
     assert err["E"] <= E_RTOL, err
     assert err["F"] <= F_ATOL_INTERNAL, err
     assert err["e"] <= 1e-5, err
@@ -62,7 +62,7 @@ def test_tf32x3_matches_fp32_path_closely(pfc, weights):
     """The two K3 implementations share no code; their g and F agree to fp32 rounding."""
     wl = W.config4(n_replicas=300)
     out = []
-    for path in (pfc.MLP_FP32, pfc.MLP_TF32X3):
+    for path in (pfc.MLP_FP32, pfc.MLP_TENSOR):
         p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=path)
         E, F = p.energy_forces(_dev(pfc, wl.pos))
         _, g = p.intermediates()
@@ -76,8 +76,8 @@ def test_plain_tf32_misses_the_fp32_bars(pfc, weights):
     """Evidence for the tensor-core decision (north_star (3)): one-term TF32 is 2-3 orders of
     magnitude less accurate in g than the split and misses the internal force target."""
     wl = W.make_config(1)
-    e1 = _errors(pfc, weights, wl, pfc.MLP_TF32X1)
-    e3 = _errors(pfc, weights, wl, pfc.MLP_TF32X3)
+    e1 = _errors(pfc, weights, wl, pfc.MLP_TENSOR_1TERM)
+    e3 = _errors(pfc, weights, wl, pfc.MLP_TENSOR)
     assert e3["g"] <= G_ATOL and e3["F"] <= F_ATOL_INTERNAL
     assert e1["g"] > 50 * e3["g"], (e1, e3)
     assert e1["F"] > F_ATOL_INTERNAL, e1
@@ -85,7 +85,7 @@ def test_plain_tf32_misses_the_fp32_bars(pfc, weights):
 
 
 def _trajectory(pfc, weights, wl, n_steps, cell=False, allow_outliers=0):
-    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TF32X3)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TENSOR)
     pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
     E, F = p.set_state(pos, vel)
     p.step(n_steps, wl.dt_fs)
@@ -122,7 +122,7 @@ def test_uncompensated_tf32x3_misses_the_trajectory_bar(pfc, weights):
     """Evidence for the compensation: switched off (pfc_tuning_t.tc_comp_override with both factors 0)
     the worst replica of config 1 leaves the 1e-4 A bar while all the others keep it."""
     wl = W.make_config(1)
-    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TF32X3,
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TENSOR,
                 tuning=pfc.Tuning(tc_comp_override=1, tc_comp_forward=0.0, tc_comp_backward=0.0))
     pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
     p.set_state(pos, vel)
@@ -148,7 +148,7 @@ def test_tf32x3_bitwise_determinism(pfc, weights):
     wl = W.config4(n_replicas=300)                       # > 148 tiles? no: ~17k rows = 135 tiles + padding
     outs = []
     for _ in range(2):
-        p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TF32X3)
+        p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TENSOR)
         pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
         E, F = p.set_state(pos, vel)
         p.step(10, 0.5)
@@ -166,7 +166,7 @@ def test_compensation_holds_for_another_weight_draw(pfc):
     w7 = W.make_weights(7)
     wl = W.config1(n_replicas=64)
     ref = oracle.energy_forces(wl.pos.astype(np.float64), wl.species, wl.sys_offsets, w7, want_intermediates=True)
-    p = pfc.Pfc(wl.species, wl.sys_offsets, w7, mlp_path=pfc.MLP_TF32X3)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, w7, mlp_path=pfc.MLP_TENSOR)
     pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
     E, F = p.energy_forces(pos)
     torch.cuda.synchronize()
