@@ -83,7 +83,10 @@ typedef struct {
   float tc_comp_forward;      /* used when tc_comp_override = 1 */
   float tc_comp_backward;
   int32_t steps_per_graph;    /* MD steps captured per CUDA graph by pfc_step: 0 = default (16); >= 1 */
-  int32_t reserved[2];        /* must be 0 */
+  int32_t k3_cluster;         /* FP32 MLP of a batch of at most 18 16-row tiles (a single small molecule): 0 = one
+                                 cluster of 8 CTAs per tile (unless k3_tile_rows / k3_deep_ring ask for a variant);
+                                 1 = never; 2 = required (PFC_ERR_ARG if the batch has more tiles) */
+  int32_t reserved;           /* must be 0 */
 } pfc_tuning_t;
 
 typedef struct pfc_ctx pfc_t;           /* opaque; owned by the library          */

@@ -14,8 +14,10 @@ extern "C" {
  * pfc_energy_forces, launched kernel by kernel with a CUDA event recorded on `stream` at every
  * stage boundary; synchronises and returns the device time of each stage in milliseconds,
  * ms HOST [PFC_N_STAGES]: 0 = K1 neighbour build, 1 = K2 AEV forward, 2 = K3 MLP
- * forward+backward, 3 = K4a AEV backward, 4 = K4b force gather, 5 = per-system energy sum. */
-#define PFC_N_STAGES 6
+ * forward+backward, 3 = K4a AEV backward, 4 = K4b force gather, 5 = per-system energy sum,
+ * 6 = K5, the fused integrator kernel of a steady-state step (run on internal staging buffers: the
+ * caller's state does not move; 0 while a pfc_run_host state occupies those buffers). */
+#define PFC_N_STAGES 7
 int pfc_profile_stages(pfc_t *ctx, const float *pos, float *E, float *F, void *stream, float *ms);
 
 /* Work counts of the last evaluation, for the roofline arithmetic: counts HOST [4] =
@@ -33,7 +35,15 @@ int pfc_k3_timeline(pfc_t *ctx, int64_t *cycles, int32_t n);
  * getters of pfc.h into HOST memory. */
 int pfc_copy_to_host(const void *device_src, void *host_dst, size_t bytes);
 
-/* The MLP path in use (PFC_MLP_AUTO resolved by pfc_create). */
+/* Truncation compensation of the tensor-core MLP, per element e = 0..3:
+ * out HOST [32], out[8e + ..] = {lambda forward, lambda backward, residual slope of e_i, residual slope of g,
+ * max|de| / rms e, max|dg| / rms g (all against the library's FP32 MLP on the calibration batch; 0 for an
+ * element below the calibration size), 1 if the scales are final (calibrated or fixed by pfc_tuning_t),
+ * 1 if PFC_MLP_AUTO went back to the FP32 MLP because an element missed the check}. */
+int pfc_tc_calibration(pfc_t *ctx, float *out);
+
+/* The MLP path in use (PFC_MLP_AUTO resolved by pfc_create; after the first evaluation: by the
+ * calibration check as well). */
 int pfc_mlp_path(pfc_t *ctx, int32_t *path);
 
 /* Kernel launches one energy/forces evaluation and one steady-state MD step consist of, and the

@@ -37,8 +37,9 @@
 // The accumulate step of the tensor core rounds toward zero -- the running sum once per MMA
 // instruction, and every product as it is aligned to it (measured: a chain of n K=16 MMAs shrinks
 // an all-positive sum by 9e-8 n, a mixed-sign one by 2e-8 n); the one-sided loss is compensated in
-// the epilogues: every phase returns (1 + beta_p) z with beta_p = lambda n_p 2.15e-8 (kf folds it
-// in; lambda is calibrated per element against the FP32 path at first use).
+// the epilogues: every phase returns (1 + beta_p) z with beta_p = lambda n_p 2.15e-8 (ks, kb below);
+// lambda (forward phases / backward phases) is calibrated per element against the library's own
+// FP32 MLP on the handle's first batch (pfc_api.cu: calibrate_tc).
 #pragma once
 #include <cuda_fp16.h>
 
@@ -117,13 +118,16 @@ constexpr size_t TC_SMEM_BYTES = 1024 + (size_t)TC_ND1 * TC_A_SLOT + (size_t)TC_
                                  (size_t)TC_NB * TC_B_SLOT + sizeof(TcSmem);
 static_assert(TC_SMEM_BYTES <= 227 * 1024, "shared memory budget");
 
-// per element: b1[160] b2[128] b3[96] w4[96] b4[1] pad[3] w4s[96] (w4 times the delta scale) kf[8]
+// per element: b1[160] b2[128] b3[96] w4[96] b4[1] pad[3] w4s[96] (w4 times the delta scale) ks[6] kb[6]
+// Epilogue q returns ks[q] z + kb[q] z: ks[q] = 2^-(operand scales), an exact power of two, and
+// kb[q] = beta_q ks[q] the truncation compensation -- two FMAs, because (1 + beta) itself is not
+// representable finer than 1.2e-7 and beta_q is 4e-7 .. 1.5e-6.
 constexpr int TC_BIAS_B1 = 0, TC_BIAS_B2 = D1, TC_BIAS_B3 = D1 + D2, TC_BIAS_W4 = D1 + D2 + D3,
-              TC_BIAS_B4 = D1 + D2 + D3 + D3, TC_BIAS_W4S = 484, TC_BIAS_KF = 580, TC_BIAS_LEN = 588;
+              TC_BIAS_B4 = D1 + D2 + D3 + D3, TC_BIAS_W4S = 484, TC_BIAS_KS = 580, TC_BIAS_KB = 586, TC_BIAS_LEN = 592;
 
 struct TcParams {
   const uint8_t* wpack;        // [NSPEC][TC_W_BYTES_PER_ELEM] packed hi|lo swizzled weight chunks (scaled)
-  const float* bias[NSPEC];    // TC_BIAS_LEN floats per element; kf[q] = (1 + beta_q) 2^-(operand scales) of epilogue q
+  const float* bias[NSPEC];    // TC_BIAS_LEN floats per element (ks[q], kb[q]: scale and compensation of epilogue q)
   int row_start[NSPEC + 1];
   int n_tiles;
   long long* trace;            // DEVICE or NULL: pfc_k3_timeline (CTA 0 records clock64 at the events of TC_TRACE_*)
@@ -280,7 +284,8 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         // drain g of the previous tile: pass 0 and 2 from buffer A, pass 1 from buffer B
         if (have_prev) {
           const int row0 = tile_of(it - 1) * TC_TM;
-          const float kg = __ldg(P.bias[elem_of(tile_of(it - 1))] + TC_BIAS_KF + 5);
+          const float* bprev = P.bias[elem_of(tile_of(it - 1))];
+          const float kg = __ldg(bprev + TC_BIAS_KS + 5), kgb = __ldg(bprev + TC_BIAS_KB + 5);
 #pragma unroll 1
           for (int pass = 0; pass < TC_NPASS; ++pass) {
             const int buf = pass == 1 ? 1 : 0;
@@ -300,8 +305,9 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
               tc::tmem_ld_wait();
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
-                stg[lane * 8 + (k ^ (lane & 7))] = make_float4(kg * v0[4 * k], kg * v0[4 * k + 1], kg * v0[4 * k + 2], kg * v0[4 * k + 3]);
-                stg[lane * 8 + ((4 + k) ^ (lane & 7))] = make_float4(kg * v1[4 * k], kg * v1[4 * k + 1], kg * v1[4 * k + 2], kg * v1[4 * k + 3]);
+                auto sc = [&](float v) { return fmaf(v, kgb, v * kg); };
+                stg[lane * 8 + (k ^ (lane & 7))] = make_float4(sc(v0[4 * k]), sc(v0[4 * k + 1]), sc(v0[4 * k + 2]), sc(v0[4 * k + 3]));
+                stg[lane * 8 + ((4 + k) ^ (lane & 7))] = make_float4(sc(v1[4 * k]), sc(v1[4 * k + 1]), sc(v1[4 * k + 2]), sc(v1[4 * k + 3]));
               }
               __syncwarp();
               float* blk = g + (size_t)(row0 + 32 * q) * AEV_LEN + pass * TC_GN + 32 * c;
@@ -325,8 +331,10 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       // ------------------------------ chain of the current tile ------------------------------
       const int row0 = tile_of(it) * TC_TM;
       const float* bias = P.bias[elem_of(tile_of(it))];
-      const float k0 = __ldg(bias + TC_BIAS_KF + 0), k1 = __ldg(bias + TC_BIAS_KF + 1), k2 = __ldg(bias + TC_BIAS_KF + 2),
-                  k3 = __ldg(bias + TC_BIAS_KF + 3), k4 = __ldg(bias + TC_BIAS_KF + 4);
+      const float k0 = __ldg(bias + TC_BIAS_KS + 0), k1 = __ldg(bias + TC_BIAS_KS + 1), k2 = __ldg(bias + TC_BIAS_KS + 2),
+                  k3 = __ldg(bias + TC_BIAS_KS + 3), k4 = __ldg(bias + TC_BIAS_KS + 4);
+      const float c0 = __ldg(bias + TC_BIAS_KB + 0), c1 = __ldg(bias + TC_BIAS_KB + 1), c2 = __ldg(bias + TC_BIAS_KB + 2),
+                  c3 = __ldg(bias + TC_BIAS_KB + 3), c4 = __ldg(bias + TC_BIAS_KB + 4);
       // ---- z1 -> h1 = CELU(z1 + b1): operand of phase 1 ----
       tc::mbar_wait(&S.z_full[0], par);
       tc::tc_fence_after();
@@ -339,7 +347,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k0, bb[k]));
+        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k0, fmaf(z[k], c0, bb[k])));
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
@@ -358,7 +366,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k1, bb[k]));
+        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k1, fmaf(z[k], c1, bb[k])));
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
@@ -383,7 +391,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
 #pragma unroll
           for (int k = 0; k < 16; ++k) {
             float h, d;
-            celu_both(fmaf(z[k], k2, bb[k]), h, d);
+            celu_both(fmaf(z[k], k2, fmaf(z[k], c2, bb[k])), h, d);
             epart = fmaf(w4[k], h, epart);
             dl[k] = w4s[k] * d;
           }
@@ -414,7 +422,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) p[k] = (p[k] * k3) * celu_d(fmaf(z[k], k1, bb[k]));
+        for (int k = 0; k < 16; ++k) p[k] = fmaf(p[k], c3, p[k] * k3) * celu_d(fmaf(z[k], k1, fmaf(z[k], c1, bb[k])));
         tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
       }
       publish(&S.dd_full);
@@ -432,7 +440,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) p[k] = (p[k] * k4) * celu_d(fmaf(z[k], k0, bb[k]));
+        for (int k = 0; k < 16; ++k) p[k] = fmaf(p[k], c4, p[k] * k4) * celu_d(fmaf(z[k], k0, fmaf(z[k], c0, bb[k])));
         tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
         publish(&S.d1_full[c]);
       }

@@ -18,6 +18,7 @@
 #include "k1_neighbors.cuh"
 #include "k2_aev.cuh"
 #include "k3_mlp_fp32.cuh"
+#include "k3_mlp_cluster.cuh"
 #include "k3_mlp_tc.cuh"
 #include "k4_forces.cuh"
 #include "k5_verlet.cuh"
@@ -27,6 +28,7 @@ using namespace pfc;
 namespace {
 
 constexpr size_t ALIGN = 256;
+constexpr int CALIB_NSTAT = 6;                // calibration, per 128-row block: sum e^2, sum de e, sum g^2, sum dg g, max|de|, max|dg|
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 // per-element FFMA weight block on the device (floats): packed phase images, then b1 b2 b3 w4 b4
@@ -63,13 +65,16 @@ struct Buffers {
   int2 *cnt, *block_tot;
   int *r_off, *a_off, *r_idx, *a_idx;   // CSR export (pfc_get_neighbors only)
   float *aev, *g, *e_row;       // aev: fp32 rows (FP32 MLP) or the packed fp16 operand image (tensor MLP), same bytes
-  float* aev_unpacked;          // pfc_get_intermediates on the tensor path
+  float* aev_unpacked;          // pfc_get_intermediates on the tensor path; calibration: fp32 AEV rows, then the FP32 MLP's g
+  float* e_ref;                 // calibration: the FP32 MLP's per-row energies
+  double* calib_part;           // calibration: per 128-row block partial sums
   float4 *edge, *self, *xlo;
   uint32_t* status;
   StepParams* sp;
   unsigned long long* work;     // pfc_work_counts
   long long* trace;             // pfc_k3_timeline
   float* weights;
+  float* wcl;                   // cluster MLP (single small molecule): per element and cluster rank, the six weight slices
   uint8_t* wtc;                 // tensor-core path: packed hi|lo swizzled weight chunks
   float* bias_tc;
   // cell list
@@ -104,6 +109,8 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.g = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.aev_unpacked = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.e_row = c.take<float>((size_t)s.n_rows);
+  t.e_ref = c.take<float>((size_t)s.n_rows);
+  t.calib_part = c.take<double>((size_t)(s.n_rows / ROW_PAD) * CALIB_NSTAT);
   t.edge = c.take<float4>((size_t)s.cap_r);
   t.self = c.take<float4>(N);
   t.xlo = c.take<float4>(N);
@@ -112,6 +119,7 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.work = c.take<unsigned long long>(8);
   t.trace = c.take<long long>((size_t)TC_TRACE_STRIDE * TC_TRACE_ITERS);
   t.weights = c.take<float>((size_t)NSPEC * DEV_W_PER_ELEM);
+  t.wcl = c.take<float>((size_t)NSPEC * CL_SIZE * CL_W_FLOATS);
   t.wtc = c.take<uint8_t>((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
   t.bias_tc = c.take<float>((size_t)NSPEC * TC_BIAS_LEN);
   t.cell_sys = c.take<int>((size_t)s.n_cell_sys + 1);
@@ -135,7 +143,11 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
 
 inline int cells_for(int n_sys_atoms) { return n_sys_atoms + 64 + 1; }
 // default scale of the tensor-core MLP's truncation compensation, forward / backward phases
-constexpr float TC_LAMBDA_FWD = 1.0f, TC_LAMBDA_BWD = 1.0f;
+constexpr float TC_LAMBDA_FWD = 0.85f, TC_LAMBDA_BWD = 0.85f;   // uncalibrated elements (fewer than CALIB_MIN_ROWS atoms)
+constexpr int CALIB_MIN_ROWS = 256;           // atoms of an element below which its lambdas stay at the defaults
+// a calibrated element keeps the tensor path only if, against the FP32 MLP on the same batch, the least-squares
+// slopes of its e_i and g errors and its largest errors (relative to the rms of e_i / g) stay below these
+constexpr double CALIB_MAX_SLOPE = 3e-7, CALIB_MAX_DE = 1e-4, CALIB_MAX_DG = 5e-5;
 constexpr int ROW_CAP = 192;                  // neighbour-row capacity of an atom: min(ROW_CAP, N_sys - 1); bulk at 0.1 / A^3 has 59
 constexpr int K1_MIN_BLOCK = 8, K1_MAX_BLOCK = 64;   // atoms per K1 brute-force work item
 
@@ -173,9 +185,21 @@ struct pfc_ctx {
   Sizes sz;
   Buffers b;
   MlpParams mlp;
+  ClParams clp;
+  bool mlp_cluster = false;     // FP32 MLP of a batch of <= CL_MAX_TILES 16-row tiles: one cluster of 8 CTAs per tile
   TcParams tcp;
   int device = 0;               // the CUDA device the handle was created on
   int mlp_path;
+  int mlp_requested = PFC_MLP_AUTO;
+  // tensor-core MLP: truncation compensation
+  std::vector<float> bias_host;               // host copy of the per-element tables (ks / kb are rewritten)
+  int tc_inv_scale[NSPEC][6] = {};
+  int tc_terms = 3;
+  int count[NSPEC] = {0, 0, 0, 0};
+  bool tc_calibrated = false;                 // lambdas final (calibrated, or fixed by pfc_tuning_t)
+  float tc_lambda[NSPEC][2];                  // forward / backward
+  float tc_resid[NSPEC][4] = {};              // after calibration: slope e, slope g, max|de|/rms e, max|dg|/rms g
+  int tc_fallback = 0;                        // 1: AUTO went back to the FP32 MLP because an element failed the check
   int mlp_tm = 128;             // FFMA K3 tile height
   bool mlp_deep = false;        // FFMA K3 staging: 8-stage mbarrier ring (few tiles per SM) or two buffers
   int n_sms = 148;
@@ -218,15 +242,9 @@ inline bool on_device(const pfc_ctx* c) {      // every call must run with the h
   return cudaGetDevice(&dev) == cudaSuccess && dev == c->device;
 }
 
-// K1..K4 + energy sum on `st`
-// `ev` (optional): PFC_N_STAGES+1 events recorded at the stage boundaries K1|K2|K3|K4a|K4b|E-sum
-void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool with_xlo, cudaStream_t st,
-                    cudaEvent_t* ev = nullptr) {
-  auto mark = [&](int k) { if (ev) cudaEventRecord(ev[k], st); };
-  mark(0);
-  const Sizes& s = c->sz;
+// K1: neighbour rows of `pos` (and the packed position copies every later kernel reads)
+void enqueue_k1(pfc_ctx* c, const float4* pos, bool with_xlo, cudaStream_t st) {
   const Buffers& b = c->b;
-  const int N = s.n_atoms;
   // the low position words belong to the bound MD state only
   const float4* xlo = with_xlo ? b.xlo : nullptr;
   if (c->n_items > 0)
@@ -246,36 +264,69 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool wit
            b.atom_cell_sys, b.atom_cell, pos, b.species, xlo, b.grids, b.cell_start, b.cell_xyz, b.xs, b.xsl,
            b.row_beg, b.nbr, b.cnt, b.status);
   }
-  mark(1);
-  if (c->mlp_path == PFC_MLP_FP32)
+}
+
+// K2 into `aev`: fp32 rows (PACK16 false) or the tensor MLP's first operand image
+void enqueue_k2(pfc_ctx* c, bool pack16, float* aev, cudaStream_t st) {
+  const Buffers& b = c->b;
+  const int N = c->sz.n_atoms;
+  if (!pack16)
     LAUNCH(c, k2_aev_fwd_kernel<false>, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
-           b.row_of_atom, b.aev, b.status);
+           b.row_of_atom, aev, b.status);
   else                                                    // the tensor MLP's first operand, as it sits in shared memory
     LAUNCH(c, k2_aev_fwd_kernel<true>, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
-           b.row_of_atom, b.aev, b.status);
-  mark(2);
-  if (c->mlp_path == PFC_MLP_FP32) {
+           b.row_of_atom, aev, b.status);
+}
+
+// K3, FP32 FFMA: tile height and staging chosen by pfc_create.  `g` may be `aev` (a tile's AEV rows are
+// consumed in its first phase, long before its g rows are written)
+void enqueue_k3_fp32(pfc_ctx* c, const float* aev, float* g, float* e_row, cudaStream_t st) {
+  const Sizes& s = c->sz;
+  if (c->mlp_cluster) {
+    LAUNCH(c, k3_mlp_cluster_kernel, c->clp.n_tiles * CL_SIZE, CL_THREADS, CL_SMEM_BYTES, st, c->clp, aev, g, e_row);
+    return;
+  }
 #define K3_LAUNCH(TM_, DEEP_)                                                                          \
   LAUNCH(c, (k3_mlp_fp32_kernel<TM_, DEEP_>), s.n_rows / TM_, (MlpCfg<TM_, DEEP_>::THREADS),             \
-         (MlpCfg<TM_, DEEP_>::SMEM), st, c->mlp, b.aev, b.g, b.e_row)
-    if (c->mlp_deep) {                                   // tile height and staging chosen by pfc_create
-      if (c->mlp_tm == 32) K3_LAUNCH(32, true); else K3_LAUNCH(16, true);
-    } else {
-      switch (c->mlp_tm) {
-        case 128: K3_LAUNCH(128, false); break;
-        case 64:  K3_LAUNCH(64, false); break;
-        case 32:  K3_LAUNCH(32, false); break;
-        default:  K3_LAUNCH(16, false); break;
-      }
-    }
-#undef K3_LAUNCH
+         (MlpCfg<TM_, DEEP_>::SMEM), st, c->mlp, aev, g, e_row)
+  if (c->mlp_deep) {
+    if (c->mlp_tm == 32) K3_LAUNCH(32, true); else K3_LAUNCH(16, true);
   } else {
-    const int grid = c->tcp.n_tiles < c->n_sms ? c->tcp.n_tiles : c->n_sms;   // persistent: one CTA per SM
-    if (c->mlp_path == PFC_MLP_TENSOR)
-      LAUNCH(c, k3_mlp_tc_kernel<3>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, (const uint8_t*)b.aev, b.g, b.e_row);
-    else
-      LAUNCH(c, k3_mlp_tc_kernel<1>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, (const uint8_t*)b.aev, b.g, b.e_row);
+    switch (c->mlp_tm) {
+      case 128: K3_LAUNCH(128, false); break;
+      case 64:  K3_LAUNCH(64, false); break;
+      case 32:  K3_LAUNCH(32, false); break;
+      default:  K3_LAUNCH(16, false); break;
+    }
   }
+#undef K3_LAUNCH
+}
+
+// K3, tcgen05: persistent, one CTA per SM
+void enqueue_k3_tc(pfc_ctx* c, cudaStream_t st) {
+  const Buffers& b = c->b;
+  const int grid = c->tcp.n_tiles < c->n_sms ? c->tcp.n_tiles : c->n_sms;
+  if (c->tc_terms == 3)
+    LAUNCH(c, k3_mlp_tc_kernel<3>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, (const uint8_t*)b.aev, b.g, b.e_row);
+  else
+    LAUNCH(c, k3_mlp_tc_kernel<1>, grid, TC_THREADS, TC_SMEM_BYTES, st, c->tcp, (const uint8_t*)b.aev, b.g, b.e_row);
+}
+
+// K1..K4 + energy sum on `st`
+// `ev` (optional): events recorded at the seven stage boundaries K1|K2|K3|K4a|K4b|E-sum|
+void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool with_xlo, cudaStream_t st,
+                    cudaEvent_t* ev = nullptr) {
+  auto mark = [&](int k) { if (ev) cudaEventRecord(ev[k], st); };
+  mark(0);
+  const Sizes& s = c->sz;
+  const Buffers& b = c->b;
+  const int N = s.n_atoms;
+  enqueue_k1(c, pos, with_xlo, st);
+  mark(1);
+  enqueue_k2(c, c->mlp_path != PFC_MLP_FP32, b.aev, st);
+  mark(2);
+  if (c->mlp_path == PFC_MLP_FP32) enqueue_k3_fp32(c, b.aev, b.g, b.e_row, st);
+  else enqueue_k3_tc(c, st);
   mark(3);
   LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
          b.row_of_atom, b.g, b.edge, b.self);
@@ -286,6 +337,140 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool wit
   if (c->n_cell_sys > 0) LAUNCH(c, k_energy_sum_kernel<1024>, s.n_systems, 1024, 0, st, b.sys_off, F, E, b.status);
   else LAUNCH(c, k_energy_sum_kernel<128>, s.n_systems, 128, 0, st, b.sys_off, F, E, b.status);
   mark(6);
+}
+
+// ---- truncation compensation of the tensor-core MLP ----------------------
+// ks[q] = 2^-(operand scales of epilogue q), kb[q] = beta_q ks[q], beta_q = lambda n_q 2.15e-8 with n_q the
+// MMA instructions of the accumulator chain and lambda = tc_lambda[e][q < 3 ? 0 : 1]
+int upload_tc_factors(pfc_ctx* c, cudaStream_t st) {
+  for (int e = 0; e < NSPEC; ++e) {
+    float* bt = c->bias_host.data() + (size_t)e * TC_BIAS_LEN;
+    for (int q = 0; q < 6; ++q) {
+      const float beta = c->tc_lambda[e][q < 3 ? 0 : 1] * (float)tc_chain_mmas(q, c->tc_terms) * 2.15e-8f;
+      bt[TC_BIAS_KS + q] = ldexpf(1.0f, c->tc_inv_scale[e][q]);
+      bt[TC_BIAS_KB + q] = ldexpf(beta, c->tc_inv_scale[e][q]);
+    }
+    if (cudaMemcpyAsync(c->b.bias_tc + (size_t)e * TC_BIAS_LEN + TC_BIAS_KS, bt + TC_BIAS_KS, sizeof(float) * 12,
+                        cudaMemcpyHostToDevice, st) != cudaSuccess)
+      return PFC_ERR_CUDA;
+  }
+  return PFC_OK;
+}
+
+// per 128-row block (one element): sums over its real rows of the FP32 MLP's outputs (ref) and the
+// differences of the tensor MLP's outputs to them; fixed order, one owner per partial
+__global__ void __launch_bounds__(256)
+k_calib_stats_kernel(const __grid_constant__ MlpParams P, const float* __restrict__ g_ref, const float* __restrict__ g_tc,
+                     const float* __restrict__ e_ref, const float* __restrict__ e_tc, double* __restrict__ part) {
+  __shared__ double sh[8][CALIB_NSTAT];
+  const int row0 = blockIdx.x * ROW_PAD, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int el = 0;
+#pragma unroll
+  for (int k = 1; k < NSPEC; ++k) el += (row0 >= P.row_start[k]);
+  const int rend = min(row0 + ROW_PAD, P.row_end[el]);
+  double see = 0.0, sde = 0.0, sgg = 0.0, sdg = 0.0, mde = 0.0, mdg = 0.0;
+  for (int r = row0 + warp; r < rend; r += 8) {
+    for (int col = lane; col < AEV_LEN; col += 32) {
+      const float a = g_ref[(size_t)r * AEV_LEN + col], d = g_tc[(size_t)r * AEV_LEN + col] - a;
+      sgg += (double)a * a; sdg += (double)d * a; mdg = fmax(mdg, (double)fabsf(d));
+    }
+    if (lane == 0) {
+      const float a = e_ref[r], d = e_tc[r] - a;
+      see += (double)a * a; sde += (double)d * a; mde = fmax(mde, (double)fabsf(d));
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    see += __shfl_xor_sync(0xffffffffu, see, o); sde += __shfl_xor_sync(0xffffffffu, sde, o);
+    sgg += __shfl_xor_sync(0xffffffffu, sgg, o); sdg += __shfl_xor_sync(0xffffffffu, sdg, o);
+    mde = fmax(mde, __shfl_xor_sync(0xffffffffu, mde, o)); mdg = fmax(mdg, __shfl_xor_sync(0xffffffffu, mdg, o));
+  }
+  if (lane == 0) { sh[warp][0] = see; sh[warp][1] = sde; sh[warp][2] = sgg; sh[warp][3] = sdg; sh[warp][4] = mde; sh[warp][5] = mdg; }
+  __syncthreads();
+  if (threadIdx.x < CALIB_NSTAT) {
+    double v = sh[0][threadIdx.x];
+    for (int w = 1; w < 8; ++w) v = threadIdx.x < 4 ? v + sh[w][threadIdx.x] : fmax(v, sh[w][threadIdx.x]);
+    part[(size_t)blockIdx.x * CALIB_NSTAT + threadIdx.x] = v;
+  }
+}
+
+// Calibrates the two compensation scales of every element on the batch at `pos` against the
+// library's own FP32 MLP (never the oracle): K1, K2 (fp32 rows), FP32 MLP -> reference e_i, g; K2 (operand
+// image), then the tensor MLP with (lambda_f, lambda_b) = (0,0), (1,0), (0,1): the error slopes are linear in
+// both, solved per element; one more run checks the result.  With PFC_MLP_AUTO an element that misses the
+// check sends the whole handle back to the FP32 MLP.  Synchronises `st` (first use of a handle only).
+int calibrate_tc(pfc_ctx* c, const float4* pos, bool with_xlo, cudaStream_t st) {
+  const Buffers& b = c->b;
+  const int n_blocks = c->sz.n_rows / ROW_PAD;
+  enqueue_k1(c, pos, with_xlo, st);
+  enqueue_k2(c, false, b.aev_unpacked, st);
+  enqueue_k3_fp32(c, b.aev_unpacked, b.aev_unpacked, b.e_ref, st);
+  enqueue_k2(c, true, b.aev, st);
+  std::vector<double> part((size_t)n_blocks * CALIB_NSTAT);
+  struct Stat { double see = 0, sde = 0, sgg = 0, sdg = 0, mde = 0, mdg = 0; };
+  auto run = [&](Stat* out) -> int {
+    int rc = upload_tc_factors(c, st);
+    if (rc != PFC_OK) return rc;
+    enqueue_k3_tc(c, st);
+    LAUNCH(c, k_calib_stats_kernel, n_blocks, 256, 0, st, c->mlp, b.aev_unpacked, b.g, b.e_ref, b.e_row, b.calib_part);
+    if (cudaMemcpyAsync(part.data(), b.calib_part, sizeof(double) * part.size(), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+      return PFC_ERR_CUDA;
+    for (int e = 0; e < NSPEC; ++e) {
+      Stat t;
+      for (int blk = c->mlp.row_start[e] / ROW_PAD; blk < c->mlp.row_start[e + 1] / ROW_PAD; ++blk) {   // fixed order
+        const double* p = part.data() + (size_t)blk * CALIB_NSTAT;
+        t.see += p[0]; t.sde += p[1]; t.sgg += p[2]; t.sdg += p[3];
+        t.mde = p[4] > t.mde ? p[4] : t.mde; t.mdg = p[5] > t.mdg ? p[5] : t.mdg;
+      }
+      out[e] = t;
+    }
+    return PFC_OK;
+  };
+  auto set_all = [&](float lf, float lb) {
+    for (int e = 0; e < NSPEC; ++e)
+      if (c->count[e] >= CALIB_MIN_ROWS) { c->tc_lambda[e][0] = lf; c->tc_lambda[e][1] = lb; }
+  };
+  Stat s00[NSPEC], s10[NSPEC], s01[NSPEC], fin[NSPEC];
+  int rc;
+  set_all(0.f, 0.f); if ((rc = run(s00)) != PFC_OK) return rc;
+  set_all(1.f, 0.f); if ((rc = run(s10)) != PFC_OK) return rc;
+  set_all(0.f, 1.f); if ((rc = run(s01)) != PFC_OK) return rc;
+  auto slope = [](double sd, double ss) { return ss > 0.0 ? sd / ss : 0.0; };
+  auto clamp = [](double v) { return !(v >= 0.0) ? 0.0 : v > 2.5 ? 2.5 : v; };
+  for (int e = 0; e < NSPEC; ++e) {
+    if (c->count[e] < CALIB_MIN_ROWS) continue;
+    const double e0 = slope(s00[e].sde, s00[e].see), e1 = slope(s10[e].sde, s10[e].see);
+    const double g0 = slope(s00[e].sdg, s00[e].sgg), g1 = slope(s10[e].sdg, s10[e].sgg), g2 = slope(s01[e].sdg, s01[e].sgg);
+    const double lf = fabs(e1 - e0) > 1e-9 ? clamp(-e0 / (e1 - e0)) : TC_LAMBDA_FWD;
+    const double lb = fabs(g2 - g0) > 1e-9 ? clamp(-(g0 + (g1 - g0) * lf) / (g2 - g0)) : TC_LAMBDA_BWD;
+    c->tc_lambda[e][0] = (float)lf; c->tc_lambda[e][1] = (float)lb;
+  }
+  if ((rc = run(fin)) != PFC_OK) return rc;
+  bool ok = true;
+  for (int e = 0; e < NSPEC; ++e) {
+    if (c->count[e] < CALIB_MIN_ROWS) continue;
+    const double n = (double)c->count[e];
+    const double rms_e = sqrt(fin[e].see / n), rms_g = sqrt(fin[e].sgg / (n * AEV_LEN));
+    c->tc_resid[e][0] = (float)slope(fin[e].sde, fin[e].see);
+    c->tc_resid[e][1] = (float)slope(fin[e].sdg, fin[e].sgg);
+    c->tc_resid[e][2] = (float)(rms_e > 0.0 ? fin[e].mde / rms_e : 0.0);
+    c->tc_resid[e][3] = (float)(rms_g > 0.0 ? fin[e].mdg / rms_g : 0.0);
+    if (!(fabs(c->tc_resid[e][0]) <= CALIB_MAX_SLOPE) || !(fabs(c->tc_resid[e][1]) <= CALIB_MAX_SLOPE) ||
+        !(c->tc_resid[e][2] <= CALIB_MAX_DE) || !(c->tc_resid[e][3] <= CALIB_MAX_DG))
+      ok = false;
+  }
+  c->tc_calibrated = true;
+  if (!ok && c->mlp_requested == PFC_MLP_AUTO) {          // this weight set / batch is not for the tensor path
+    c->mlp_path = PFC_MLP_FP32;
+    c->tc_fallback = 1;
+  }
+  return PFC_OK;
+}
+
+inline int ensure_calibrated(pfc_ctx* c, const float4* pos, bool with_xlo, cudaStream_t st) {
+  if (c->mlp_path == PFC_MLP_FP32 || c->tc_calibrated) return PFC_OK;
+  return calibrate_tc(c, pos, with_xlo, st);
 }
 
 template <int MODE>
@@ -365,7 +550,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
       tun.k3_tile_rows != 128)
     return PFC_ERR_ARG;
   if (tun.k3_deep_ring < 0 || tun.k3_deep_ring > 2 || tun.steps_per_graph < 0 || tun.steps_per_graph > 256 ||
-      tun.reserved[0] != 0 || tun.reserved[1] != 0)
+      tun.k3_cluster < 0 || tun.k3_cluster > 2 || tun.reserved != 0)
     return PFC_ERR_ARG;
 
   pfc_ctx* c = new (std::nothrow) pfc_ctx();
@@ -376,7 +561,9 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   // SMs.  Measured ms/step, FFMA vs tensor, replicas of config 1: 2,200 atoms 0.108 / 0.111, 3,960
   // 0.113 / 0.115, 4,840 0.136 / 0.121, 5,632 0.139 / 0.124; of config 4: 3,758 atoms 0.143 / 0.145,
   // 4,749 0.163 / 0.147; config 2 (1,500 atoms) 0.111 / 0.141
+  c->mlp_requested = d->mlp_path;
   c->mlp_path = d->mlp_path == PFC_MLP_AUTO ? (d->n_atoms >= 4096 ? PFC_MLP_TENSOR : PFC_MLP_FP32) : d->mlp_path;
+  for (int e = 0; e < NSPEC; ++e) c->count[e] = count[e];
   c->sz = worst_case_sizes(N, NS);                      // capacities are the worst-case ones
   // static element grouping: rows sorted by element, blocks padded to ROW_PAD
   int row_start[NSPEC + 1];
@@ -460,12 +647,49 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   }
   for (int e = 0; e <= NSPEC; ++e) c->mlp.row_start[e] = row_start[e];
 
+  // cluster MLP (k3_mlp_cluster.cuh): per element and cluster rank r, the column slices [k][nc] of the six
+  // phases back to back; and the table of 16-row tiles that hold real rows
+  std::vector<float> wcl((size_t)NSPEC * CL_SIZE * CL_W_FLOATS);
+  for (int e = 0; e < NSPEC; ++e) {
+    const float* src = d->weights + (size_t)e * W_PER_ELEM;
+    const float *W1 = src, *W2 = W1 + D1 * D0 + D1, *W3 = W2 + D2 * D1 + D2;
+    for (int r = 0; r < CL_SIZE; ++r) {
+      float* o = wcl.data() + ((size_t)e * CL_SIZE + r) * CL_W_FLOATS;
+      for (int k = 0; k < D0; ++k) for (int cc = 0; cc < CL_NC0; ++cc) o[CL_W0 + k * CL_NC0 + cc] = W1[(r * CL_NC0 + cc) * D0 + k];
+      for (int k = 0; k < D1; ++k) for (int cc = 0; cc < CL_NC1; ++cc) o[CL_W1 + k * CL_NC1 + cc] = W2[(r * CL_NC1 + cc) * D1 + k];
+      for (int k = 0; k < D2; ++k) for (int cc = 0; cc < CL_NC2; ++cc) o[CL_W2 + k * CL_NC2 + cc] = W3[(r * CL_NC2 + cc) * D2 + k];
+      for (int k = 0; k < D3; ++k) for (int cc = 0; cc < CL_NC3; ++cc) o[CL_W3 + k * CL_NC3 + cc] = W3[k * D2 + r * CL_NC3 + cc];
+      for (int k = 0; k < D2; ++k) for (int cc = 0; cc < CL_NC4; ++cc) o[CL_W4 + k * CL_NC4 + cc] = W2[k * D1 + r * CL_NC4 + cc];
+      for (int k = 0; k < D1; ++k) for (int cc = 0; cc < CL_NC5; ++cc) o[CL_W5 + k * CL_NC5 + cc] = W1[k * D0 + r * CL_NC5 + cc];
+    }
+    c->clp.vec[e] = c->mlp.vec[e];
+  }
+  c->clp.wcl = b.wcl;
+  {
+    int nt = 0;
+    for (int e = 0; e < NSPEC; ++e) nt += (count[e] + CL_TM - 1) / CL_TM;
+    // one wave of clusters: config 0 (22 atoms, 4 tiles) 37 -> ~10 us; beyond CL_MAX_TILES the one-CTA-per-tile
+    // kernel's better per-SM efficiency wins (config 2 would need 95 clusters = 5 waves)
+    c->mlp_cluster = nt <= CL_MAX_TILES && tun.k3_cluster != 1 && tun.k3_tile_rows == 0 && tun.k3_deep_ring == 0;
+    if (tun.k3_cluster == 2 && nt > CL_MAX_TILES) { delete c; return PFC_ERR_ARG; }
+    if (tun.k3_cluster == 2) c->mlp_cluster = true;
+    c->clp.n_tiles = 0;
+    if (c->mlp_cluster)
+      for (int e = 0; e < NSPEC; ++e)
+        for (int t = 0; t * CL_TM < count[e]; ++t) {
+          const int q = c->clp.n_tiles++;
+          c->clp.row0[q] = row_start[e] + t * CL_TM;
+          c->clp.elem[q] = e;
+          c->clp.rows[q] = count[e] - t * CL_TM < CL_TM ? count[e] - t * CL_TM : CL_TM;
+        }
+  }
+
   // tensor-core path: per element, the B operand of every phase chunk exactly as it sits in
   // shared memory -- [N rows x 32 k] fp16, K-major, SWIZZLE_64B, hi block then lo block -- with every
   // weight matrix scaled by the power of two that puts max|W| into [256, 512) (k3_mlp_tc.cuh)
   std::vector<uint8_t> wtc((size_t)NSPEC * TC_W_BYTES_PER_ELEM);
   std::vector<float> bias_tc((size_t)NSPEC * TC_BIAS_LEN, 0.0f);
-  const int n_terms = c->mlp_path == PFC_MLP_TENSOR_1TERM ? 1 : 3;
+  c->tc_terms = c->mlp_path == PFC_MLP_TENSOR_1TERM ? 1 : 3;
   for (int e = 0; e < NSPEC; ++e) {
     const float* src = d->weights + (size_t)e * W_PER_ELEM;
     const float *W1 = src, *b1 = W1 + D1 * D0, *W2 = b1 + D1, *b2 = W2 + D2 * D1, *W3 = b2 + D2,
@@ -512,21 +736,22 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
     memcpy(bt + TC_BIAS_W4, W4, sizeof(float) * D3);
     bt[TC_BIAS_B4] = b4[0];
     for (int k = 0; k < D3; ++k) bt[TC_BIAS_W4S + k] = ldexpf(W4[k], eD);
-    // epilogue factors: (1 + beta_q) times the inverse operand scales; beta_q = lambda n_q 2.15e-8 is the
-    // expected relative truncation loss of a chain of n_q MMA instructions (pfc_tuning_t.tc_comp_* scale it)
-    const float lf = tun.tc_comp_override ? tun.tc_comp_forward : TC_LAMBDA_FWD;
-    const float lb = tun.tc_comp_override ? tun.tc_comp_backward : TC_LAMBDA_BWD;
+    // epilogue factors (upload_tc_factors): inverse operand scales and the truncation compensation.  The
+    // compensation scales start at the defaults and are calibrated on the handle's first batch
+    // (calibrate_tc) unless pfc_tuning_t fixes them
     const int inv_scale[6] = {-(TC_AEV_SCALE_LOG2 + eW1), -eW2, -eW3, -eW3, -eW2, -(eW1 + eD)};
-    for (int q = 0; q < 6; ++q) {
-      const float beta = (q < 3 ? lf : lb) * (float)tc_chain_mmas(q, n_terms) * 2.15e-8f;
-      bt[TC_BIAS_KF + q] = ldexpf(1.0f + beta, inv_scale[q]);
-    }
+    for (int q = 0; q < 6; ++q) c->tc_inv_scale[e][q] = inv_scale[q];
+    c->tc_lambda[e][0] = tun.tc_comp_override ? tun.tc_comp_forward : TC_LAMBDA_FWD;
+    c->tc_lambda[e][1] = tun.tc_comp_override ? tun.tc_comp_backward : TC_LAMBDA_BWD;
     c->tcp.bias[e] = c->b.bias_tc + (size_t)e * TC_BIAS_LEN;
   }
   c->tcp.wpack = c->b.wtc;
   for (int e = 0; e <= NSPEC; ++e) c->tcp.row_start[e] = row_start[e];
   c->tcp.n_tiles = c->sz.n_rows / TC_TM;
   c->tcp.trace = nullptr;
+  c->bias_host = bias_tc;
+  // fixed by the caller, or a path that is evidence only: nothing to calibrate
+  c->tc_calibrated = tun.tc_comp_override != 0 || c->mlp_path == PFC_MLP_TENSOR_1TERM;
 
   StepParams sp0{};
   {
@@ -548,8 +773,10 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   up(b.sys_off, d->sys_offsets, sizeof(int) * (NS + 1));
   up(b.row_of_atom, row_of_atom.data(), sizeof(int) * N);
   up(b.weights, w.data(), sizeof(float) * w.size());
+  up(b.wcl, wcl.data(), sizeof(float) * wcl.size());
   up(b.wtc, wtc.data(), wtc.size());
   up(b.bias_tc, bias_tc.data(), sizeof(float) * bias_tc.size());
+  if (upload_tc_factors(c, nullptr) != PFC_OK) ok = false;
   up(b.cell_sys, cell_sys.data(), sizeof(int) * cell_sys.size());
   up(b.cell_cap_base, cell_cap_base.data(), sizeof(int) * cell_cap_base.size());
   up(b.cell_slot_base, cell_slot_base.data(), sizeof(int) * cell_slot_base.size());
@@ -557,6 +784,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   up(b.atom_cell_sys, atom_cell_sys.data(), sizeof(int) * atom_cell_sys.size());
   // padded AEV rows are never written by K2: zero everything once
   if (cudaMemset(b.aev, 0, sizeof(float) * (size_t)c->sz.n_rows * AEV_LEN) != cudaSuccess) ok = false;
+  if (cudaMemset(b.aev_unpacked, 0, sizeof(float) * (size_t)c->sz.n_rows * AEV_LEN) != cudaSuccess) ok = false;
   if (cudaMemset(b.status, 0, 256) != cudaSuccess) ok = false;
   if (cudaMemset(b.work, 0, 64) != cudaSuccess) ok = false;
   if (c->k1_smem > 48 * 1024 &&
@@ -569,6 +797,8 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   K3_SMEM_ATTR(128, false); K3_SMEM_ATTR(64, false); K3_SMEM_ATTR(32, false); K3_SMEM_ATTR(16, false);
   K3_SMEM_ATTR(32, true); K3_SMEM_ATTR(16, true);
 #undef K3_SMEM_ATTR
+  if (cudaFuncSetAttribute(k3_mlp_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)CL_SMEM_BYTES) != cudaSuccess) ok = false;
   if (cudaFuncSetAttribute(k3_mlp_tc_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)TC_SMEM_BYTES) != cudaSuccess) ok = false;
   if (cudaFuncSetAttribute(k3_mlp_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -632,6 +862,8 @@ int pfc_energy_forces(pfc_t* c, const float* pos, float* E, float* F, void* stre
   cudaStream_t st = (cudaStream_t)stream;
   // the low position words belong to the bound MD state only
   const bool with_xlo = c->bound && (const float4*)pos == c->pos;
+  int rc0 = ensure_calibrated(c, (const float4*)pos, with_xlo, st);
+  if (rc0 != PFC_OK) return rc0;
   cudaGraphExec_t g = nullptr;
   const int rc = ef_graph(c, (const float4*)pos, E, (float4*)F, with_xlo, &g);
   if (rc != PFC_OK) return rc;
@@ -648,6 +880,8 @@ int pfc_energy_forces_nm(pfc_t* c, const float* pos_nm, float* E_kj, float* F_kj
   const int N = c->sz.n_atoms, NS = c->sz.n_systems;
   Buffers& b = c->b;
   k0_pack_nm_kernel<<<cdiv(N, K0_THREADS), K0_THREADS, 0, st>>>(N, pos_nm, b.h_pos);
+  int rc0 = ensure_calibrated(c, b.h_pos, false, st);
+  if (rc0 != PFC_OK) return rc0;
   cudaGraphExec_t g = nullptr;
   const int rc = ef_graph(c, b.h_pos, b.h_E, b.h_frc, false, &g);
   if (rc != PFC_OK) return rc;
@@ -664,7 +898,18 @@ int pfc_profile_stages(pfc_t* c, const float* pos, float* E, float* F, void* str
   cudaEvent_t ev[PFC_N_STAGES + 1];
   for (int k = 0; k <= PFC_N_STAGES; ++k)
     if (cudaEventCreate(&ev[k]) != cudaSuccess) return PFC_ERR_CUDA;
+  {
+    const int rc0 = ensure_calibrated(c, (const float4*)pos, c->bound && (const float4*)pos == c->pos, st);
+    if (rc0 != PFC_OK) return rc0;
+  }
   enqueue_forces(c, (const float4*)pos, E, (float4*)F, c->bound && (const float4*)pos == c->pos, st, ev);
+  // stage 6: the fused integrator kernel of a steady-state step (kick + kick + drift), timed on the library's
+  // staging buffers so that no caller state moves (their contents do not matter for the time; `self` is free
+  // between two force evaluations and stands in for the low position words)
+  if (!c->bound || c->pos != c->b.h_pos)
+    LAUNCH(c, k5_verlet_kernel<2>, cdiv(c->sz.n_atoms, K5_THREADS), K5_THREADS, 0, st, c->sz.n_atoms, c->b.sp,
+           c->b.species, (const float4*)F, c->b.h_pos, c->b.h_vel, c->b.self);
+  cudaEventRecord(ev[PFC_N_STAGES], st);
   int rc = cudaStreamSynchronize(st) == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
   for (int k = 0; k < PFC_N_STAGES && rc == PFC_OK; ++k)
     if (cudaEventElapsedTime(&ms[k], ev[k], ev[k + 1]) != cudaSuccess) rc = PFC_ERR_CUDA;
@@ -760,6 +1005,7 @@ static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
   cudaStream_t st = c->stream;
   int rc;
   const int kind = langevin ? 2 : 1;
+  if ((rc = ensure_calibrated(c, c->pos, true, st)) != PFC_OK) return rc;   // before anything is captured
   if (!c->g_forces && (rc = capture(c, 0, 1, c->pos, c->E, c->frc, true, &c->g_forces)) != PFC_OK) return rc;
   cudaGraphExec_t* g1 = langevin ? &c->g_lstep : &c->g_step;
   cudaGraphExec_t* gk = langevin ? &c->g_lstepk : &c->g_stepk;
@@ -917,6 +1163,17 @@ int pfc_status(pfc_t* c, uint32_t* bits) {
   if (!on_device(c)) return PFC_ERR_STATE;
   if (cudaStreamSynchronize(c->stream) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpy(bits, c->b.status, sizeof(uint32_t), cudaMemcpyDeviceToHost) != cudaSuccess) return PFC_ERR_CUDA;
+  return PFC_OK;
+}
+
+int pfc_tc_calibration(pfc_t* c, float* out) {
+  if (!c || !out) return PFC_ERR_ARG;
+  for (int e = 0; e < NSPEC; ++e) {
+    out[8 * e + 0] = c->tc_lambda[e][0]; out[8 * e + 1] = c->tc_lambda[e][1];
+    for (int k = 0; k < 4; ++k) out[8 * e + 2 + k] = c->tc_resid[e][k];
+    out[8 * e + 6] = c->tc_calibrated ? 1.0f : 0.0f;
+    out[8 * e + 7] = (float)c->tc_fallback;
+  }
   return PFC_OK;
 }
 

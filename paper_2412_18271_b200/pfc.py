@@ -29,15 +29,15 @@ STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
                4: "angular row longer than PFC_MAX_ANGULAR", 8: "non-finite energy",
                16: "cell grid overflow"}
 
-N_STAGES = 6
-STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum")
+N_STAGES = 7
+STAGE_NAMES = ("K1_neighbors", "K2_aev_fwd", "K3_mlp", "K4a_aev_bwd", "K4b_gather", "energy_sum", "K5_integrate")
 
 # include/pfc.h (the provider boundary) and include/pfc_debug.h (measurement / parity helpers)
 EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy_forces_nm", "pfc_set_state",
            "pfc_step", "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host",
            "pfc_run_host_resume", "pfc_get_neighbors", "pfc_get_intermediates", "pfc_status", "pfc_destroy",
            "pfc_error_string")
-DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_k3_timeline", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts")
+DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_k3_timeline", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts", "pfc_tc_calibration")
 
 
 class PfcError(RuntimeError):
@@ -48,7 +48,7 @@ class Tuning(ctypes.Structure):
     """pfc_tuning_t (include/pfc.h): a zero-filled struct is "all defaults"."""
     _fields_ = [("k3_tile_rows", c_int32), ("k3_deep_ring", c_int32), ("tc_comp_override", c_int32),
                 ("tc_comp_forward", c_float), ("tc_comp_backward", c_float), ("steps_per_graph", c_int32),
-                ("reserved", c_int32 * 2)]
+                ("k3_cluster", c_int32), ("reserved", c_int32)]
 
 
 class _Desc(ctypes.Structure):
@@ -93,6 +93,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_copy_to_host.argtypes = [c_void_p, c_void_p, c_size_t]
     lib.pfc_status.argtypes = [c_void_p, POINTER(c_uint32)]
     lib.pfc_mlp_path.argtypes = [c_void_p, POINTER(c_int32)]
+    lib.pfc_tc_calibration.argtypes = [c_void_p, POINTER(c_float)]
     lib.pfc_launch_counts.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32)]
     lib.pfc_destroy.argtypes = [c_void_p]
     lib.pfc_error_string.argtypes = [c_int]
@@ -271,6 +272,12 @@ class Pfc:
         v = c_int32()
         _check(self._lib.pfc_mlp_path(self._h, byref(v)), "pfc_mlp_path")
         return int(v.value)
+
+    def tc_calibration(self):
+        """pfc_tc_calibration: per element {lambda_f, lambda_b, slope_e, slope_g, max_de, max_dg, final, fallback}."""
+        out = (c_float * 32)()
+        _check(self._lib.pfc_tc_calibration(self._h, out), "pfc_tc_calibration")
+        return np.array(out[:], dtype=np.float32).reshape(4, 8)
 
     @_on_device
     def status(self) -> int:

@@ -1,10 +1,10 @@
 #!/usr/bin/env python
-"""Writes tests/golden/cfg4_conditioning.txt: how far the fp64 ORACLE's own 100-step trajectory of
-every config-4 replica moves when its inputs are disturbed at the fp32 rounding level -- the
-conditioning of the 1e-4 A trajectory bar (reading S30).
+"""Writes tests/golden/cfg{1,4}_conditioning.txt: how far the fp64 ORACLE's own 100-step trajectory of
+every replica of config 1 / config 4 moves when its inputs are disturbed at the fp32 rounding level --
+the conditioning of the 1e-4 A trajectory bar (reading S30).
 
 Calls only oracle/ and the seeded generator (tier rule: no stored value comes from the CUDA path).
-For each of the 4,096 replicas of config 4 (BASELINE.json:configs[4]) it integrates 100 steps of
+For each replica (256 of config 1, 4,096 of config 4; BASELINE.json:configs) it integrates 100 steps of
 0.5 fs (O8) from the generator's state, then again from each disturbed state
 
   P1, P2, P3  every initial coordinate moved to the next fp32 value up or down, the signs drawn by
@@ -15,9 +15,10 @@ For each of the 4,096 replicas of config 4 (BASELINE.json:configs[4]) it integra
 
 and records the per-replica RMSD (A) between the disturbed and the undisturbed oracle at step 100.
 No fp32 evaluation of F can be expected to track the fp64 trajectory of a replica closer than
-these distances.  About 22 minutes on 16 cores (five 100-step oracle runs of 227,857 atoms).
+these distances.  Config 4: about 22 minutes on 16 cores (five 100-step oracle runs of 227,857 atoms);
+config 1: under a minute.
 
-  python tests/golden/make_cfg4_conditioning.py [n_replicas]
+  python tests/golden/make_conditioning.py <config: 1 or 4> [n_replicas]
 """
 import os
 import sys
@@ -33,11 +34,12 @@ from paper_2412_18271_b200 import workloads as W                 # noqa: E402
 
 
 def main():
-    n_rep = int(sys.argv[1]) if len(sys.argv) > 1 else 4096
-    out_path = sys.argv[2] if len(sys.argv) > 2 else os.path.join(os.path.dirname(os.path.abspath(__file__)),
-                                                                  "cfg4_conditioning.txt")
+    cfg = int(sys.argv[1]) if len(sys.argv) > 1 else 4
+    assert cfg in (1, 4)
+    n_rep = int(sys.argv[2]) if len(sys.argv) > 2 else (4096 if cfg == 4 else 256)
+    out_path = os.path.join(os.path.dirname(os.path.abspath(__file__)), f"cfg{cfg}_conditioning.txt")
     w = W.make_weights()
-    wl = W.config4(n_replicas=n_rep)
+    wl = W.config4(n_replicas=n_rep) if cfg == 4 else W.config1(n_replicas=n_rep)
     off = wl.sys_offsets
 
     def rmsd(x, y):
@@ -59,7 +61,7 @@ def main():
     print(f"M {time.time() - t0:.0f} s", flush=True)
     names = ("P1", "P2", "P3", "M")
     with open(out_path, "w") as f:
-        f.write("# written by tests/golden/make_cfg4_conditioning.py (oracle only): per-replica RMSD (A) at step 100\n"
+        f.write(f"# written by tests/golden/make_conditioning.py {cfg} (oracle only): per-replica RMSD (A) at step 100\n"
                 "# between the fp64 oracle and the same oracle with inputs disturbed by one fp32 ulp\n"
                 "# replica  n_atoms  P1  P2  P3  M\n")
         for s in range(len(off) - 1):

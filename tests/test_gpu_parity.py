@@ -108,7 +108,30 @@ def test_config3_brute_force_enumeration_matches_cell_path(pfc, weights):
 
 
 # ---- 100-step trajectories -----------------------------------------------------------
-def _trajectory(pfc, weights, wl, n_steps, cell=False, mlp_path=None):
+COND_FACTOR = 4.0     # a replica may miss 1e-4 A only within this factor of its own one-ulp sensitivity (S30)
+
+
+def _conditioning(k):
+    """tests/golden/cfg{k}_conditioning.txt (written by make_conditioning.py from the oracle alone): per
+    replica of config k (1 or 4), how far the fp64 oracle's own 100-step trajectory moves when its inputs
+    are disturbed by one fp32 ulp -- the worst of the recorded disturbances."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"cfg{k}_conditioning.txt")
+    t = np.loadtxt(path)
+    assert np.array_equal(t[:, 0], np.arange(t.shape[0]))
+    return t[:, 1].astype(int), t[:, 2:].max(axis=1)
+
+
+def _trajectory(pfc, weights, wl, n_steps, cell=False, mlp_path=None, cond=None):
+    """cond = config index with a conditioning table (reading S30): the bar of system s is then
+    max(1e-4 A, COND_FACTOR * its one-ulp sensitivity) -- on config 1 that matters for one replica (68),
+    whose fp64 trajectory itself moves by 1.1e-4 A under a one-ulp input error."""
+    floor = np.zeros(wl.n_systems)
+    if cond is not None:
+        sizes, sens = _conditioning(cond)
+        assert np.array_equal(sizes[:wl.n_systems], np.diff(wl.sys_offsets))
+        floor = COND_FACTOR * sens[:wl.n_systems]
+    rel = np.maximum(1.0, floor / RMSD_TOL)                      # 1 wherever the plain bar applies
     p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_AUTO if mlp_path is None else mlp_path)
     pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
     E, F = p.set_state(pos, vel)
@@ -119,7 +142,7 @@ def _trajectory(pfc, weights, wl, n_steps, cell=False, mlp_path=None):
     x = pos.cpu().numpy()[:, :3].astype(np.float64)
     v = vel.cpu().numpy()[:, :3].astype(np.float64)
     rmsd = _rmsd_per_system(x, ref["pos"], wl.sys_offsets)
-    assert rmsd.max() <= RMSD_TOL, rmsd.max()
+    assert (rmsd <= RMSD_TOL * rel).all(), (rmsd / rel).max()
     # velocities: north_star states no bound; DESIGN.md "Tolerances" derives one from the position
     # bound: an error that reaches 1e-4 A while growing with e-folding time tau moves at 1e-4/tau;
     # measured tau >= 2.5 fs (config 3, steps 80-100: 3.4 fs) gives 4e-5 A/fs, taken like the
@@ -127,7 +150,7 @@ def _trajectory(pfc, weights, wl, n_steps, cell=False, mlp_path=None):
     # has no core repulsion; single atoms in a 0.08 A contact at step 100 of config 2 are
     # ill-conditioned).  Thermal H speed is 1.6e-2 A/fs.
     vrms = _rmsd_per_system(v, ref["vel"], wl.sys_offsets)
-    assert vrms.max() <= VEL_TOL, vrms.max()
+    assert (vrms <= VEL_TOL * rel).all(), (vrms / rel).max()
     # synchronous state: F and E are those of the FINAL GPU positions -- checked by evaluating
     # the oracle at exactly those fp32 positions (the paper's frame replay), so the
     # force bound is not blurred by the 1e-6..1e-5 A by which the two trajectories differ
@@ -148,7 +171,7 @@ def test_trajectory_config0(pfc, weights):
 
 
 def test_trajectory_config1_all_256_replicas(pfc, weights):
-    _trajectory(pfc, weights, cfg(1), 100)
+    _trajectory(pfc, weights, cfg(1), 100, cond=1)
 
 
 def test_trajectory_config2(pfc, weights):
@@ -161,14 +184,14 @@ def test_trajectory_config3_full_size(pfc, weights):
 
 def test_trajectory_fp32_path_configs_1_and_3(pfc, weights):
     """The FFMA path on the two configs whose default is the tensor-core MLP."""
-    _trajectory(pfc, weights, cfg(1), 100, mlp_path=pfc.MLP_FP32)
+    _trajectory(pfc, weights, cfg(1), 100, mlp_path=pfc.MLP_FP32, cond=1)
     _trajectory(pfc, weights, cfg(3), 100, cell=True, mlp_path=pfc.MLP_FP32)
 
 
 def test_trajectory_config4_subset_of_64_replicas(pfc, weights):
     """100 steps on the first 64 replicas of config 4 with every check of _trajectory (velocities, final
     lists, E, F); all 4,096 replicas are integrated by the next test."""
-    _trajectory(pfc, weights, W.config4(n_replicas=64), 100)
+    _trajectory(pfc, weights, W.config4(n_replicas=64), 100, cond=4)
 
 
 # ---- all 4,096 replicas of config 4, both MLP paths, with the conditioning of the bar (reading S30) ----
@@ -182,18 +205,6 @@ def _cfg4_oracle(weights):
     return _cfg4_ref["pos"]
 
 
-def _cfg4_conditioning():
-    """tests/golden/cfg4_conditioning.txt (written by make_cfg4_conditioning.py from the oracle alone): per
-    replica, how far the fp64 oracle's own 100-step trajectory moves when its inputs are disturbed by one
-    fp32 ulp -- the worst of the recorded disturbances."""
-    import os
-    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg4_conditioning.txt")
-    t = np.loadtxt(path)
-    assert t.shape[0] == 4096 and np.array_equal(t[:, 0], np.arange(4096))
-    return t[:, 1].astype(int), t[:, 2:].max(axis=1)
-
-
-CFG4_COND_FACTOR = 4.0     # a replica may miss 1e-4 A only within this factor of its own one-ulp sensitivity
 
 
 @pytest.mark.slow
@@ -203,12 +214,12 @@ def test_trajectory_config4_all_4096_replicas(pfc, weights, path):
     bar itself is ill-conditioned for a handful of replicas (this random-weight potential has no core
     repulsion; atoms in sub-0.1 A contacts amplify any perturbation): the fp64 oracle, rerun with its fp32
     inputs moved by ONE ulp, leaves the bar on 18 of the 4,096 replicas (tests/golden/cfg4_conditioning.txt).
-    Asserted here, per replica s:   RMSD_s <= max(1e-4 A, CFG4_COND_FACTOR * sensitivity_s),
+    Asserted here, per replica s:   RMSD_s <= max(1e-4 A, COND_FACTOR * sensitivity_s),
     i.e. every replica either meets the bar or is within a small factor of what an exact evaluation of the
     same trajectory does under a one-ulp input error; and no more replicas miss the bar than the disturbed
     oracle itself.  The floor (second term) is active for the replicas reported in the message."""
     wl = cfg(4)
-    sizes, sens = _cfg4_conditioning()
+    sizes, sens = _conditioning(4)
     assert np.array_equal(sizes, np.diff(wl.sys_offsets))
     ref = _cfg4_oracle(weights)
     p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_FP32 if path == "fp32" else pfc.MLP_TENSOR)
@@ -219,7 +230,7 @@ def test_trajectory_config4_all_4096_replicas(pfc, weights, path):
     assert p.status() == 0
     rmsd = _rmsd_per_system(pos.cpu().numpy()[:, :3].astype(np.float64), ref, wl.sys_offsets)
     p.close()
-    bound = np.maximum(RMSD_TOL, CFG4_COND_FACTOR * sens)
+    bound = np.maximum(RMSD_TOL, COND_FACTOR * sens)
     miss = np.where(rmsd > RMSD_TOL)[0]
     report = (f"{path}: {len(miss)} of 4096 replicas above 1e-4 A (disturbed oracle: {int((sens > RMSD_TOL).sum())}); "
               f"median {np.median(rmsd):.2e}, worst {rmsd.max():.2e}; worst ratio to the bound {(rmsd / bound).max():.2f}; "
@@ -469,10 +480,12 @@ def test_nve_energy_conservation_on_gpu(pfc, weights):
 
 
 # ---- every K3 tile variant, on element blocks that end inside a warp's rows / a tile ----------------
-@pytest.mark.parametrize("tm,deep", [(16, 0), (16, 1), (32, 0), (32, 1), (64, 0), (128, 0)])
+@pytest.mark.parametrize("tm,deep", [(0, 0), (16, 0), (16, 1), (32, 0), (32, 1), (64, 0), (128, 0)])
 def test_k3_tile_variants_on_ragged_element_blocks(pfc, weights, tm, deep):
-    """pfc_create picks one tile height per batch; pfc_tuning_t.k3_tile_rows / k3_deep_ring force the
-    others.  Element counts 1 / 9 / 33 / 41 end inside an 8-row warp group, a 16-row and a 32-row tile."""
+    """pfc_create picks one FP32 MLP kernel per batch; pfc_tuning_t.k3_tile_rows / k3_deep_ring / k3_cluster
+    force the others (tm = 0: the cluster kernel for single small molecules, 8 CTAs per 16-row tile, which is
+    what this 84-atom batch gets by default).  Element counts 1 / 9 / 33 / 41 end inside an 8-row warp
+    group, a 16-row and a 32-row tile."""
     rng = np.random.default_rng(20241218)
     counts = [33, 41, 1, 9]                                     # H, C, N, O
     species = np.repeat(np.arange(4, dtype=np.int32), counts)
@@ -485,11 +498,12 @@ def test_k3_tile_variants_on_ragged_element_blocks(pfc, weights, tm, deep):
             pts.append(c)
     pos = np.asarray(pts, dtype=np.float32)
     off = np.array([0, 30, n], dtype=np.int32)                   # two systems
-    p = pfc.Pfc(species, off, weights, mlp_path=pfc.MLP_FP32,
-                tuning=pfc.Tuning(k3_tile_rows=tm, k3_deep_ring=2 if deep else 1))
+    tuning = pfc.Tuning(k3_cluster=2) if tm == 0 else pfc.Tuning(k3_tile_rows=tm, k3_deep_ring=2 if deep else 1)
+    p = pfc.Pfc(species, off, weights, mlp_path=pfc.MLP_FP32, tuning=tuning)
     E, F = p.energy_forces(_dev(pfc, pos))
     torch.cuda.synchronize()
-    ref = oracle.energy_forces(pos.astype(np.float64), species, off, weights)
+    ref = oracle.energy_forces(pos.astype(np.float64), species, off, weights, want_intermediates=True)
+    assert np.abs(p.intermediates()[1] - ref["g"]).max() <= 2e-6
     Eh, Fh = E.cpu().numpy().astype(np.float64), F.cpu().numpy().astype(np.float64)
     assert (np.abs(Eh - ref["E"]) <= E_RTOL * np.maximum(np.abs(ref["E"]), 1.0)).all()
     assert np.abs(Fh[:, :3] - ref["F"]).max() <= F_ATOL_INTERNAL
