@@ -23,7 +23,8 @@
 //   5      delta1   (160)     W1^T [k][48]          g -> global                        (384: 48)
 // Activations live TRANSPOSED in shared memory ([k][16 rows]): a thread owns 4 rows x 1 column and,
 // per k, reads one weight (consecutive lanes: consecutive columns) and one float4 of activations
-// (a broadcast).  K is split over KS thread groups whose partial sums are added in a fixed order;
+// (a broadcast).  K is split over KS thread groups (512 threads: 12 to 80 k per thread) whose partial sums
+// are added in a fixed order;
 // CELU' of the own columns stays in registers between the forward and the backward phase (the
 // thread mapping of phases 0/4 and 1/3 is the same).  The energy is reduced over the 12 columns of
 // a CTA and then over the 8 CTAs (into CTA 0's shared memory), both in a fixed order: no atomics,
@@ -35,14 +36,15 @@ namespace pfc {
 
 constexpr int CL_SIZE = 8;                       // CTAs per cluster (the portable maximum)
 constexpr int CL_TM = 16;                        // rows per tile
-constexpr int CL_THREADS = 256;
+constexpr int CL_THREADS = 512;
 constexpr int CL_MAX_TILES = 18;                 // 18 clusters x 8 CTAs <= 148 SMs: one wave
 constexpr int CL_NC0 = D1 / CL_SIZE, CL_NC1 = D2 / CL_SIZE, CL_NC2 = D3 / CL_SIZE, CL_NC3 = D2 / CL_SIZE,
               CL_NC4 = D1 / CL_SIZE, CL_NC5 = D0 / CL_SIZE;     // 20 16 12 16 20 48
 constexpr int CL_W0 = 0, CL_W1 = CL_W0 + D0 * CL_NC0, CL_W2 = CL_W1 + D1 * CL_NC1, CL_W3 = CL_W2 + D2 * CL_NC2,
               CL_W4 = CL_W3 + D3 * CL_NC3, CL_W5 = CL_W4 + D2 * CL_NC4, CL_W_FLOATS = CL_W5 + D1 * CL_NC5;   // 23,552
 static_assert(CL_W_FLOATS == 23552 && CL_W_FLOATS * CL_SIZE == MLP_P_FLOATS, "weight slices of one CTA");
-constexpr int CL_SCRATCH = 4 * 20 * 4 * 4;       // partial sums: KS x (NC x 4 row groups) x 4 rows (largest: phase 0, 3 x 80 x 4)
+constexpr int CL_PART = 2048;                    // partial sums: (KS - 1) x (NC x 4 row groups) x 4 rows (largest: 7 x 64 x 4)
+constexpr int CL_SCRATCH = CL_PART + CL_TM * CL_NC5;   // + phase 5: the g block [16][48]
 
 struct ClSmem {
   float w[CL_W_FLOATS];                          // my column slices of the six weight matrices, [k][nc] each
@@ -99,7 +101,7 @@ template <int K, int NC, int KS>
 __device__ __forceinline__ bool cl_gemm(const float* __restrict__ actT, const float* __restrict__ Ws, float* scratch,
                                         int& c, int& rg, float4& acc) {
   constexpr int PAIRS = NC * 4, KL = K / KS;
-  static_assert(K % KS == 0 && PAIRS * KS <= CL_THREADS && PAIRS * KS * 4 <= CL_SCRATCH || KS == 1, "thread / scratch budget");
+  static_assert(K % KS == 0 && KL % 4 == 0 && PAIRS * KS <= CL_THREADS && PAIRS * (KS - 1) * 4 <= CL_PART, "thread / scratch budget");
   const int tid = threadIdx.x, ks = tid / PAIRS, rem = tid - ks * PAIRS;
   c = rem % NC; rg = rem / NC;
   const bool active = ks < KS;
@@ -107,7 +109,7 @@ __device__ __forceinline__ bool cl_gemm(const float* __restrict__ actT, const fl
   if (active) {
     const float* a = actT + (size_t)ks * KL * CL_TM + 4 * rg;
     const float* w = Ws + (size_t)ks * KL * NC + c;
-#pragma unroll 8
+#pragma unroll 4
     for (int k = 0; k < KL; ++k) {
       const float4 x = *reinterpret_cast<const float4*>(a + k * CL_TM);
       const float wk = w[k * NC];
@@ -134,8 +136,8 @@ __device__ __forceinline__ float cl_dcelu(float x) { return x > 0.0f ? 1.0f : ex
 __global__ void __cluster_dims__(CL_SIZE, 1, 1) __launch_bounds__(CL_THREADS, 1)
 k3_mlp_cluster_kernel(const __grid_constant__ ClParams P, const float* __restrict__ aev, float* __restrict__ g,
                       float* __restrict__ e_row) {
-  extern __shared__ uint8_t cl_smem_raw[];
-  ClSmem& S = *reinterpret_cast<ClSmem*>(((uintptr_t)cl_smem_raw + 15) & ~(uintptr_t)15);
+  extern __shared__ __align__(16) uint8_t cl_smem_raw[];
+  ClSmem& S = *reinterpret_cast<ClSmem*>(cl_smem_raw);      // (no integer round trip: the accesses stay LDS / STS)
   const int tid = threadIdx.x;
   const uint32_t rank = cl::cta_rank();
   const int tile = blockIdx.x / CL_SIZE;
@@ -170,7 +172,7 @@ k3_mlp_cluster_kernel(const __grid_constant__ ClParams P, const float* __restric
 
   // ---- phase 0: h1 ----
   tc::mbar_wait(&S.wbar[0], 0);
-  if (cl_gemm<D0, CL_NC0, 3>(S.aevT, S.w + CL_W0, S.scratch, c, rg, acc)) {
+  if (cl_gemm<D0, CL_NC0, 6>(S.aevT, S.w + CL_W0, S.scratch, c, rg, acc)) {
     const int n = (int)rank * CL_NC0 + c;
     const float b = __ldg(V + MLP_V_B1 + n);
     const float4 z = make_float4(acc.x + b, acc.y + b, acc.z + b, acc.w + b);
@@ -180,7 +182,7 @@ k3_mlp_cluster_kernel(const __grid_constant__ ClParams P, const float* __restric
   cl::cluster_sync();
   // ---- phase 1: h2 ----
   tc::mbar_wait(&S.wbar[1], 0);
-  if (cl_gemm<D1, CL_NC1, 4>(S.h1T, S.w + CL_W1, S.scratch, c, rg, acc)) {
+  if (cl_gemm<D1, CL_NC1, 8>(S.h1T, S.w + CL_W1, S.scratch, c, rg, acc)) {
     const int n = (int)rank * CL_NC1 + c;
     const float b = __ldg(V + MLP_V_B2 + n);
     const float4 z = make_float4(acc.x + b, acc.y + b, acc.z + b, acc.w + b);
@@ -190,7 +192,7 @@ k3_mlp_cluster_kernel(const __grid_constant__ ClParams P, const float* __restric
   cl::cluster_sync();
   // ---- phase 2: energy and delta3 ----
   tc::mbar_wait(&S.wbar[2], 0);
-  if (cl_gemm<D2, CL_NC2, 4>(S.h2T, S.w + CL_W2, S.scratch, c, rg, acc)) {
+  if (cl_gemm<D2, CL_NC2, 8>(S.h2T, S.w + CL_W2, S.scratch, c, rg, acc)) {
     const int n = (int)rank * CL_NC2 + c;
     const float b = __ldg(V + MLP_V_B3 + n), w4 = __ldg(V + MLP_V_W4 + n);
     const float4 z = make_float4(acc.x + b, acc.y + b, acc.z + b, acc.w + b);
@@ -213,29 +215,30 @@ k3_mlp_cluster_kernel(const __grid_constant__ ClParams P, const float* __restric
   }
   // ---- phase 3: delta2 ----
   tc::mbar_wait(&S.wbar[3], 0);
-  if (cl_gemm<D3, CL_NC3, 4>(S.d3T, S.w + CL_W3, S.scratch, c, rg, acc)) {
+  if (cl_gemm<D3, CL_NC3, 8>(S.d3T, S.w + CL_W3, S.scratch, c, rg, acc)) {
     const int n = (int)rank * CL_NC3 + c;
     cl::broadcast4(S.h2T, n, rg, make_float4(acc.x * dc2.x, acc.y * dc2.y, acc.z * dc2.z, acc.w * dc2.w));
   }
   cl::cluster_sync();
   // ---- phase 4: delta1 ----
   tc::mbar_wait(&S.wbar[4], 0);
-  if (cl_gemm<D2, CL_NC4, 2>(S.h2T, S.w + CL_W4, S.scratch, c, rg, acc)) {
+  if (cl_gemm<D2, CL_NC4, 4>(S.h2T, S.w + CL_W4, S.scratch, c, rg, acc)) {
     const int n = (int)rank * CL_NC4 + c;
     cl::broadcast4(S.h1T, n, rg, make_float4(acc.x * dc1.x, acc.y * dc1.y, acc.z * dc1.z, acc.w * dc1.w));
   }
   cl::cluster_sync();
   // ---- phase 5: g, my 48 columns of the 16 rows ----
   tc::mbar_wait(&S.wbar[5], 0);
-  if (cl_gemm<D1, CL_NC5, 1>(S.h1T, S.w + CL_W5, S.scratch, c, rg, acc)) {
-    S.scratch[(4 * rg + 0) * CL_NC5 + c] = acc.x; S.scratch[(4 * rg + 1) * CL_NC5 + c] = acc.y;
-    S.scratch[(4 * rg + 2) * CL_NC5 + c] = acc.z; S.scratch[(4 * rg + 3) * CL_NC5 + c] = acc.w;
+  if (cl_gemm<D1, CL_NC5, 2>(S.h1T, S.w + CL_W5, S.scratch, c, rg, acc)) {
+    float* blk = S.scratch + CL_PART;
+    blk[(4 * rg + 0) * CL_NC5 + c] = acc.x; blk[(4 * rg + 1) * CL_NC5 + c] = acc.y;
+    blk[(4 * rg + 2) * CL_NC5 + c] = acc.z; blk[(4 * rg + 3) * CL_NC5 + c] = acc.w;
   }
   __syncthreads();
   for (int q = tid; q < n_real * (CL_NC5 / 4); q += CL_THREADS) {
     const int r = q / (CL_NC5 / 4), c4 = q - r * (CL_NC5 / 4);
     *reinterpret_cast<float4*>(g + (size_t)(row0 + r) * AEV_LEN + (int)rank * CL_NC5 + 4 * c4) =
-        *reinterpret_cast<const float4*>(S.scratch + r * CL_NC5 + 4 * c4);
+        *reinterpret_cast<const float4*>(S.scratch + CL_PART + r * CL_NC5 + 4 * c4);
   }
 }
 

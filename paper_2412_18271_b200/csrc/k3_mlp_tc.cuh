@@ -222,7 +222,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1)
 k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__ aev16, float* __restrict__ g,
                  float* __restrict__ e_row) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* base = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  // 1024-byte alignment by pointer arithmetic on the shared array (an integer round trip would turn every
+  // access below into a generic load / store)
+  uint8_t* base = smem_raw + ((1024u - (tc::smem_u32(smem_raw) & 1023u)) & 1023u);
   uint8_t* resD1 = base;                                   // resident delta1 operand: 5 chunks
   uint8_t* ringA = resD1 + TC_ND1 * TC_A_SLOT;
   uint8_t* ringB = ringA + TC_NA * TC_A_SLOT;
