@@ -206,6 +206,9 @@ def per_kernel_roofline(stage_ms, counts, n_atoms, n_systems, mlp_is_tensor, pea
     }
     out = {}
     for (name, (bound, flops, nbytes)), ms in zip(rows.items(), stage_ms):
+        if not ms > 0.0:                                         # small systems: the energy sum is part of the K4b kernel
+            out[name] = {"bound": bound, "ms": 0.0, "fused_into": "K4b_gather"}
+            continue
         sec = ms * 1e-3
         e = {"bound": bound, "ms": float(ms), "algorithmic_bytes": nbytes, "gbs": nbytes / sec / 1e9,
              "hbm_frac": nbytes / sec / 1e9 / hbm, "hbm_frac_nominal": nbytes / sec / 1e9 / 8000.0}
@@ -278,6 +281,10 @@ def run_pfc(args):
     pfc.load_library()
     weights = W.make_weights()
     wl = W.make_config(args.config)
+    if args.replicas and args.config in (1, 4):
+        import dataclasses
+        wl = (W.config1 if args.config == 1 else W.config4)(n_replicas=args.replicas)
+        wl = dataclasses.replace(wl, name=f"{wl.name}_first{args.replicas}")
     N = wl.n_atoms
     stream = torch.cuda.Stream(device=dev)
     p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=args.mlp, device=dev)
@@ -448,6 +455,9 @@ def main():
     ap.add_argument("--mlp", type=int, default=3, choices=[0, 1, 3],
                     help="3 = auto (library default: tensor-core MLP from 4096 atoms on), 0 = FP32 FFMA, 1 = tcgen05 fp16 split")
     ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (100 steps each)")
+    ap.add_argument("--replicas", type=int, default=0,
+                    help="configs 1 and 4 only: the first N replicas instead of all (profiling / sanitizer runs; "
+                         "the workload name in the JSON line says so)")
     args = ap.parse_args()
     INTEGRATOR["kind"] = args.integrator
     if args.warmup < 3 and args.impl == "pfc":

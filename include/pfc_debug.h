@@ -35,6 +35,14 @@ int pfc_k3_timeline(pfc_t *ctx, int64_t *cycles, int32_t n);
  * getters of pfc.h into HOST memory. */
 int pfc_copy_to_host(const void *device_src, void *host_dst, size_t bytes);
 
+/* How the tensor core accumulates: ONE accumulator chain of n_mma tcgen05.mma
+ * kind::f16 instructions (M 128, N 64, K 16, fp32 accumulate), instruction i multiplying the 16-k slice
+ * (i mod n_slices) of A DEVICE [128][16 n_slices] and B DEVICE [64][16 n_slices] (row-major fp32 values, which
+ * must be exactly representable in fp16; 1 <= n_slices <= 16), staged in shared memory exactly as the MLP
+ * kernel stages its operands.  D DEVICE [128][64]: the raw accumulator.  No handle; enqueues one kernel on
+ * `stream` of the current device. */
+int pfc_tc_chain_probe(const float *A, const float *B, int32_t n_slices, int32_t n_mma, float *D, void *stream);
+
 /* Truncation compensation of the tensor-core MLP, per element e = 0..3:
  * out HOST [32], out[8e + ..] = {lambda forward, lambda backward, residual slope of e_i, residual slope of g,
  * max|de| / rms e, max|dg| / rms g (all against the library's FP32 MLP on the calibration batch; 0 for an

@@ -36,7 +36,13 @@
 
 namespace pfc {
 
-constexpr int K2_TCH = 96;                       // padded triple slots per chunk (3 passes of 32 lanes)
+#ifndef PFC_K2_TCH
+#define PFC_K2_TCH 96
+#endif
+#ifndef PFC_K2_MINB
+#define PFC_K2_MINB 24
+#endif
+constexpr int K2_TCH = PFC_K2_TCH;               // padded triple slots per chunk (3 passes of 32 lanes)
 constexpr int K2_TLD = K2_TCH + 4;               // row stride of the transposed factor tables: 4 mod 32 banks
 
 struct AevFwdSmem {
@@ -53,7 +59,7 @@ constexpr int K2_PACK_CHUNK_BYTES = 2 * 128 * 64;     // == TC_A_SLOT: hi block 
 constexpr float K2_PACK_SCALE = 8.0f;                // == 2^TC_AEV_SCALE_LOG2
 
 template <bool PACK16>
-__global__ void __launch_bounds__(AEV_WARPS * 32, 8)
+__global__ void __launch_bounds__(AEV_WARPS * 32, PFC_K2_MINB)
 k2_aev_fwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __restrict__ xsl,
                   const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr, const int2* __restrict__ cnt,
                   const int* __restrict__ row_of_atom,

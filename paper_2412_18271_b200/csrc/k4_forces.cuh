@@ -38,7 +38,10 @@ struct AevBwdSmem {
   float tC[K4_TCH], tA[K4_TCH], tB[K4_TCH];
 };
 
-__global__ void __launch_bounds__(AEV_WARPS * 32, 7)
+#ifndef PFC_K4A_MINB
+#define PFC_K4A_MINB 25
+#endif
+__global__ void __launch_bounds__(AEV_WARPS * 32, PFC_K4A_MINB)
 k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __restrict__ xsl,
                    const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr, const int2* __restrict__ cnt,
                    const int* __restrict__ row_of_atom,

@@ -8,6 +8,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <cmath>
 #include <new>
 #include <vector>
@@ -20,6 +21,7 @@
 #include "k3_mlp_fp32.cuh"
 #include "k3_mlp_cluster.cuh"
 #include "k3_mlp_tc.cuh"
+#include "tc_probe.cuh"
 #include "k4_forces.cuh"
 #include "k5_verlet.cuh"
 
@@ -1164,6 +1166,17 @@ int pfc_status(pfc_t* c, uint32_t* bits) {
   if (cudaStreamSynchronize(c->stream) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpy(bits, c->b.status, sizeof(uint32_t), cudaMemcpyDeviceToHost) != cudaSuccess) return PFC_ERR_CUDA;
   return PFC_OK;
+}
+
+int pfc_tc_chain_probe(const float* A, const float* B, int32_t n_slices, int32_t n_mma, float* D, void* stream) {
+  if (!A || !B || !D || n_slices < 1 || n_slices > TCP_MAX_SLICES || n_mma < 1 || n_mma > 4096) return PFC_ERR_ARG;
+  const size_t smem = 1024 + (size_t)((n_slices + 1) / 2) * (TCP_M + TCP_N) * 64;
+  if (cudaFuncSetAttribute(tc_chain_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    cudaGetLastError();
+    return PFC_ERR_CUDA;
+  }
+  tc_chain_probe_kernel<<<1, 128, smem, (cudaStream_t)stream>>>(A, B, n_slices, n_mma, D);
+  return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
 }
 
 int pfc_tc_calibration(pfc_t* c, float* out) {

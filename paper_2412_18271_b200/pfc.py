@@ -37,7 +37,7 @@ EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy
            "pfc_step", "pfc_step_langevin", "pfc_set_frames", "pfc_frames_written", "pfc_run_host",
            "pfc_run_host_resume", "pfc_get_neighbors", "pfc_get_intermediates", "pfc_status", "pfc_destroy",
            "pfc_error_string")
-DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_k3_timeline", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts", "pfc_tc_calibration")
+DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_k3_timeline", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts", "pfc_tc_calibration", "pfc_tc_chain_probe")
 
 
 class PfcError(RuntimeError):
@@ -94,6 +94,7 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_status.argtypes = [c_void_p, POINTER(c_uint32)]
     lib.pfc_mlp_path.argtypes = [c_void_p, POINTER(c_int32)]
     lib.pfc_tc_calibration.argtypes = [c_void_p, POINTER(c_float)]
+    lib.pfc_tc_chain_probe.argtypes = [c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
     lib.pfc_launch_counts.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32)]
     lib.pfc_destroy.argtypes = [c_void_p]
     lib.pfc_error_string.argtypes = [c_int]
@@ -108,6 +109,20 @@ def load_library() -> ctypes.CDLL:
 def _check(rc: int, what: str) -> None:
     if rc != 0:
         raise PfcError(f"{what}: {load_library().pfc_error_string(rc).decode()} ({rc})")
+
+
+def tc_chain_probe(A, B, n_mma: int, stream=None):
+    """pfc_tc_chain_probe: cuda float32 tensors A [128, 16 s], B [64, 16 s] (fp16-representable values) -> raw
+    accumulator [128, 64] of a chain of n_mma tcgen05.mma kind::f16 instructions cycling through the s slices."""
+    import torch
+    assert A.is_cuda and B.is_cuda and A.dtype == torch.float32 and B.dtype == torch.float32
+    assert A.shape[0] == 128 and B.shape[0] == 64 and A.shape[1] == B.shape[1] and A.shape[1] % 16 == 0
+    A, B = A.contiguous(), B.contiguous()
+    D = torch.empty(128, 64, dtype=torch.float32, device=A.device)
+    with torch.cuda.device(A.device):
+        _check(load_library().pfc_tc_chain_probe(A.data_ptr(), B.data_ptr(), A.shape[1] // 16, int(n_mma), D.data_ptr(),
+                                                 _stream_ptr(stream)), "pfc_tc_chain_probe")
+    return D
 
 
 def pfc_workspace_bytes(n_atoms: int, n_systems: int) -> int:

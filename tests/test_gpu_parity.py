@@ -17,9 +17,15 @@ from paper_2412_18271_b200 import workloads as W                 # noqa: E402
 
 E_RTOL = 1e-5
 F_ATOL = 1e-3
-F_ATOL_INTERNAL = 5e-5
+F_ATOL_INTERNAL = 5e-5       # dense / unusual test geometries
 RMSD_TOL = 1e-4
 VEL_TOL = 4e-5
+# Builder-set bounds on the five configs at step 0, each <= 3x the worst value measured on either MLP path
+# (max|dF| 1.9e-6, max|daev| 5.3e-6, max|dg| 3.9e-7, max|de_i| 8.8e-7)
+F_ATOL_STEP0 = 6e-6
+AEV_ATOL = 1e-5
+G_ATOL = 1.2e-6
+E_ATOM_ATOL = 3e-6
 
 
 @pytest.fixture(scope="module")
@@ -68,9 +74,12 @@ def _check_energy_forces(E, F, ref, tight=True):
     assert (np.abs(Eh - ref["E"]) <= tol_e).all(), float((np.abs(Eh - ref["E"]) / tol_e).max())
     dF = np.abs(Fh[:, :3] - ref["F"]).max()
     assert dF <= F_ATOL, dF
-    if tight:
-        assert dF <= F_ATOL_INTERNAL, dF
-    assert np.abs(Fh[:, 3] - ref["e"]).max() <= 1e-5
+    de = np.abs(Fh[:, 3] - ref["e"]).max()
+    if tight:                                                    # the generators' states (step 0)
+        assert dF <= F_ATOL_STEP0, dF
+        assert de <= E_ATOM_ATOL, de
+    else:                                                        # evolved states: atoms in close contacts carry larger e_i
+        assert de <= 1e-5 * max(1.0, np.abs(ref["e"]).max()), de
     return dF
 
 
@@ -92,8 +101,8 @@ def test_step0_lists_energy_forces_full_size(pfc, weights, k, path):
                                cell=(k == 3), want_intermediates=True)
     _check_energy_forces(E, F, ref)
     aev, g = p.intermediates()
-    assert np.abs(aev - ref["aev"]).max() <= 1e-5
-    assert np.abs(g - ref["g"]).max() <= 2e-6
+    assert np.abs(aev - ref["aev"]).max() <= AEV_ATOL
+    assert np.abs(g - ref["g"]).max() <= G_ATOL
     p.close()
 
 

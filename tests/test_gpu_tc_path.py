@@ -17,8 +17,11 @@ from paper_2412_18271_b200 import workloads as W                 # noqa: E402
 
 E_RTOL = 1e-5
 F_ATOL = 1e-3                # FP32-path bar of north_star
-F_ATOL_INTERNAL = 5e-5
-G_ATOL = 2e-6
+F_ATOL_INTERNAL = 5e-5       # other weight sets
+G_ATOL = 2e-6                # other weight sets
+F_ATOL_STEP0 = 6e-6          # standard weights, the five configs: <= 3x the measured worst case
+G_ATOL_STEP0 = 1.2e-6
+E_ATOM_ATOL = 3e-6
 RMSD_TOL = 1e-4
 
 
@@ -55,9 +58,9 @@ def test_f16x3_step0_energy_forces_full_size(pfc, weights, k):
     wl = W.make_config(k)
     err = _errors(pfc, weights, wl, pfc.MLP_TENSOR, cell=(k == 3))
     assert err["E"] <= E_RTOL, err
-    assert err["F"] <= F_ATOL_INTERNAL, err
-    assert err["e"] <= 1e-5, err
-    assert err["g"] <= G_ATOL, err
+    assert err["F"] <= F_ATOL_STEP0, err
+    assert err["e"] <= E_ATOM_ATOL, err
+    assert err["g"] <= G_ATOL_STEP0, err
 
 
 def test_f16x3_matches_fp32_path_closely(pfc, weights):
