@@ -286,6 +286,35 @@ def test_bitwise_determinism(pfc, weights):
         assert np.array_equal(a, b)
 
 
+@pytest.mark.parametrize("what", ["tensor", "cluster"])
+def test_repeated_evaluations_are_bit_identical(pfc, weights, what):
+    """Stands in for racecheck (compute-sanitizer is closed on this pool, profiles/r2_sanitizer.md): a race in the
+    tensor kernel's mbarrier / TMEM pipeline (three warp roles, TMEM columns reused under live readers), in the
+    cluster kernel's distributed-shared-memory exchange or in the graph replay shows as a run-to-run difference.
+    40 evaluations of one batch, every output identical bit for bit; then a second handle reproduces them."""
+    if what == "tensor":
+        wl = W.config4(n_replicas=300)                            # 135 tiles + padding on 148 persistent CTAs
+        mk = lambda: pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_TENSOR)
+    else:
+        wl = W.config1(n_replicas=8)                              # 12 tiles of 16 rows: the cluster kernel
+        mk = lambda: pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_FP32, tuning=pfc.Tuning(k3_cluster=2))
+    pos = _dev(pfc, wl.pos)
+    ref = None
+    for handle in range(2):
+        p = mk()
+        for _ in range(40 if handle == 0 else 3):
+            E, F = p.energy_forces(pos)
+            torch.cuda.synchronize()
+            _, g = p.intermediates()
+            out = (E.cpu().numpy().copy(), F.cpu().numpy().copy(), g.copy())
+            if ref is None:
+                ref = out
+            for a, b in zip(out, ref):
+                assert np.array_equal(a, b)
+        assert p.status() == 0
+        p.close()
+
+
 def test_step_splits_are_equivalent(pfc, weights):
     """pfc_step(60) == pfc_step(25) + pfc_step(35) bit for bit (the state at exit is synchronous)."""
     wl = W.config1(n_replicas=8)
