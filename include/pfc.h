@@ -27,7 +27,13 @@
  *  - Atoms of system s are the contiguous range sys_offsets[s]..sys_offsets[s+1];
  *    there are no pairs across systems.
  *  - Every call except create/destroy/status/run_host only ENQUEUES work on
- *    the given stream and returns; it never synchronises.
+ *    the given stream and returns; it never synchronises.  One exception, once per
+ *    handle: the FIRST evaluation (pfc_energy_forces, pfc_energy_forces_nm or pfc_step)
+ *    of a handle on the tensor-core MLP measures its truncation compensation on that
+ *    batch against the library's FP32 MLP (five extra MLP launches)
+ *    and synchronises the stream; it must not be issued under a stream capture of the
+ *    caller's.  Under PFC_MLP_AUTO the handle stays on the tensor-core MLP only if the
+ *    check of that measurement passes (pfc_mlp_path in pfc_debug.h reports the outcome).
  *  - Return value: PFC_OK (0) or a negative PFC_ERR_* code.  Nothing throws or
  *    aborts across this boundary.  Conditions detected on the device
  *    (neighbour capacity overflow, angular row longer than PFC_MAX_ANGULAR,
@@ -69,7 +75,7 @@ extern "C" {
 #define PFC_MLP_FP32 0                  /* FP32 FFMA grouped MLP                 */
 #define PFC_MLP_TENSOR 1                /* tcgen05 kind::f16, fp16 hi|lo 3-term split, fp32 accumulate */
 #define PFC_MLP_TENSOR_1TERM 2          /* tcgen05 plain fp16 operands: tolerance evidence only (fails it) */
-#define PFC_MLP_AUTO 3                  /* TENSOR for batches of >= 4096 atoms, FP32 below */
+#define PFC_MLP_AUTO 3                  /* TENSOR for batches of >= 4096 atoms if its calibration check passes, FP32 otherwise */
 
 /* Optional tuning knobs, passed explicitly through pfc_desc_t.tuning (HOST pointer, NULL = all
  * defaults; a zero-filled struct is also "all defaults").  The library reads no environment
@@ -78,8 +84,9 @@ typedef struct {
   int32_t k3_tile_rows;       /* FP32 MLP tile height: 0 = chosen by pfc_create from the batch; 16, 32, 64 or 128 */
   int32_t k3_deep_ring;       /* FP32 MLP weight staging: 0 = chosen by pfc_create; 1 = two buffers;
                                  2 = eight-stage ring (tiles of <= 32 rows only, ignored otherwise) */
-  int32_t tc_comp_override;   /* 0 = default truncation compensation of the tensor-core MLP (DESIGN.md
-                                 section 5); 1 = scale it by the two factors below (0 switches it off) */
+  int32_t tc_comp_override;   /* 0 = truncation compensation of the tensor-core MLP calibrated per handle on its first
+                                 batch; 1 = no calibration: the two scales below (0 switches
+                                 the compensation off) */
   float tc_comp_forward;      /* used when tc_comp_override = 1 */
   float tc_comp_backward;
   int32_t steps_per_graph;    /* MD steps captured per CUDA graph by pfc_step: 0 = default (16); >= 1 */

@@ -130,8 +130,9 @@ __device__ __forceinline__ bool cl_gemm(const float* __restrict__ actT, const fl
   return active && ks == 0;
 }
 
-__device__ __forceinline__ float cl_celu(float x) { return x > 0.0f ? x : CELU_ALPHA * (expf(x * (1.0f / CELU_ALPHA)) - 1.0f); }
-__device__ __forceinline__ float cl_dcelu(float x) { return x > 0.0f ? 1.0f : expf(x * (1.0f / CELU_ALPHA)); }
+// CELU and CELU', alpha = 0.1, branch-free: e = exp(min(x, 0) / alpha) is exactly 1 for x >= 0
+__device__ __forceinline__ float cl_dcelu(float x) { return ex2_approx(fminf(x, 0.0f) * (LOG2E / CELU_ALPHA)); }
+__device__ __forceinline__ float cl_celu(float x) { return fmaxf(x, 0.0f) + fmaf(CELU_ALPHA, cl_dcelu(x), -CELU_ALPHA); }
 
 __global__ void __cluster_dims__(CL_SIZE, 1, 1) __launch_bounds__(CL_THREADS, 1)
 k3_mlp_cluster_kernel(const __grid_constant__ ClParams P, const float* __restrict__ aev, float* __restrict__ g,
@@ -165,14 +166,15 @@ k3_mlp_cluster_kernel(const __grid_constant__ ClParams P, const float* __restric
     S.aevT[(4 * k4 + 2) * CL_TM + r] = v.z; S.aevT[(4 * k4 + 3) * CL_TM + r] = v.w;
   }
   __syncthreads();                               // aevT complete, barriers initialised
-  cl::cluster_sync();                            // every CTA of the cluster is running: its shared memory may be written
   int c, rg;
   float4 acc;
   float4 dc1 = make_float4(0.f, 0.f, 0.f, 0.f), dc2 = dc1;   // CELU' of my columns of z1 / z2
 
   // ---- phase 0: h1 ----
   tc::mbar_wait(&S.wbar[0], 0);
-  if (cl_gemm<D0, CL_NC0, 6>(S.aevT, S.w + CL_W0, S.scratch, c, rg, acc)) {
+  const bool own0 = cl_gemm<D0, CL_NC0, 6>(S.aevT, S.w + CL_W0, S.scratch, c, rg, acc);
+  cl::cluster_sync();                            // every CTA of the cluster is running: its shared memory may be written
+  if (own0) {
     const int n = (int)rank * CL_NC0 + c;
     const float b = __ldg(V + MLP_V_B1 + n);
     const float4 z = make_float4(acc.x + b, acc.y + b, acc.z + b, acc.w + b);

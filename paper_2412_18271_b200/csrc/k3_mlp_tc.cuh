@@ -9,7 +9,7 @@
 // accuracy: 3e-8 of the operand's scale).  Every operand class is pre-scaled by an exact power of
 // two that puts its typical magnitude well inside fp16's range (weights per layer and element from
 // max|W|, the AEV by 8, the backward deltas from max|w4|); the scales leave through the epilogue
-// factor of each phase (TcParams::kf), so no rounding is added.  Against the round-1 kind::tf32
+// factor of each phase (ks[q] in the per-element table), so no rounding is added.  Against the round-1 kind::tf32
 // split this is half the tensor-pipe time per k (K = 16 per MMA instead of 8), half the operand
 // bytes in shared memory and in the weight stream.  (A bf16 remainder would not need the scaling,
 // but the hardware rejects instruction descriptors that mix fp16 and bf16 operands -- measured.)

@@ -316,8 +316,16 @@ void enqueue_k3_tc(pfc_ctx* c, cudaStream_t st) {
 
 // K1..K4 + energy sum on `st`
 // `ev` (optional): events recorded at the seven stage boundaries K1|K2|K3|K4a|K4b|E-sum|
+void enqueue_energy_sum(pfc_ctx* c, const float4* F, float* E, cudaStream_t st) {
+  const Buffers& b = c->b;
+  if (c->n_cell_sys > 0) LAUNCH(c, k_energy_sum_kernel<1024>, c->sz.n_systems, 1024, 0, st, b.sys_off, F, E, b.status);
+  else LAUNCH(c, k_energy_sum_kernel<128>, c->sz.n_systems, 128, 0, st, b.sys_off, F, E, b.status);
+}
+
+// `with_esum` false: the per-system energies are not formed (the steps inside a pfc_step call: nobody can read E
+// between them; run_steps sums once at the end)
 void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool with_xlo, cudaStream_t st,
-                    cudaEvent_t* ev = nullptr) {
+                    cudaEvent_t* ev = nullptr, bool with_esum = true) {
   auto mark = [&](int k) { if (ev) cudaEventRecord(ev[k], st); };
   mark(0);
   const Sizes& s = c->sz;
@@ -336,8 +344,7 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool wit
   LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.row_beg, b.nbr, b.cnt, b.edge, b.self,
          b.row_of_atom, b.e_row, F);
   mark(5);
-  if (c->n_cell_sys > 0) LAUNCH(c, k_energy_sum_kernel<1024>, s.n_systems, 1024, 0, st, b.sys_off, F, E, b.status);
-  else LAUNCH(c, k_energy_sum_kernel<128>, s.n_systems, 128, 0, st, b.sys_off, F, E, b.status);
+  if (with_esum) enqueue_energy_sum(c, F, E, st);
   mark(6);
 }
 
@@ -508,7 +515,7 @@ int capture(pfc_ctx* c, int kind, int n_rep, const float4* pos, float* E, float4
   for (int r = 0; r < n_rep; ++r) {
     if (kind == 1) enqueue_verlet<2>(c, c->cap_stream);
     if (kind == 2) enqueue_langevin<2>(c, c->cap_stream);
-    enqueue_forces(c, pos, E, F, with_xlo, c->cap_stream);
+    enqueue_forces(c, pos, E, F, with_xlo, c->cap_stream, nullptr, kind == 0);
   }
   cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
   if (e != cudaSuccess || !graph) { cudaGetLastError(); return PFC_ERR_CAPTURE; }
@@ -832,7 +839,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (!ok) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
   // launch counts (static: depends only on the configuration)
   c->launches_ef = 5 + (c->n_items > 0 ? 1 : 0) + (c->n_cell_sys > 0 ? 5 : 0);
-  c->launches_step = c->launches_ef + 1;
+  c->launches_step = c->launches_ef;            // integrator kernel + forces, no energy sum inside a pfc_step call
   *out = c;
   return PFC_OK;
 }
@@ -1026,7 +1033,8 @@ static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
   if (n_steps == 0) return PFC_OK;
   // step 1: half kick + drift, forces.  steps 2..n: fused (trailing half kick + leading half kick +
   // drift), forces -- K of them per graph launch while no frame falls inside the span, else one per
-  // launch.  Then the last half kick.
+  // launch.  Then the last half kick and the per-system energies of the final state (the step graphs
+  // leave the energy sum out: E cannot be read between the steps of one call).
   if (langevin) enqueue_langevin<1>(c, st); else enqueue_verlet<1>(c, st);
   if (cudaGraphLaunch(c->g_forces, st) != cudaSuccess) return PFC_ERR_CUDA;
   if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
@@ -1044,6 +1052,7 @@ static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
     }
   }
   enqueue_verlet<0>(c, st);
+  if (n_steps > 1) enqueue_energy_sum(c, c->frc, c->E, st);   // (n_steps == 1: the force graph of step 1 has summed)
   return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
 }
 

@@ -1,9 +1,7 @@
-// tc_ptx.cuh -- inline-PTX wrappers for the sm_100a features the tensor-core MLP uses:
-// mbarrier, bulk async copy (TMA, cp.async.bulk), tcgen05 (TMEM alloc, MMA kind::tf32,
-// commit, ld) and the UMMA shared-memory / instruction descriptors.
-//
-// Descriptor bit layouts follow the PTX ISA "tcgen05 matrix descriptor" / "instruction
-// descriptor" tables (restated in DESIGN.md section 5).
+// tc_ptx.cuh -- inline-PTX wrappers for the sm_100a features the MLP kernels use:
+// mbarrier, bulk async copy (TMA, cp.async.bulk), tcgen05 TMEM allocation, commit and ld.
+// (The kind::f16 shared-memory / instruction descriptors and the MMA wrapper are in
+// k3_mlp_tc.cuh, next to the operand layout they describe.)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -79,36 +77,7 @@ __device__ __forceinline__ void tc_fence_after() {
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 }
 
-// ---- descriptors -------------------------------------------------------------------
-// Shared-memory matrix descriptor, K-major operand, SWIZZLE_128B: rows of 128 bytes
-// (32 tf32), 8-row groups 1024 bytes apart (SBO), 16-byte chunk j of row r stored at chunk
-// j ^ (r & 7).  bits [0,14) start>>4 | [16,30) LBO>>4 (=1, unused when swizzled) |
-// [32,46) SBO>>4 | [46,48) version=1 | [61,64) layout: 2 = SWIZZLE_128B.
-__device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t smem_addr) {
-  uint64_t d = (uint64_t)((smem_addr & 0x3FFFFu) >> 4);
-  d |= (uint64_t)1 << 16;
-  d |= (uint64_t)(1024 >> 4) << 32;
-  d |= (uint64_t)1 << 46;
-  d |= (uint64_t)2 << 61;
-  return d;
-}
-// Instruction descriptor, kind::tf32, fp32 accumulate, A and B K-major, M x N tile:
-// [4,6) D fmt: 1 = f32 | [7,10) A fmt: 2 = tf32 | [10,13) B fmt: 2 = tf32 | [15] A major: 0 = K |
-// [16] B major: 0 = K | [17,23) N>>3 | [24,29) M>>4.
-__host__ __device__ constexpr uint32_t idesc_tf32(int M, int N) {
-  return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
-}
-
-// D[tmem] (+)= A[smem] * B[smem]^T, issued by ONE thread
-__device__ __forceinline__ void mma_tf32_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
-                                            uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
-      "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-      : "memory");
-}
+// ---- tcgen05.mma completion (the kind::f16 descriptors and the MMA wrapper live in k3_mlp_tc.cuh) ----
 // all previously issued MMAs of this thread complete -> one arrival on the mbarrier
 __device__ __forceinline__ void mma_commit(uint64_t* bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
@@ -128,26 +97,8 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
 #pragma unroll
   for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
-// registers -> TMEM, same shape
-__device__ __forceinline__ void tmem_st16(uint32_t taddr, const float (&v)[16]) {
-  asm volatile(
-      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr),
-      "r"(__float_as_uint(v[0])), "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])), "r"(__float_as_uint(v[3])),
-      "r"(__float_as_uint(v[4])), "r"(__float_as_uint(v[5])), "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])),
-      "r"(__float_as_uint(v[8])), "r"(__float_as_uint(v[9])), "r"(__float_as_uint(v[10])), "r"(__float_as_uint(v[11])),
-      "r"(__float_as_uint(v[12])), "r"(__float_as_uint(v[13])), "r"(__float_as_uint(v[14])), "r"(__float_as_uint(v[15]))
-      : "memory");
-}
-__device__ __forceinline__ void tmem_st_wait() {
-  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-}
 __device__ __forceinline__ void tmem_ld_wait() {
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-}
-
-// byte offset of element (row r, k in 0..31) inside a [rows x 32] fp32 SWIZZLE_128B tile
-__host__ __device__ constexpr uint32_t sw128_off(uint32_t r, uint32_t k) {
-  return r * 128u + ((((k >> 2) ^ (r & 7u)) << 4) | ((k & 3u) << 2));
 }
 
 }  // namespace tc
