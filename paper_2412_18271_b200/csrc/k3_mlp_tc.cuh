@@ -166,6 +166,14 @@ __device__ __forceinline__ void tc_mma_f16(uint32_t d_tmem, uint64_t a_desc, uin
       : "memory");
 }
 
+// one lane of a converged warp (elect.sync: ptxas then knows that a single thread runs the guarded region and moves
+// its operands to uniform registers without a waterfall loop)
+__device__ __forceinline__ bool tc_elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
 // (x0, x1) -> packed (hi, lo): hi = fp16(x) to nearest, lo = fp16(x - hi) (x - hi is exact in fp32)
 __device__ __forceinline__ void tc_split2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
   const __half2 h = __floats2half2_rn(x0, x1);
@@ -470,6 +478,15 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       };
       for (int it = 0; it <= n_my; ++it) {
         const bool have_prev = it >= 1, have_cur = it < n_my;
+        // the NEXT tile's first operand (192 KB, written by K2 and long evicted from L2 by the time K3 runs) is
+        // asked into L2 one tile ahead: its twelve chunk copies then cost an L2 latency instead of a DRAM latency
+        // (with three ring-A slots the DRAM latency paced the whole overlapped block, pfc_k3_timeline)
+        if (it + 1 < n_my) {
+          const uint8_t* nxt = aev16 + (size_t)tile_of(it + 1) * (D0 / TC_KC) * TC_A_SLOT;
+#pragma unroll 1
+          for (int c = 0; c < D0 / TC_KC; ++c)
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nxt + (size_t)c * TC_A_SLOT), "r"((uint32_t)TC_A_SLOT) : "memory");
+        }
         const uint8_t* wprev = have_prev ? P.wpack + (size_t)elem_of(tile_of(it - 1)) * TC_W_BYTES_PER_ELEM : nullptr;
         const uint8_t* wcur = have_cur ? P.wpack + (size_t)elem_of(tile_of(it)) * TC_W_BYTES_PER_ELEM : nullptr;
 #pragma unroll 1
@@ -496,7 +513,13 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
     }
   } else {
     // =========================== MMA issuer ===========================
-    if (lane == 0) {
+    // The WHOLE warp walks the schedule with warp-uniform control flow and operands (ring counters, shared-memory
+    // addresses, the TMEM base taken through a shuffle), so that descriptors and addresses are computed on the
+    // uniform datapath; one elected lane issues the tcgen05.mma / commit instructions.  (With the walk inside `if (lane == 0)`
+    // every MMA was wrapped in an ELECT / R2UR waterfall loop and the issuing thread, not the tensor pipe, paced the
+    // overlapped block: 0.5 us per 32-k chunk against 0.3 us of MMA time, pfc_k3_timeline.)
+    {
+      const uint32_t tbase = __shfl_sync(0xffffffffu, S.tmem_base, 0);
       uint32_t ia = 0, ib = 0;
       uint32_t par_a0 = 0, par_a1 = 0;                         // per-slot phase parities of a0_full / a_full
       // one 32-k chunk: 2 k steps x N_TERMS MMAs of M 128 x N into TMEM column dcol; A from `a_slot`, B from ring slot
@@ -511,15 +534,18 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         for (int ks = 0; ks < 2; ++ks) {
           const uint64_t dah = tc_desc_sw64(a_hi + 32 * ks), dal = tc_desc_sw64(a_lo + 32 * ks);
           const uint64_t dbh = tc_desc_sw64(b_hi + 32 * ks), dbl = tc_desc_sw64(b_lo + 32 * ks);
-          if (N_TERMS == 3) {
-            tc_mma_f16(dcol, dal, dbh, idesc, (first && ks == 0) ? 0u : 1u);
-            tc_mma_f16(dcol, dah, dbl, idesc, 1u);
-            tc_mma_f16(dcol, dah, dbh, idesc, 1u);
-          } else {
-            tc_mma_f16(dcol, dah, dbh, idesc, (first && ks == 0) ? 0u : 1u);
+          if (tc_elect_one()) {
+            if (N_TERMS == 3) {
+              tc_mma_f16(dcol, dal, dbh, idesc, (first && ks == 0) ? 0u : 1u);
+              tc_mma_f16(dcol, dah, dbl, idesc, 1u);
+              tc_mma_f16(dcol, dah, dbh, idesc, 1u);
+            } else {
+              tc_mma_f16(dcol, dah, dbh, idesc, (first && ks == 0) ? 0u : 1u);
+            }
           }
         }
-        tc::mma_commit(&S.b_empty[sb]);
+        if (tc_elect_one()) tc::mma_commit(&S.b_empty[sb]);
+        __syncwarp();
         ++ib;
       };
       // a chunk whose A operand comes through ring A (kind 0: first GEMM, bulk copy; kind 1: chain, 256 producers)
@@ -528,23 +554,23 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         if (kind == 0) { tc::mbar_wait(&S.a0_full[sa], (par_a0 >> sa) & 1u); par_a0 ^= 1u << sa; }
         else           { tc::mbar_wait(&S.a_full[sa], (par_a1 >> sa) & 1u); par_a1 ^= 1u << sa; }
         issue(dcol, tc::smem_u32(ringA + sa * TC_A_SLOT), N, first);
-        tc::mma_commit(&S.a_empty[sa]);
+        if (tc_elect_one()) tc::mma_commit(&S.a_empty[sa]);
         ++ia;
       };
       for (int it = 0; it <= n_my; ++it) {
         const bool have_prev = it >= 1, have_cur = it < n_my;
         const uint32_t par_prev = ((uint32_t)it + 1u) & 1u;
-        TC_TRACE(0);
+        if (tc_elect_one()) TC_TRACE(0);
         // ------------------------------ overlapped block ------------------------------
         bool p5_waited = !have_prev;
-#pragma unroll 1
-        for (int i = 0; i < TC_BLOCK_OPS; ++i) {
+#pragma unroll
+        for (int i = 0; i < TC_BLOCK_OPS; ++i) {                  // (unrolled: the op table folds into constants)
           const int op = tc_block_op(i), c = op & 15;
           if (op >> 8) {                                       // first GEMM of the current tile -> z1
             if (!have_cur) continue;
             if (!p5_waited) { tc::mbar_wait(&S.p5_done, par_prev); p5_waited = true; }   // z1 / d1pre of the previous tile were read
             issue_ring(tbase + TC_COL_Z1, D1, c == 0, 0);
-            if (c == D0 / TC_KC - 1) tc::mma_commit(&S.z_full[0]);
+            if (c == D0 / TC_KC - 1 && tc_elect_one()) tc::mma_commit(&S.z_full[0]);
           } else {                                             // g pass of the previous tile
             if (!have_prev) continue;
             const int pass = (op >> 4) & 3;
@@ -554,29 +580,25 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
             }
             if (pass == 0) tc::mbar_wait(&S.d1_full[c], par_prev);
             issue(tbase + (uint32_t)(pass == 1 ? TC_COL_GB : TC_COL_GA), tc::smem_u32(resD1 + c * TC_A_SLOT), TC_GN, c == 0);
-            if (c == TC_ND1 - 1) {
+            if (c == TC_ND1 - 1 && tc_elect_one()) {
               tc::mma_commit(&S.g_full[pass == 1 ? 1 : 0]);
               if (pass == TC_NPASS - 1) tc::mma_commit(&S.d1_free);
             }
           }
-          TC_TRACE(1 + i);
+          if (tc_elect_one()) TC_TRACE(1 + i);
         }
         if (!have_cur) break;
         // ------------------------------ chain ------------------------------
         for (int c = 0; c < tc_phase_nk(1); ++c) issue_ring(tbase + TC_COL_Z2, tc_phase_n(1), c == 0, 1);
-        tc::mma_commit(&S.z_full[1]);
-        TC_TRACE(28);
+        if (tc_elect_one()) { tc::mma_commit(&S.z_full[1]); TC_TRACE(28); }
         for (int c = 0; c < tc_phase_nk(2); ++c) issue_ring(tbase + TC_COL_Z3, tc_phase_n(2), c == 0, 1);
-        tc::mma_commit(&S.z_full[2]);
-        TC_TRACE(29);
+        if (tc_elect_one()) { tc::mma_commit(&S.z_full[2]); TC_TRACE(29); }
         for (int c = 0; c < tc_phase_nk(3); ++c) issue_ring(tbase + TC_COL_D2, tc_phase_n(3), c == 0, 1);
-        tc::mma_commit(&S.z_full[3]);
-        TC_TRACE(30);
+        if (tc_elect_one()) { tc::mma_commit(&S.z_full[3]); TC_TRACE(30); }
         tc::mbar_wait(&S.dd_full, (uint32_t)it & 1u);            // all of delta2 is in the resident region
         for (int c = 0; c < tc_phase_nk(4); ++c)
           issue(tbase + TC_COL_D1, tc::smem_u32(resD1 + c * TC_A_SLOT), tc_phase_n(4), c == 0);
-        tc::mma_commit(&S.z_full[4]);
-        TC_TRACE(31);
+        if (tc_elect_one()) { tc::mma_commit(&S.z_full[4]); TC_TRACE(31); }
       }
     }
   }
