@@ -16,7 +16,7 @@
 // N_TERMS = 1 is plain FP16 operands, kept only to produce the evidence that a single 16-bit
 // term misses the tolerance.
 //
-// One persistent CTA per SM, 320 threads, 128-row tiles of ONE element each:
+// One persistent CTA per SM, 352 threads, 128-row tiles of ONE element each:
 //   warps 0-7  workers: make the A operand of phases 1-7 in 32-wide K chunks (hi | lo, K-major,
 //              SWIZZLE_64B) from the previous accumulator in TMEM (bias, CELU, CELU', Hadamard), and
 //              drain g;
@@ -24,7 +24,9 @@
 //              from L2 into a 4-slot ring with cp.async.bulk + mbarrier -- and the A operand of
 //              phase 0, which K2 writes in exactly the chunk image the tensor core reads (AEV times 8,
 //              fp16 hi | lo, SWIZZLE_64B; one contiguous 16 KB block per tile and chunk), into ring A;
-//   warp 9     one elected thread issues tcgen05.mma and commits to the ring / phase barriers.
+//   warp 9     walks the MMA schedule; one elected lane issues tcgen05.mma and commits to the ring / phase barriers;
+//   warp 10    TMA: the first GEMM's A operand chunks into ring A (its own thread: no head-of-line blocking behind
+//              the weight stream).
 // Schedule.  The eight phases of a tile are a serial chain (each needs the previous
 // accumulator), except at its two ends: the first GEMM (AEV x W1) depends only on global
 // memory and the three g passes (delta1 x W1^T) only on delta1.  So consecutive tiles are
@@ -49,7 +51,7 @@
 namespace pfc {
 
 constexpr int TC_TM = 128;                       // rows per tile == ROW_PAD
-constexpr int TC_THREADS = 320;
+constexpr int TC_THREADS = 352;
 constexpr int TC_WORKERS = 256;                  // warps 0-7
 constexpr int TC_KC = 32;                        // k per chunk: one 64-byte SWIZZLE_64B row of fp16
 constexpr int TC_NA = 3, TC_NB = 4;              // ring depths: A operand chunks, weight chunks
@@ -177,8 +179,8 @@ __device__ __forceinline__ bool tc_elect_one() {
 // (x0, x1) -> packed (hi, lo): hi = fp16(x) to nearest, lo = fp16(x - hi) (x - hi is exact in fp32)
 __device__ __forceinline__ void tc_split2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
   const __half2 h = __floats2half2_rn(x0, x1);
-  const float2 f = __half22float2(h);
-  const __half2 l = __floats2half2_rn(x0 - f.x, x1 - f.y);
+  const float2 r = pk_fma(__half22float2(h), make_float2(-1.0f, -1.0f), make_float2(x0, x1));   // x - hi, both lanes
+  const __half2 l = __floats2half2_rn(r.x, r.y);
   hi = *reinterpret_cast<const uint32_t*>(&h);
   lo = *reinterpret_cast<const uint32_t*>(&l);
 }
@@ -190,6 +192,22 @@ __device__ __forceinline__ float celu_h(float x) { return fmaxf(x, 0.0f) + fmaf(
 __device__ __forceinline__ void celu_both(float x, float& h, float& d) {
   d = celu_d(x);
   h = fmaxf(x, 0.0f) + fmaf(CELU_ALPHA, d, -CELU_ALPHA);
+}
+// The epilogues work on PAIRS of columns in packed fp32 (fma.rn.f32x2 / mul.rn.f32x2: one issue slot for two lanes of
+// arithmetic, same rounding as the scalar forms): they are bound by instruction issue (16 instructions per element
+// in scalar form, two worker warps per scheduler), not by a pipe.
+//   x = ks z + (kb z + b)   (operand scale, truncation compensation, bias)
+__device__ __forceinline__ float2 tc_affine2(float z0, float z1, float2 ks, float2 kb, float b0, float b1) {
+  const float2 z = make_float2(z0, z1);
+  return pk_fma(z, ks, pk_fma(z, kb, make_float2(b0, b1)));
+}
+__device__ __forceinline__ float2 celu_d2(float2 x) {
+  const float2 a = pk_mul(make_float2(fminf(x.x, 0.0f), fminf(x.y, 0.0f)), make_float2(LOG2E / CELU_ALPHA, LOG2E / CELU_ALPHA));
+  return make_float2(ex2_approx(a.x), ex2_approx(a.y));
+}
+__device__ __forceinline__ float2 celu_h2(float2 x, float2 d) {
+  const float2 t = pk_fma(make_float2(CELU_ALPHA, CELU_ALPHA), d, make_float2(-CELU_ALPHA, -CELU_ALPHA));
+  return pk_fma(make_float2(fmaxf(x.x, 0.0f), fmaxf(x.y, 0.0f)), make_float2(1.0f, 1.0f), t);
 }
 
 // 16 consecutive floats of a 64-byte aligned table (biases, w4) through the read-only path, four 16-byte loads
@@ -315,9 +333,14 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
               tc::tmem_ld_wait();
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
-                auto sc = [&](float v) { return fmaf(v, kgb, v * kg); };
-                stg[lane * 8 + (k ^ (lane & 7))] = make_float4(sc(v0[4 * k]), sc(v0[4 * k + 1]), sc(v0[4 * k + 2]), sc(v0[4 * k + 3]));
-                stg[lane * 8 + ((4 + k) ^ (lane & 7))] = make_float4(sc(v1[4 * k]), sc(v1[4 * k + 1]), sc(v1[4 * k + 2]), sc(v1[4 * k + 3]));
+                auto sc2 = [&](float a, float b) {
+                  const float2 v = make_float2(a, b);
+                  return pk_fma(v, make_float2(kgb, kgb), pk_mul(v, make_float2(kg, kg)));
+                };
+                const float2 a0 = sc2(v0[4 * k], v0[4 * k + 1]), a1 = sc2(v0[4 * k + 2], v0[4 * k + 3]);
+                const float2 b0 = sc2(v1[4 * k], v1[4 * k + 1]), b1 = sc2(v1[4 * k + 2], v1[4 * k + 3]);
+                stg[lane * 8 + (k ^ (lane & 7))] = make_float4(a0.x, a0.y, a1.x, a1.y);
+                stg[lane * 8 + ((4 + k) ^ (lane & 7))] = make_float4(b0.x, b0.y, b1.x, b1.y);
               }
               __syncwarp();
               float* blk = g + (size_t)(row0 + 32 * q) * AEV_LEN + pass * TC_GN + 32 * c;
@@ -336,7 +359,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
           }
         }
       }
-      if (have_cur) ia += D0 / TC_KC;                          // the twelve first-GEMM chunks come by bulk copy (warp 8)
+      if (have_cur) ia += D0 / TC_KC;                          // the twelve first-GEMM chunks come by bulk copy (warp 10)
       if (!have_cur) break;
       // ------------------------------ chain of the current tile ------------------------------
       const int row0 = tile_of(it) * TC_TM;
@@ -345,6 +368,9 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
                   k3 = __ldg(bias + TC_BIAS_KS + 3), k4 = __ldg(bias + TC_BIAS_KS + 4);
       const float c0 = __ldg(bias + TC_BIAS_KB + 0), c1 = __ldg(bias + TC_BIAS_KB + 1), c2 = __ldg(bias + TC_BIAS_KB + 2),
                   c3 = __ldg(bias + TC_BIAS_KB + 3), c4 = __ldg(bias + TC_BIAS_KB + 4);
+      const float2 ks0 = make_float2(k0, k0), ks1 = make_float2(k1, k1), ks2 = make_float2(k2, k2), ks3 = make_float2(k3, k3),
+                   ks4 = make_float2(k4, k4), kb0 = make_float2(c0, c0), kb1 = make_float2(c1, c1), kb2 = make_float2(c2, c2),
+                   kb3 = make_float2(c3, c3), kb4 = make_float2(c4, c4);
       // ---- z1 -> h1 = CELU(z1 + b1): operand of phase 1 ----
       tc::mbar_wait(&S.z_full[0], par);
       tc::tc_fence_after();
@@ -357,7 +383,11 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k0, fmaf(z[k], c0, bb[k])));
+        for (int k = 0; k < 16; k += 2) {
+          const float2 x = tc_affine2(z[k], z[k + 1], ks0, kb0, bb[k], bb[k + 1]);
+          const float2 hh = celu_h2(x, celu_d2(x));
+          h[k] = hh.x; h[k + 1] = hh.y;
+        }
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
@@ -376,7 +406,11 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) h[k] = celu_h(fmaf(z[k], k1, fmaf(z[k], c1, bb[k])));
+        for (int k = 0; k < 16; k += 2) {
+          const float2 x = tc_affine2(z[k], z[k + 1], ks1, kb1, bb[k], bb[k + 1]);
+          const float2 hh = celu_h2(x, celu_d2(x));
+          h[k] = hh.x; h[k + 1] = hh.y;
+        }
         uint8_t* slot = acquire();
         tc_store_a16(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
@@ -388,7 +422,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       tc::tc_fence_after();
       if (tid == 0) TC_TRACE(40);
       {
-        float epart = 0.0f;
+        float2 epart2 = make_float2(0.0f, 0.0f);            // even / odd columns, added at the end
 #pragma unroll 1
         for (int c = 0; c < D3 / TC_KC; ++c) {
           float z[16], dl[16];
@@ -399,18 +433,19 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
           tc_ld16(bias + TC_BIAS_W4 + 32 * c + 16 * hf, w4);
           tc_ld16(bias + TC_BIAS_W4S + 32 * c + 16 * hf, w4s);
 #pragma unroll
-          for (int k = 0; k < 16; ++k) {
-            float h, d;
-            celu_both(fmaf(z[k], k2, fmaf(z[k], c2, bb[k])), h, d);
-            epart = fmaf(w4[k], h, epart);
-            dl[k] = w4s[k] * d;
+          for (int k = 0; k < 16; k += 2) {
+            const float2 x = tc_affine2(z[k], z[k + 1], ks2, kb2, bb[k], bb[k + 1]);
+            const float2 d = celu_d2(x);
+            epart2 = pk_fma(make_float2(w4[k], w4[k + 1]), celu_h2(x, d), epart2);
+            const float2 dd = pk_mul(make_float2(w4s[k], w4s[k + 1]), d);
+            dl[k] = dd.x; dl[k + 1] = dd.y;
           }
           uint8_t* slot = acquire();
           tc_store_a16(slot, r, hf, dl);
           publish(&S.a_full[ia % TC_NA]);
           ++ia;
         }
-        S.epart[hf][r] = epart;
+        S.epart[hf][r] = epart2.x + epart2.y;
         asm volatile("bar.sync 1, %0;" ::"n"(TC_WORKERS) : "memory");
         if (hf == 0) e_row[row0 + r] = (S.epart[0][r] + S.epart[1][r]) + __ldg(bias + TC_BIAS_B4);
       }
@@ -432,7 +467,11 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) p[k] = fmaf(p[k], c3, p[k] * k3) * celu_d(fmaf(z[k], k1, fmaf(z[k], c1, bb[k])));
+        for (int k = 0; k < 16; k += 2) {
+          const float2 pp = make_float2(p[k], p[k + 1]);
+          const float2 t = pk_mul(pk_fma(pp, kb3, pk_mul(pp, ks3)), celu_d2(tc_affine2(z[k], z[k + 1], ks1, kb1, bb[k], bb[k + 1])));
+          p[k] = t.x; p[k + 1] = t.y;
+        }
         tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
       }
       publish(&S.dd_full);
@@ -450,7 +489,11 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float bb[16];
         tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) p[k] = fmaf(p[k], c4, p[k] * k4) * celu_d(fmaf(z[k], k0, fmaf(z[k], c0, bb[k])));
+        for (int k = 0; k < 16; k += 2) {
+          const float2 pp = make_float2(p[k], p[k + 1]);
+          const float2 t = pk_mul(pk_fma(pp, kb4, pk_mul(pp, ks4)), celu_d2(tc_affine2(z[k], z[k + 1], ks0, kb0, bb[k], bb[k + 1])));
+          p[k] = t.x; p[k + 1] = t.y;
+        }
         tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
         publish(&S.d1_full[c]);
       }
@@ -461,14 +504,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
   } else if (warp == 8) {
     // =========================== TMA: weight chunks ===========================
     if (lane == 0) {
-      uint32_t ib = 0, ia = 0;
-      auto stream_a = [&](const uint8_t* src) {                // one first-GEMM operand chunk (hi | lo, as K2 wrote it) into ring A
-        const uint32_t s = ia % TC_NA, use = ia / TC_NA;
-        tc::mbar_wait(&S.a_empty[s], (use & 1u) ^ 1u);
-        tc::mbar_arrive_expect_tx(&S.a0_full[s], (uint32_t)TC_A_SLOT);
-        tc::bulk_g2s(ringA + s * TC_A_SLOT, src, (uint32_t)TC_A_SLOT, &S.a0_full[s]);
-        ++ia;
-      };
+      uint32_t ib = 0;
       auto stream = [&](const uint8_t* src, uint32_t bytes) {
         const uint32_t s = ib % TC_NB, use = ib / TC_NB;
         tc::mbar_wait(&S.b_empty[s], (use & 1u) ^ 1u);
@@ -493,10 +529,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         for (int i = 0; i < TC_BLOCK_OPS; ++i) {
           const int op = tc_block_op(i);
           if (op >> 8) {
-            if (have_cur) {
-              stream_a(aev16 + ((size_t)tile_of(it) * (D0 / TC_KC) + (size_t)(op & 15)) * TC_A_SLOT);
-              stream(wcur + tc_phase_off(0) + (size_t)(op & 15) * tc_chunk_bytes(0), (uint32_t)tc_chunk_bytes(0));
-            }
+            if (have_cur) stream(wcur + tc_phase_off(0) + (size_t)(op & 15) * tc_chunk_bytes(0), (uint32_t)tc_chunk_bytes(0));
           } else if (have_prev) {
             stream(wprev + tc_phase_off(5 + ((op >> 4) & 3)) + (size_t)(op & 15) * tc_chunk_bytes(5), (uint32_t)tc_chunk_bytes(5));
           }
@@ -508,7 +541,34 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
           const uint32_t bytes = (uint32_t)tc_chunk_bytes(p);
           for (int c = 0; c < tc_phase_nk(p); ++c) stream(src + (size_t)c * bytes, bytes);
         }
-        ia += (uint32_t)(tc_phase_nk(1) + tc_phase_nk(2) + tc_phase_nk(3));   // the chain's ring A chunks are made by the workers
+      }
+    }
+  } else if (warp == 10) {
+    // =========================== TMA: the first GEMM's A operand ===========================
+    // its own thread, so that a chunk is requested the moment a ring-A slot frees (up to three chunks ahead, and
+    // already during the previous tile's last epilogues) instead of when the weight stream's walk reaches it
+    if (lane == 0) {
+      uint32_t ia = 0, par_a1 = 0;
+      for (int it = 0; it < n_my; ++it) {
+        const uint8_t* src = aev16 + (size_t)tile_of(it) * (D0 / TC_KC) * TC_A_SLOT;
+#pragma unroll 1
+        for (int c = 0; c < D0 / TC_KC; ++c) {                 // (hi | lo chunk image, as K2 wrote it)
+          const uint32_t s = ia % TC_NA, use = ia / TC_NA;
+          tc::mbar_wait(&S.a_empty[s], (use & 1u) ^ 1u);
+          tc::mbar_arrive_expect_tx(&S.a0_full[s], (uint32_t)TC_A_SLOT);
+          tc::bulk_g2s(ringA + s * TC_A_SLOT, src + (size_t)c * TC_A_SLOT, (uint32_t)TC_A_SLOT, &S.a0_full[s]);
+          ++ia;
+        }
+        // the chain's twelve ring-A chunks are made by the workers.  This thread follows their production (a_full)
+        // before it asks for a slot again: a parity wait on a_empty cannot tell the completion it needs from one
+        // several uses earlier, so it must never be more than one use of a slot ahead
+#pragma unroll 1
+        for (int c = 0; c < tc_phase_nk(1) + tc_phase_nk(2) + tc_phase_nk(3); ++c) {
+          const uint32_t s = ia % TC_NA;
+          tc::mbar_wait(&S.a_full[s], (par_a1 >> s) & 1u);
+          par_a1 ^= 1u << s;
+          ++ia;
+        }
       }
     }
   } else {
