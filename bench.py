@@ -425,7 +425,7 @@ def run_pfc(args):
                 x2, v2 = torch.from_numpy(pfc.pack4(w2.pos)).to(dev), torch.from_numpy(pfc.pack4(w2.vel)).to(dev)
                 with torch.cuda.stream(stream):
                     q.set_state(x2, v2, stream=stream)
-                    q.step(10, DT_FS)
+                    q.step(2 * q.steps_per_graph() + 2, DT_FS)    # warm-up: calibration, and every graph captured
                 stream.synchronize()
                 n2 = 100
                 t2 = _time_steps(torch, q, stream, n2)

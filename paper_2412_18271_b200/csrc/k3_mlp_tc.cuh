@@ -514,15 +514,6 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       };
       for (int it = 0; it <= n_my; ++it) {
         const bool have_prev = it >= 1, have_cur = it < n_my;
-        // the NEXT tile's first operand (192 KB, written by K2 and long evicted from L2 by the time K3 runs) is
-        // asked into L2 one tile ahead: its twelve chunk copies then cost an L2 latency instead of a DRAM latency
-        // (with three ring-A slots the DRAM latency paced the whole overlapped block, pfc_k3_timeline)
-        if (it + 1 < n_my) {
-          const uint8_t* nxt = aev16 + (size_t)tile_of(it + 1) * (D0 / TC_KC) * TC_A_SLOT;
-#pragma unroll 1
-          for (int c = 0; c < D0 / TC_KC; ++c)
-            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nxt + (size_t)c * TC_A_SLOT), "r"((uint32_t)TC_A_SLOT) : "memory");
-        }
         const uint8_t* wprev = have_prev ? P.wpack + (size_t)elem_of(tile_of(it - 1)) * TC_W_BYTES_PER_ELEM : nullptr;
         const uint8_t* wcur = have_cur ? P.wpack + (size_t)elem_of(tile_of(it)) * TC_W_BYTES_PER_ELEM : nullptr;
 #pragma unroll 1
