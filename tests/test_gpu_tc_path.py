@@ -265,3 +265,33 @@ def test_compensation_on_other_weight_sets(pfc, kind):
     bound = np.maximum(RMSD_TOL, COND_FACTOR * sens)
     assert (per_sys <= bound).all(), (kind, np.sort(per_sys / bound)[::-1][:4])
     assert np.median(per_sys) <= 1e-5, np.median(per_sys)
+
+
+def test_auto_goes_back_to_fp32_when_the_calibration_check_fails(pfc, weights):
+    """A weight set the fp16-split operands cannot carry: with a bias of 1e6 on the second hidden layer the
+    activations h2 (the A operand of the third GEMM) exceed fp16's range.  The FP32 MLP evaluates it without
+    trouble; the tensor MLP returns non-finite values on the calibration batch, the check fails, and a
+    PFC_MLP_AUTO handle continues on the FP32 MLP -- whose results are then held to the usual bars."""
+    w = weights.copy()
+    D0, D1, D2, per = 384, 160, 128, 94689
+    for e in range(4):
+        o_b2 = e * per + D1 * D0 + D1 + D2 * D1
+        w[o_b2:o_b2 + D2] += 1.0e6
+    wl = W.make_config(1)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, w, mlp_path=pfc.MLP_AUTO)
+    assert p.mlp_path() == pfc.MLP_TENSOR                      # before the first evaluation: by size
+    E, F = p.energy_forces(_dev(pfc, wl.pos))
+    torch.cuda.synchronize()
+    assert p.mlp_path() == pfc.MLP_FP32 and (p.tc_calibration()[:, 7] == 1).all()
+    assert p.status() == 0
+    ref = oracle.energy_forces(wl.pos.astype(np.float64), wl.species, wl.sys_offsets, w)
+    Eh, Fh = E.cpu().numpy().astype(np.float64), F.cpu().numpy().astype(np.float64)
+    assert (np.abs(Eh - ref["E"]) <= E_RTOL * np.maximum(np.abs(ref["E"]), 1.0)).all()
+    assert np.abs(Fh[:, :3] - ref["F"]).max() <= F_ATOL_INTERNAL * max(1.0, np.abs(ref["F"]).max())
+    p.close()
+    # asked for explicitly, the tensor path stays (and reports what the check saw)
+    q = pfc.Pfc(wl.species, wl.sys_offsets, w, mlp_path=pfc.MLP_TENSOR)
+    q.energy_forces(_dev(pfc, wl.pos))
+    torch.cuda.synchronize()
+    assert q.mlp_path() == pfc.MLP_TENSOR and (q.tc_calibration()[:, 7] == 0).all()
+    q.close()
