@@ -287,7 +287,8 @@ def run_pfc(args):
         wl = dataclasses.replace(wl, name=f"{wl.name}_first{args.replicas}")
     N = wl.n_atoms
     stream = torch.cuda.Stream(device=dev)
-    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=args.mlp, device=dev)
+    tuning = pfc.Tuning(skin_list=1) if args.skin else None
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=args.mlp, device=dev, tuning=tuning)
     mlp = p.mlp_path()                                            # MLP_AUTO resolved by pfc_create
     pos0, vel0 = pfc.pack4(wl.pos), pfc.pack4(wl.vel)
     pos, vel = torch.from_numpy(pos0).to(dev), torch.from_numpy(vel0).to(dev)
@@ -408,7 +409,7 @@ def run_pfc(args):
             "config": _config_dict(args, wl),
             "path": {"mlp_path": "fp32_ffma" if mlp == 0 else "f16x3_tcgen05",
                      "mlp_path_requested": {0: "fp32", 1: "tensor", 2: "tensor_1term", 3: "auto"}[args.mlp],
-                     "steps_per_graph": p.steps_per_graph()},
+                     "steps_per_graph": p.steps_per_graph(), "skin_list": bool(args.skin)},
             "ns_per_day_per_replica": steps_per_s * DT_FS * 1e-6 * 86400,
             "ns_per_day_aggregate": steps_per_s * DT_FS * 1e-6 * 86400 * wl.n_systems * world,
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_step * args.steps,
@@ -455,6 +456,9 @@ def main():
     ap.add_argument("--mlp", type=int, default=3, choices=[0, 1, 3],
                     help="3 = auto (library default: tensor-core MLP from 4096 atoms on), 0 = FP32 FFMA, 1 = tcgen05 fp16 split")
     ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (100 steps each)")
+    ap.add_argument("--skin", action="store_true",
+                    help="cell-list systems (config 3): neighbour candidates with a 0.5 A skin, reused between rebuilds "
+                         "(pfc_tuning_t.skin_list; off by default)")
     ap.add_argument("--replicas", type=int, default=0,
                     help="configs 1 and 4 only: the first N replicas instead of all (profiling / sanitizer runs; "
                          "the workload name in the JSON line says so)")

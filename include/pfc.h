@@ -93,7 +93,10 @@ typedef struct {
   int32_t k3_cluster;         /* FP32 MLP of a batch of at most 18 16-row tiles (a single small molecule): 0 = one
                                  cluster of 8 CTAs per tile (unless k3_tile_rows / k3_deep_ring ask for a variant);
                                  1 = never; 2 = required (PFC_ERR_ARG if the batch has more tiles) */
-  int32_t reserved;           /* must be 0 */
+  int32_t skin_list;          /* systems above 2,048 atoms (cell list): 0 = neighbour rows rebuilt from the cell list every
+                                 evaluation (default); 1 = candidate rows with a 0.5 A skin, rebuilt only when an atom
+                                 has moved more than 0.25 A since the build, the exact predicate applied to the candidates
+                                 every evaluation (the lists are the same bit for bit; pays when atoms move slowly) */
 } pfc_tuning_t;
 
 typedef struct pfc_ctx pfc_t;           /* opaque; owned by the library          */

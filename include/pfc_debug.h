@@ -20,9 +20,10 @@ extern "C" {
 #define PFC_N_STAGES 7
 int pfc_profile_stages(pfc_t *ctx, const float *pos, float *E, float *F, void *stream, float *ms);
 
-/* Work counts of the last evaluation, for the roofline arithmetic: counts HOST [4] =
+/* Work counts of the last evaluation, for the roofline arithmetic: counts HOST [5] =
  * {radial row entries, angular row entries, triples (sum over atoms of m(m-1)/2, m = angular
- * neighbours), brute-force distance tests per evaluation}.  Synchronises the handle's stream. */
+ * neighbours), brute-force distance tests per evaluation, candidate-row builds of the cell-list
+ * systems since pfc_create (skin list: far fewer than evaluations)}.  Synchronises the handle's stream. */
 int pfc_work_counts(pfc_t *ctx, int64_t *counts);
 
 /* Timeline of the tensor-core MLP kernel (one relaunch of K3 on the AEV rows of the last evaluation; the

@@ -14,10 +14,17 @@
 //  * brute force (systems <= BRUTE_MAX atoms): one CTA per work item = (system, block of its
 //    atoms); the system's positions are staged in shared memory once, one warp per atom scans
 //    them 32 at a time; ordered compaction is ballot + popc, no sort.
-//  * cell list (systems > BRUTE_MAX atoms): per-step bounding box, cells of
-//    edge >= 5.2*(1+2^-10), atoms binned per cell, 27-cell stencil walked by one warp per atom
-//    into a shared-memory row, ordered by index with a rank-by-count pass.  The same predicate
-//    decides membership.
+//  * cell list (systems > BRUTE_MAX atoms): per-evaluation bounding box, cells of edge >= 5.2*(1+2^-10), atoms
+//    binned per cell, 27-cell stencil walked by one warp per atom into a shared-memory row, ordered by index
+//    with a rank-by-count pass.  The same predicate decides membership.
+//  * the same with a skin (pfc_tuning_t.skin_list = 1): a CANDIDATE row per
+//    atom -- every j with d2 < (RC_R + SKIN)^2, ascending index -- is built through a cell list (bounding box,
+//    cells of edge >= (RC_R + SKIN)(1+2^-10), atoms binned per cell, 27-cell stencil walked by one warp per atom
+//    into a shared-memory row, ordered by index with a rank-by-count pass) and REUSED while no atom of the
+//    system set has moved more than SKIN/2 from where it stood at the build (checked every evaluation on the
+//    device; the build kernels return at once when the flag is clear).  Every evaluation a refresh kernel
+//    applies the exact predicate to the candidates: the rows it writes are the same, bit for bit, as a
+//    fresh build would give (any pair within RC_R now was within RC_R + SKIN at the build).
 #pragma once
 #include "pfc_common.cuh"
 
@@ -170,16 +177,40 @@ struct CellGrid {          // one per cell-list system, in device memory
 constexpr int CELL_THREADS = 1024;          // one CTA per cell-list system walks all its atoms / cells
 // 2^-10 of slack: binning round-off ((x-lo)*inv_edge carries ~nc*1.2e-7 of error) can never
 // put two atoms closer than the cutoff into non-adjacent cells; the predicate decides.
-constexpr float CELL_EDGE_MIN = 5.2f * (1.0f + 9.765625e-4f);
+constexpr float SKIN = 0.5f;                // A
+constexpr float RC_CAND = RC_R + SKIN;      // candidate cutoff 5.7 A
+constexpr float RC2_CAND = RC_CAND * RC_CAND * (1.0f + 1e-4f);     // (margins: fp32 rounding of the two tests is ~1e-7)
+constexpr float SKIN_MOVE2 = 0.249f * 0.249f;                      // rebuild when an atom moved further than this (< SKIN/2)
+constexpr int CAND_CAP = 384;               // candidates per atom (bulk at 0.1 / A^3: 78); twice the row capacity
+constexpr float CELL_EDGE_MIN = RC_R * (1.0f + 9.765625e-4f);            // skin list off
+constexpr float CELL_EDGE_MIN_SKIN = RC_CAND * (1.0f + 9.765625e-4f);    // skin list on
+// skin state words (device): [0] rebuild flag, [1] builds so far, [2] the constant 1 (the build kernels' flag
+// when the skin list is off: they then run every evaluation)
+constexpr int SKIN_FLAG = 0, SKIN_BUILDS = 1, SKIN_ALWAYS = 2;
+
+// any atom further than SKIN/2 from its position at the last build (or a non-finite coordinate) -> rebuild
+__global__ void k1_skin_check_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
+                                     const float4* __restrict__ pos, const float4* __restrict__ x_build,
+                                     int* __restrict__ skin_state) {
+  const int q = blockIdx.x * blockDim.x + threadIdx.x;
+  bool moved = false;
+  if (q < n_cell_atoms) {
+    const float4 p = pos[cell_atom_list[q]], b = x_build[q];
+    const float dx = p.x - b.x, dy = p.y - b.y, dz = p.z - b.z;
+    moved = !(dx * dx + dy * dy + dz * dz <= SKIN_MOVE2);
+  }
+  if (__any_sync(0xffffffffu, moved) && lane_id() == 0) atomicOr(&skin_state[SKIN_FLAG], 1);
+}
 
 // one CTA per cell-list system: bounding box -> grid; zero the cell counters
 __global__ void __launch_bounds__(CELL_THREADS)
-k1_cell_grid_kernel(const int* __restrict__ cell_sys, const int* __restrict__ sys_off,
+k1_cell_grid_kernel(const int* __restrict__ skin_state, const int* __restrict__ cell_sys, const int* __restrict__ sys_off,
                     const int* __restrict__ cell_cap_base, const float4* __restrict__ pos,
                     CellGrid* __restrict__ grids, int* __restrict__ cell_count,
-                    uint32_t* __restrict__ status) {
+                    uint32_t* __restrict__ status, float edge_min) {
   __shared__ float smin[3][CELL_THREADS / 32], smax[3][CELL_THREADS / 32];
   __shared__ CellGrid g;
+  if (skin_state[SKIN_FLAG] == 0) return;        // the candidate rows are still valid
   int cs = blockIdx.x, sid = cell_sys[cs];
   int b = sys_off[sid], e = sys_off[sid + 1];
   float lo[3] = {3e38f, 3e38f, 3e38f}, hi[3] = {-3e38f, -3e38f, -3e38f};
@@ -209,7 +240,7 @@ k1_cell_grid_kernel(const int* __restrict__ cell_sys, const int* __restrict__ sy
     }
     // cells of edge >= CELL_EDGE_MIN; if the grid would exceed its capacity
     // (an expanding cluster), grow the edge -- larger cells are still correct.
-    float edge = CELL_EDGE_MIN;
+    float edge = edge_min;
     for (int it = 0; it < 64; ++it) {
       long long tot = 1;
       for (int d = 0; d < 3; ++d) { g.nc[d] = max(1, (int)floorf(ext[d] / edge)); tot *= g.nc[d]; }
@@ -221,7 +252,7 @@ k1_cell_grid_kernel(const int* __restrict__ cell_sys, const int* __restrict__ sy
       atomicOr(status, ST_CELL_OVERFLOW);
     }
     for (int d = 0; d < 3; ++d) {
-      float ce = fmaxf(ext[d] / (float)g.nc[d], edge);   // actual edge >= CELL_EDGE_MIN
+      float ce = fmaxf(ext[d] / (float)g.nc[d], edge);   // actual edge >= edge_min
       g.inv_edge[d] = 1.0f / ce;
     }
     g.cell_base = cell_cap_base[cs];
@@ -238,12 +269,13 @@ __device__ __forceinline__ int cell_coord(float x, float lo, float inv_edge, int
 }
 
 // per atom of a cell-list system: cell id + histogram
-__global__ void k1_cell_assign_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
+__global__ void k1_cell_assign_kernel(const int* __restrict__ skin_state, int n_cell_atoms,
+                                      const int* __restrict__ cell_atom_list,
                                       const int* __restrict__ atom_cell_sys,
                                       const float4* __restrict__ pos, const CellGrid* __restrict__ grids,
                                       int* __restrict__ atom_cell, int* __restrict__ cell_count) {
   int q = blockIdx.x * blockDim.x + threadIdx.x;
-  if (q >= n_cell_atoms) return;
+  if (q >= n_cell_atoms || skin_state[SKIN_FLAG] == 0) return;
   int i = cell_atom_list[q];
   const CellGrid& g = grids[atom_cell_sys[q]];
   float4 p = pos[i];
@@ -258,11 +290,13 @@ __global__ void k1_cell_assign_kernel(int n_cell_atoms, const int* __restrict__ 
 // one CTA per cell-list system: exclusive scan of its cell histogram -> cell_start
 // (pooled, relative to the system's first slot), and reset the fill cursors.
 __global__ void __launch_bounds__(CELL_THREADS)
-k1_cell_scan_kernel(const int* __restrict__ cell_sys, const int* __restrict__ cell_slot_base,
+k1_cell_scan_kernel(const int* __restrict__ skin_state, const int* __restrict__ cell_sys,
+                    const int* __restrict__ cell_slot_base,
                     const CellGrid* __restrict__ grids, const int* __restrict__ cell_count,
                     int* __restrict__ cell_start, int* __restrict__ cell_cursor) {
   __shared__ int wsum[CELL_THREADS / 32];
   __shared__ int carry;
+  if (skin_state[SKIN_FLAG] == 0) return;
   const CellGrid g = grids[blockIdx.x];
   if (threadIdx.x == 0) carry = cell_slot_base[blockIdx.x];
   __syncthreads();
@@ -292,22 +326,23 @@ k1_cell_scan_kernel(const int* __restrict__ cell_sys, const int* __restrict__ ce
 // ordered by index afterwards, so the final lists do not depend on it)
 // cell_xyz[slot] = {x, y, z, bitcast(atom index | species << 29)}: the rows kernel streams a cell
 // line's positions contiguously instead of gathering pos[cell_atoms[p]] (two dependent loads per round)
-__global__ void k1_cell_fill_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
+__global__ void k1_cell_fill_kernel(const int* __restrict__ skin_state, int n_cell_atoms,
+                                    const int* __restrict__ cell_atom_list,
                                     const int* __restrict__ atom_cell, const float4* __restrict__ pos,
                                     const int* __restrict__ species,
                                     int* __restrict__ cell_cursor, float4* __restrict__ cell_xyz) {
   int q = blockIdx.x * blockDim.x + threadIdx.x;
-  if (q >= n_cell_atoms) return;
+  if (q >= n_cell_atoms || skin_state[SKIN_FLAG] == 0) return;
   int slot = atomicAdd(&cell_cursor[atom_cell[q]], 1);
   const int i = cell_atom_list[q];
   const float4 p = pos[i];
   cell_xyz[slot] = make_float4(p.x, p.y, p.z, __int_as_float(i | (species[i] << 29)));
 }
 
-// neighbour rows through the cell list: one warp per atom, one pass.  The row is collected
+constexpr int CELL_ROW_MAX = 512;        // longest row the in-warp ordering supports
+// neighbour rows through the cell list (skin list off: the default), one warp per atom, one pass.  The row is collected
 // unordered in shared memory, then ordered by index with a rank-by-count pass (all indices are
 // distinct) straight into the atom's fixed-capacity row.
-constexpr int CELL_ROW_MAX = 512;        // longest radial row the in-warp ordering supports
 __global__ void __launch_bounds__(K1_WARPS * 32)
 k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
                     const int* __restrict__ atom_cell_sys, const int* __restrict__ atom_cell,
@@ -375,6 +410,120 @@ k1_cell_rows_kernel(int n_cell_atoms, const int* __restrict__ cell_atom_list,
   for (int o = 16; o > 0; o >>= 1) na += __shfl_xor_sync(0xffffffffu, na, o);
   if (lane == 0) cnt[i] = make_int2(min(n, cap), na);
 }
+
+
+// candidate rows through the cell list: one warp per atom, one pass.  The row is collected
+// unordered in shared memory, then ordered by index with a rank-by-count pass (all indices are
+// distinct) into the atom's candidate row; the atom's position at this build is kept for the skin check.
+__global__ void __launch_bounds__(K1_WARPS * 32)
+k1_cell_cand_kernel(int* __restrict__ skin_state, int n_cell_atoms, const int* __restrict__ cell_atom_list,
+                    const int* __restrict__ atom_cell_sys, const int* __restrict__ atom_cell,
+                    const float4* __restrict__ pos, const CellGrid* __restrict__ grids,
+                    const int* __restrict__ cell_start, const float4* __restrict__ cell_xyz,
+                    uint32_t* __restrict__ cand, int* __restrict__ ccnt, float4* __restrict__ x_build,
+                    uint32_t* __restrict__ status) {
+  __shared__ uint32_t srow[K1_WARPS][CELL_ROW_MAX];
+  int q = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
+  if (q >= n_cell_atoms || skin_state[SKIN_FLAG] == 0) return;
+  const uint32_t lane = lane_id(), lt = lanemask_lt();
+  uint32_t* row = srow[threadIdx.x >> 5];
+  int i = cell_atom_list[q];
+  const CellGrid g = grids[atom_cell_sys[q]];
+  float4 pi = pos[i];
+  if (lane == 0) {
+    x_build[q] = pi;
+    if (q == 0) atomicAdd(&skin_state[SKIN_BUILDS], 1);
+  }
+  int c = atom_cell[q] - g.cell_base;
+  int cx = c % g.nc[0], cy = (c / g.nc[0]) % g.nc[1], cz = c / (g.nc[0] * g.nc[1]);
+  int nr = 0;
+  for (int z = max(cz - 1, 0); z <= min(cz + 1, g.nc[2] - 1); ++z)
+    for (int y = max(cy - 1, 0); y <= min(cy + 1, g.nc[1] - 1); ++y) {
+      // cells x-1..x+1 of one (y,z) line are contiguous in the pooled array
+      int c0 = g.cell_base + (z * g.nc[1] + y) * g.nc[0] + max(cx - 1, 0);
+      int c1 = g.cell_base + (z * g.nc[1] + y) * g.nc[0] + min(cx + 1, g.nc[0] - 1);
+      int s0 = cell_start[c0], s1 = cell_start[c1 + 1];
+      for (int p0 = s0; p0 < s1; p0 += 32) {
+        int p = p0 + (int)lane;
+        uint32_t w = 0;
+        float d2 = 1e30f;
+        if (p < s1) {
+          const float4 pj = cell_xyz[p];
+          w = (uint32_t)__float_as_int(pj.w);
+          if (nbr_index(w) != i) d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+        }
+        uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_CAND);
+        int slot = nr + __popc(mr & lt);
+        if (d2 < RC2_CAND && slot < CELL_ROW_MAX) row[slot] = w;
+        nr += __popc(mr);
+      }
+    }
+  if (nr > CAND_CAP && lane == 0) atomicOr(status, ST_RADIAL_OVERFLOW);
+  const int n = min(nr, CELL_ROW_MAX);
+  __syncwarp();
+  // order by index: rank = number of smaller entries (entries are distinct); keep the first CAND_CAP
+  uint32_t* out = cand + (size_t)q * CAND_CAP;
+  for (int s = lane; s < n; s += 32) {
+    const uint32_t v = row[s];
+    const int key = nbr_index(v);
+    int rank = 0;
+    for (int t = 0; t < n; ++t) rank += (nbr_index(row[t]) < key);
+    if (rank < CAND_CAP) out[rank] = v;
+  }
+  if (lane == 0) ccnt[q] = min(n, CAND_CAP);
+}
+
+// every evaluation: the exact predicate on the candidates (ascending index, so the row comes out ordered) ->
+// the atom's fixed-capacity neighbour row, exactly as a fresh cell-list pass would write it.  Also the
+// packed position copies K2 / K4a read; and the skin flag is cleared (the build kernels, earlier on the
+// stream, have all seen it).
+__global__ void __launch_bounds__(K1_WARPS * 32)
+k1_skin_refresh_kernel(int* __restrict__ skin_state, int n_cell_atoms, const int* __restrict__ cell_atom_list,
+                       const float4* __restrict__ pos, const int* __restrict__ species,
+                       const float4* __restrict__ xlo, const uint32_t* __restrict__ cand, const int* __restrict__ ccnt,
+                       float4* __restrict__ xs, float4* __restrict__ xsl,
+                       const int* __restrict__ row_beg, uint32_t* __restrict__ nbr, int2* __restrict__ cnt,
+                       uint32_t* __restrict__ status) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) skin_state[SKIN_FLAG] = 0;
+  const int q = blockIdx.x * K1_WARPS + (threadIdx.x >> 5);
+  if (q >= n_cell_atoms) return;
+  const uint32_t lane = lane_id(), lt = lanemask_lt();
+  const int i = cell_atom_list[q];
+  const float4 pi = pos[i];
+  if (lane == 0) {
+    float4 o = pi;
+    o.w = __int_as_float(species[i]);
+    xs[i] = o;
+    xsl[i] = xlo ? xlo[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+  }
+  const int beg = row_beg[i], cap = row_beg[i + 1] - beg;
+  const uint32_t* row = cand + (size_t)q * CAND_CAP;
+  const int nc = ccnt[q];
+  int nr = 0, na = 0;
+  for (int k0 = 0; k0 < nc; k0 += 32) {
+    const int k = k0 + (int)lane;
+    uint32_t w = 0;
+    float d2 = 1e30f;
+    if (k < nc) {
+      w = row[k];
+      const float4 pj = pos[nbr_index(w)];
+      d2 = dist2_rn(pi.x, pi.y, pi.z, pj.x, pj.y, pj.z);
+    }
+    const uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
+    const int slot = nr + __popc(mr & lt);
+    const bool stored = d2 < RC2_R && slot < cap;
+    const bool ang = d2 < RC2_A;
+    if (stored) nbr[beg + slot] = w | (ang ? 0x80000000u : 0u);
+    na += __popc(__ballot_sync(0xffffffffu, stored && ang));
+    nr += __popc(mr);
+  }
+  if (lane == 0) {
+    if (nr > cap) atomicOr(status, ST_RADIAL_OVERFLOW);
+    cnt[i] = make_int2(min(nr, cap), na);
+  }
+}
+
+__global__ void k1_skin_invalidate_kernel(int* __restrict__ skin_state) { skin_state[SKIN_FLAG] = 1; }
 
 // ---- CSR export (pfc_get_neighbors; not on the step path) ----------------------------------
 // r_off / a_off come from k1_scan_* over cnt; this copies the rows into the canonical int32 CSR of

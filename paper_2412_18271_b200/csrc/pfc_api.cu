@@ -65,7 +65,11 @@ struct Buffers {
   int* row_beg;                 // [N+1] first entry of every atom's fixed-capacity neighbour row
   uint32_t* nbr;                // [cap_r] entry words (k1_neighbors.cuh)
   int2 *cnt, *block_tot;
-  int *r_off, *a_off, *r_idx, *a_idx;   // CSR export (pfc_get_neighbors only)
+  int *r_off, *a_off, *r_idx, *a_idx;   // CSR export (pfc_get_neighbors only); r_idx | a_idx are one block ...
+  uint32_t* cand;               // ... which between exports holds the cell-list systems' candidate rows (skin list)
+  int* ccnt;                    // [cell atoms] candidates per atom
+  float4* x_build;              // [cell atoms] positions at the last candidate build
+  int* skin_state;              // [4] {rebuild flag, builds so far}
   float *aev, *g, *e_row;       // aev: fp32 rows (FP32 MLP) or the packed fp16 operand image (tensor MLP), same bytes
   float* aev_unpacked;          // pfc_get_intermediates on the tensor path; calibration: fp32 AEV rows, then the FP32 MLP's g
   float* e_ref;                 // calibration: the FP32 MLP's per-row energies
@@ -105,8 +109,9 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.block_tot = c.take<int2>((size_t)s.n_scan_blocks);
   t.r_off = c.take<int>(N + 1);
   t.a_off = c.take<int>(N + 1);
-  t.r_idx = c.take<int>((size_t)s.cap_r);
-  t.a_idx = c.take<int>((size_t)s.cap_r);
+  t.r_idx = c.take<int>(2 * (size_t)s.cap_r);             // r_idx | a_idx contiguous: 2 x 192 = CAND_CAP words per cell-list atom
+  t.a_idx = t.r_idx ? t.r_idx + s.cap_r : nullptr;
+  t.cand = (uint32_t*)t.r_idx;
   t.aev = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.g = c.take<float>((size_t)s.n_rows * AEV_LEN);
   t.aev_unpacked = c.take<float>((size_t)s.n_rows * AEV_LEN);
@@ -132,6 +137,9 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.atom_cell_sys = c.take<int>((size_t)s.n_cell_atoms + 1);
   t.atom_cell = c.take<int>((size_t)s.n_cell_atoms + 1);
   t.cell_xyz = c.take<float4>((size_t)s.n_cell_atoms + 1);
+  t.x_build = c.take<float4>((size_t)s.n_cell_atoms + 1);
+  t.ccnt = c.take<int>((size_t)s.n_cell_atoms + 1);
+  t.skin_state = c.take<int>(4);
   t.cell_count = c.take<int>((size_t)s.cell_slots + 1);
   t.cell_start = c.take<int>((size_t)s.cell_slots + 1);
   t.cell_cursor = c.take<int>((size_t)s.cell_slots + 1);
@@ -188,6 +196,7 @@ struct pfc_ctx {
   Buffers b;
   MlpParams mlp;
   ClParams clp;
+  bool skin_list = false;       // cell-list systems: candidate rows with a skin, reused between rebuilds (pfc_tuning_t.skin_list)
   bool mlp_cluster = false;     // FP32 MLP of a batch of <= CL_MAX_TILES 16-row tiles: one cluster of 8 CTAs per tile
   TcParams tcp;
   int device = 0;               // the CUDA device the handle was created on
@@ -254,17 +263,30 @@ void enqueue_k1(pfc_ctx* c, const float4* pos, bool with_xlo, cudaStream_t st) {
            b.row_beg, b.nbr, b.cnt, b.status);
   if (c->n_cell_sys > 0) {
     const int nca = c->n_cell_atoms;
-    LAUNCH(c, k1_cell_grid_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.sys_off, b.cell_cap_base,
-           pos, b.grids, b.cell_count, b.status);
-    LAUNCH(c, k1_cell_assign_kernel, cdiv(nca, 256), 256, 0, st, nca, b.cell_atom_list, b.atom_cell_sys, pos,
+    // skin list on: has any atom moved more than SKIN/2 since the candidate rows were built?  If so the five
+    // build kernels run (they return at once otherwise); then the exact predicate on the candidates, every time.
+    // Off (the default): the build kernels see a flag that is always set and write the rows themselves.
+    const int* flag = c->skin_list ? b.skin_state : b.skin_state + SKIN_ALWAYS;
+    if (c->skin_list)
+      LAUNCH(c, k1_skin_check_kernel, cdiv(nca, 256), 256, 0, st, nca, b.cell_atom_list, pos, b.x_build, b.skin_state);
+    LAUNCH(c, k1_cell_grid_kernel, c->n_cell_sys, CELL_THREADS, 0, st, flag, b.cell_sys, b.sys_off, b.cell_cap_base,
+           pos, b.grids, b.cell_count, b.status, c->skin_list ? CELL_EDGE_MIN_SKIN : CELL_EDGE_MIN);
+    LAUNCH(c, k1_cell_assign_kernel, cdiv(nca, 256), 256, 0, st, flag, nca, b.cell_atom_list, b.atom_cell_sys, pos,
            b.grids, b.atom_cell, b.cell_count);
-    LAUNCH(c, k1_cell_scan_kernel, c->n_cell_sys, CELL_THREADS, 0, st, b.cell_sys, b.cell_slot_base, b.grids,
+    LAUNCH(c, k1_cell_scan_kernel, c->n_cell_sys, CELL_THREADS, 0, st, flag, b.cell_sys, b.cell_slot_base, b.grids,
            b.cell_count, b.cell_start, b.cell_cursor);
-    LAUNCH(c, k1_cell_fill_kernel, cdiv(nca, 256), 256, 0, st, nca, b.cell_atom_list, b.atom_cell,
+    LAUNCH(c, k1_cell_fill_kernel, cdiv(nca, 256), 256, 0, st, flag, nca, b.cell_atom_list, b.atom_cell,
            pos, b.species, b.cell_cursor, b.cell_xyz);
-    LAUNCH(c, k1_cell_rows_kernel, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
-           b.atom_cell_sys, b.atom_cell, pos, b.species, xlo, b.grids, b.cell_start, b.cell_xyz, b.xs, b.xsl,
-           b.row_beg, b.nbr, b.cnt, b.status);
+    if (c->skin_list) {
+      LAUNCH(c, k1_cell_cand_kernel, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, b.skin_state, nca, b.cell_atom_list,
+             b.atom_cell_sys, b.atom_cell, pos, b.grids, b.cell_start, b.cell_xyz, b.cand, b.ccnt, b.x_build, b.status);
+      LAUNCH(c, k1_skin_refresh_kernel, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, b.skin_state, nca, b.cell_atom_list,
+             pos, b.species, xlo, b.cand, b.ccnt, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt, b.status);
+    } else {
+      LAUNCH(c, k1_cell_rows_kernel, cdiv(nca, K1_WARPS), K1_WARPS * 32, 0, st, nca, b.cell_atom_list,
+             b.atom_cell_sys, b.atom_cell, pos, b.species, xlo, b.grids, b.cell_start, b.cell_xyz, b.xs, b.xsl,
+             b.row_beg, b.nbr, b.cnt, b.status);
+    }
   }
 }
 
@@ -559,13 +581,14 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
       tun.k3_tile_rows != 128)
     return PFC_ERR_ARG;
   if (tun.k3_deep_ring < 0 || tun.k3_deep_ring > 2 || tun.steps_per_graph < 0 || tun.steps_per_graph > 256 ||
-      tun.k3_cluster < 0 || tun.k3_cluster > 2 || tun.reserved != 0)
+      tun.k3_cluster < 0 || tun.k3_cluster > 2 || tun.skin_list < 0 || tun.skin_list > 1)
     return PFC_ERR_ARG;
 
   pfc_ctx* c = new (std::nothrow) pfc_ctx();
   if (!c) return PFC_ERR_ARG;
   if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
   if (tun.steps_per_graph > 0) c->steps_per_graph = tun.steps_per_graph;
+  c->skin_list = tun.skin_list == 1;
   // AUTO: the tensor-core MLP pays from about 4,000 atoms on, where its 128-row tiles start to fill the
   // SMs.  Measured ms/step, FFMA vs tensor, replicas of config 1: 2,200 atoms 0.108 / 0.111, 3,960
   // 0.113 / 0.115, 4,840 0.136 / 0.121, 5,632 0.139 / 0.124; of config 4: 3,758 atoms 0.143 / 0.145,
@@ -796,6 +819,10 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (cudaMemset(b.aev_unpacked, 0, sizeof(float) * (size_t)c->sz.n_rows * AEV_LEN) != cudaSuccess) ok = false;
   if (cudaMemset(b.status, 0, 256) != cudaSuccess) ok = false;
   if (cudaMemset(b.work, 0, 64) != cudaSuccess) ok = false;
+  {
+    const int skin0[4] = {1, 0, 1, 0};                  // no candidate rows yet: the first evaluation builds them; [2] = always 1
+    up(b.skin_state, skin0, sizeof(skin0));
+  }
   if (c->k1_smem > 48 * 1024 &&
       cudaFuncSetAttribute(k1_brute_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->k1_smem) != cudaSuccess)
     ok = false;
@@ -838,7 +865,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (cudaDeviceSynchronize() != cudaSuccess) ok = false;
   if (!ok) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
   // launch counts (static: depends only on the configuration)
-  c->launches_ef = 5 + (c->n_items > 0 ? 1 : 0) + (c->n_cell_sys > 0 ? 5 : 0);
+  c->launches_ef = 5 + (c->n_items > 0 ? 1 : 0) + (c->n_cell_sys > 0 ? (c->skin_list ? 7 : 5) : 0);
   c->launches_step = c->launches_ef;            // integrator kernel + forces, no energy sum inside a pfc_step call
   *out = c;
   return PFC_OK;
@@ -970,6 +997,10 @@ int pfc_work_counts(pfc_t* c, int64_t* counts) {
   if (cudaStreamSynchronize(st) != cudaSuccess) return PFC_ERR_CUDA;
   counts[0] = (int64_t)h[0]; counts[1] = (int64_t)h[1]; counts[2] = (int64_t)h[2];
   counts[3] = (int64_t)c->brute_tests;
+  int builds = 0;
+  if (c->n_cell_sys > 0 && cudaMemcpy(&builds, c->b.skin_state + SKIN_BUILDS, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess)
+    return PFC_ERR_CUDA;
+  counts[4] = (int64_t)builds;
   return PFC_OK;
 }
 
@@ -1136,6 +1167,8 @@ int pfc_get_neighbors(pfc_t* c, const int32_t** r_off, const int32_t** r_idx, co
   k1_scan_kernel<<<s.n_scan_blocks, SCAN_THREADS, 0, st>>>(s.n_atoms, b.cnt, b.block_tot, b.r_off, b.a_off);
   k1_export_csr_kernel<<<cdiv(s.n_atoms, K1_WARPS), K1_WARPS * 32, 0, st>>>(s.n_atoms, b.row_beg, b.nbr, b.cnt, b.r_off,
                                                                           b.a_off, b.r_idx, b.a_idx);
+  // the export overwrote the block that holds the candidate rows of cell-list systems: rebuild them next time
+  if (c->n_cell_sys > 0 && c->skin_list) k1_skin_invalidate_kernel<<<1, 1, 0, st>>>(b.skin_state);
   if (cudaGetLastError() != cudaSuccess) return PFC_ERR_CUDA;
   if (r_off) *r_off = b.r_off;
   if (r_idx) *r_idx = b.r_idx;

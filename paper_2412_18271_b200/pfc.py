@@ -48,7 +48,7 @@ class Tuning(ctypes.Structure):
     """pfc_tuning_t (include/pfc.h): a zero-filled struct is "all defaults"."""
     _fields_ = [("k3_tile_rows", c_int32), ("k3_deep_ring", c_int32), ("tc_comp_override", c_int32),
                 ("tc_comp_forward", c_float), ("tc_comp_backward", c_float), ("steps_per_graph", c_int32),
-                ("k3_cluster", c_int32), ("reserved", c_int32)]
+                ("k3_cluster", c_int32), ("skin_list", c_int32)]
 
 
 class _Desc(ctypes.Structure):
@@ -325,10 +325,11 @@ class Pfc:
 
     @_on_device
     def work_counts(self):
-        """Row totals of the last evaluation: dict(radial, angular, triples, brute_tests); synchronises."""
-        v = (ctypes.c_int64 * 4)()
+        """Row totals of the last evaluation: dict(radial, angular, triples, brute_tests, skin_builds); synchronises."""
+        v = (ctypes.c_int64 * 5)()
         _check(self._lib.pfc_work_counts(self._h, v), "pfc_work_counts")
-        return {"radial": int(v[0]), "angular": int(v[1]), "triples": int(v[2]), "brute_tests": int(v[3])}
+        return {"radial": int(v[0]), "angular": int(v[1]), "triples": int(v[2]), "brute_tests": int(v[3]),
+                "skin_builds": int(v[4])}
 
     @_on_device
     def neighbors(self):

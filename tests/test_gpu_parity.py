@@ -440,6 +440,35 @@ def test_brute_force_to_cell_list_switch(pfc, weights):
         p.close()
 
 
+def test_skin_list_reuse_keeps_the_lists_bit_exact(pfc, weights):
+    """pfc_tuning_t.skin_list = 1: cell-list systems keep candidate rows (cutoff 5.2 + 0.5 A) and rebuild them only
+    when an atom has moved more than 0.25 A since the build; every step the exact predicate runs on the candidates.  The lists must be
+    the O(N^2) definition's, bit for bit, at the positions the GPU has reached -- after a stretch of steps that
+    reused the candidates, after the export (which invalidates them) and after a jump of all positions."""
+    wl = W.config3(n_atoms=5000)
+    p = pfc.Pfc(wl.species, wl.sys_offsets, weights, tuning=pfc.Tuning(skin_list=1))
+    pos, vel = _dev(pfc, wl.pos), _dev(pfc, wl.vel)
+    p.set_state(pos, vel)
+    p.step(40, wl.dt_fs)
+    torch.cuda.synchronize()
+    builds = p.work_counts()["skin_builds"]
+    assert 1 <= builds <= 12, builds                            # 41 evaluations, a handful of builds
+    _assert_lists_equal(p.neighbors(), oracle.neighbors(pos.cpu().numpy()[:, :3], wl.sys_offsets, cell=False))
+    p.step(25, wl.dt_fs)
+    torch.cuda.synchronize()
+    _assert_lists_equal(p.neighbors(), oracle.neighbors(pos.cpu().numpy()[:, :3], wl.sys_offsets, cell=False))
+    # a jump: every atom displaced by up to 0.6 A -> the check must trigger a rebuild
+    rng = np.random.default_rng(5)
+    moved = (pos.cpu().numpy()[:, :3] + rng.uniform(-0.35, 0.35, size=(wl.n_atoms, 3))).astype(np.float32)
+    before = p.work_counts()["skin_builds"]
+    p.energy_forces(_dev(pfc, moved))
+    torch.cuda.synchronize()
+    assert p.work_counts()["skin_builds"] == before + 1
+    _assert_lists_equal(p.neighbors(), oracle.neighbors(moved, wl.sys_offsets, cell=False))
+    assert p.status() == 0
+    p.close()
+
+
 def test_mixed_batch_of_cell_and_brute_systems(pfc, weights):
     """One handle holding a 2,500-atom cluster (cell list), small molecules and a 1-atom system."""
     big = W.config3(n_atoms=2500)
