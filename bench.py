@@ -454,7 +454,7 @@ def main():
     ap.add_argument("--integrator", default="verlet", choices=["verlet", "langevin"],
                     help="langevin = the paper's timing protocol (friction 0.1 ps^-1, 10 frames), PAPER.md:94")
     ap.add_argument("--mlp", type=int, default=3, choices=[0, 1, 3],
-                    help="3 = auto (library default: tensor-core MLP from 4096 atoms on), 0 = FP32 FFMA, 1 = tcgen05 fp16 split")
+                    help="3 = auto (library default: tensor-core MLP from 1024 atoms on), 0 = FP32 FFMA, 1 = tcgen05 fp16 split")
     ap.add_argument("--all-configs", action="store_true", help="also time the other four configs (100 steps each)")
     ap.add_argument("--skin", action="store_true",
                     help="cell-list systems (config 3): neighbour candidates with a 0.5 A skin, reused between rebuilds "

@@ -75,7 +75,7 @@ extern "C" {
 #define PFC_MLP_FP32 0                  /* FP32 FFMA grouped MLP                 */
 #define PFC_MLP_TENSOR 1                /* tcgen05 kind::f16, fp16 hi|lo 3-term split, fp32 accumulate */
 #define PFC_MLP_TENSOR_1TERM 2          /* tcgen05 plain fp16 operands: tolerance evidence only (fails it) */
-#define PFC_MLP_AUTO 3                  /* TENSOR for batches of >= 4096 atoms if its calibration check passes, FP32 otherwise */
+#define PFC_MLP_AUTO 3                  /* TENSOR for batches of >= 1024 atoms if its calibration check passes, FP32 otherwise */
 
 /* Optional tuning knobs, passed explicitly through pfc_desc_t.tuning (HOST pointer, NULL = all
  * defaults; a zero-filled struct is also "all defaults").  The library reads no environment

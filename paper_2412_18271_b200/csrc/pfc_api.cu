@@ -157,7 +157,15 @@ constexpr float TC_LAMBDA_FWD = 0.85f, TC_LAMBDA_BWD = 0.85f;   // uncalibrated 
 constexpr int CALIB_MIN_ROWS = 256;           // atoms of an element below which its lambdas stay at the defaults
 // a calibrated element keeps the tensor path only if, against the FP32 MLP on the same batch, the least-squares
 // slopes of its e_i and g errors and its largest errors (relative to the rms of e_i / g) stay below these
-constexpr double CALIB_MAX_SLOPE = 3e-7, CALIB_MAX_DE = 1e-4, CALIB_MAX_DG = 5e-5;
+// (the slope of e_i is a weak statistic when the e_i of an element are nearly equal -- 500 O atoms of a water
+// cluster: it then measures an offset of 1e-7 eV, not a scale -- so its bound sits 5x inside the 1e-5 energy bar
+// instead of at the level of the g slope, which is what a trajectory feels)
+constexpr double CALIB_MAX_SLOPE_E = 2e-6, CALIB_MAX_SLOPE_G = 3e-7, CALIB_MAX_DE = 1e-4, CALIB_MAX_DG = 5e-5;
+// PFC_MLP_AUTO: the tensor-core MLP from this many atoms on.  Its cost is one tile chain (33 us) until the
+// batch has more tiles than SMs; measured ms/step, FP32 / tensor (round 2): 1,100 atoms 0.062 / 0.049, 2,200 atoms
+// 0.091 / 0.051, config 2 (1,500) 0.081 / 0.069, config 1 (5,632) 0.139 / 0.061.  Below, the FP32 kernels (the
+// cluster kernel up to 18 16-row tiles, 15 us)
+constexpr int TC_AUTO_MIN_ATOMS = 1024;
 constexpr int ROW_CAP = 192;                  // neighbour-row capacity of an atom: min(ROW_CAP, N_sys - 1); bulk at 0.1 / A^3 has 59
 constexpr int K1_MIN_BLOCK = 8, K1_MAX_BLOCK = 64;   // atoms per K1 brute-force work item
 
@@ -487,7 +495,7 @@ int calibrate_tc(pfc_ctx* c, const float4* pos, bool with_xlo, cudaStream_t st) 
     c->tc_resid[e][1] = (float)slope(fin[e].sdg, fin[e].sgg);
     c->tc_resid[e][2] = (float)(rms_e > 0.0 ? fin[e].mde / rms_e : 0.0);
     c->tc_resid[e][3] = (float)(rms_g > 0.0 ? fin[e].mdg / rms_g : 0.0);
-    if (!(fabs(c->tc_resid[e][0]) <= CALIB_MAX_SLOPE) || !(fabs(c->tc_resid[e][1]) <= CALIB_MAX_SLOPE) ||
+    if (!(fabs(c->tc_resid[e][0]) <= CALIB_MAX_SLOPE_E) || !(fabs(c->tc_resid[e][1]) <= CALIB_MAX_SLOPE_G) ||
         !(c->tc_resid[e][2] <= CALIB_MAX_DE) || !(c->tc_resid[e][3] <= CALIB_MAX_DG))
       ok = false;
   }
@@ -589,12 +597,8 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); delete c; return PFC_ERR_CUDA; }
   if (tun.steps_per_graph > 0) c->steps_per_graph = tun.steps_per_graph;
   c->skin_list = tun.skin_list == 1;
-  // AUTO: the tensor-core MLP pays from about 4,000 atoms on, where its 128-row tiles start to fill the
-  // SMs.  Measured ms/step, FFMA vs tensor, replicas of config 1: 2,200 atoms 0.108 / 0.111, 3,960
-  // 0.113 / 0.115, 4,840 0.136 / 0.121, 5,632 0.139 / 0.124; of config 4: 3,758 atoms 0.143 / 0.145,
-  // 4,749 0.163 / 0.147; config 2 (1,500 atoms) 0.111 / 0.141
   c->mlp_requested = d->mlp_path;
-  c->mlp_path = d->mlp_path == PFC_MLP_AUTO ? (d->n_atoms >= 4096 ? PFC_MLP_TENSOR : PFC_MLP_FP32) : d->mlp_path;
+  c->mlp_path = d->mlp_path == PFC_MLP_AUTO ? (d->n_atoms >= TC_AUTO_MIN_ATOMS ? PFC_MLP_TENSOR : PFC_MLP_FP32) : d->mlp_path;
   for (int e = 0; e < NSPEC; ++e) c->count[e] = count[e];
   c->sz = worst_case_sizes(N, NS);                      // capacities are the worst-case ones
   // static element grouping: rows sorted by element, blocks padded to ROW_PAD

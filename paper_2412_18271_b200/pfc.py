@@ -23,7 +23,7 @@ N_WEIGHTS = 378756
 MLP_FP32 = 0
 MLP_TENSOR = 1
 MLP_TENSOR_1TERM = 2      # plain fp16 operands: tolerance evidence only
-MLP_AUTO = 3              # MLP_TENSOR from 4096 atoms on, FP32 below
+MLP_AUTO = 3              # MLP_TENSOR from 1024 atoms on, FP32 below
 
 STATUS_BITS = {1: "radial capacity overflow", 2: "angular capacity overflow",
                4: "angular row longer than PFC_MAX_ANGULAR", 8: "non-finite energy",

@@ -84,14 +84,14 @@ def _check_energy_forces(E, F, ref, tight=True):
 
 
 # ---- step 0 on every config at full size: lists, E, F --------------------------------
-# (the default MLP path is PFC_MLP_AUTO: the compensated tensor-core MLP on configs 1, 3, 4, FP32 FFMA on
-# configs 0 and 2; "fp32" pins the FFMA path on the large configs as well)
+# (the default MLP path is PFC_MLP_AUTO: the calibrated tensor-core MLP from 1,024 atoms on -- configs 1 to 4 --,
+# the FP32 cluster kernel on config 0; "fp32" pins the FP32 kernels on the larger configs as well)
 @pytest.mark.parametrize("k,path", [(0, "auto"), (1, "auto"), (2, "auto"), (3, "auto"), (4, "auto"),
-                                    (1, "fp32"), (3, "fp32"), (4, "fp32")])
+                                    (1, "fp32"), (2, "fp32"), (3, "fp32"), (4, "fp32")])
 def test_step0_lists_energy_forces_full_size(pfc, weights, k, path):
     wl = cfg(k)
     p = pfc.Pfc(wl.species, wl.sys_offsets, weights, mlp_path=pfc.MLP_AUTO if path == "auto" else pfc.MLP_FP32)
-    assert p.mlp_path() == (pfc.MLP_TENSOR if (path == "auto" and wl.n_atoms >= 4096) else pfc.MLP_FP32)
+    assert p.mlp_path() == (pfc.MLP_TENSOR if (path == "auto" and wl.n_atoms >= 1024) else pfc.MLP_FP32)
     E, F = p.energy_forces(_dev(pfc, wl.pos))
     assert p.status() == 0
     # the definition is the O(N^2) enumeration; config 3 (20,000 atoms) goes through the
@@ -191,9 +191,10 @@ def test_trajectory_config3_full_size(pfc, weights):
     _trajectory(pfc, weights, cfg(3), 100, cell=True)
 
 
-def test_trajectory_fp32_path_configs_1_and_3(pfc, weights):
-    """The FFMA path on the two configs whose default is the tensor-core MLP."""
+def test_trajectory_fp32_path_configs_1_2_3(pfc, weights):
+    """The FP32 MLP on the configs whose default is the tensor-core MLP (config 4: the all-replica test)."""
     _trajectory(pfc, weights, cfg(1), 100, mlp_path=pfc.MLP_FP32, cond=1)
+    _trajectory(pfc, weights, cfg(2), 100, mlp_path=pfc.MLP_FP32)
     _trajectory(pfc, weights, cfg(3), 100, cell=True, mlp_path=pfc.MLP_FP32)
 
 
