@@ -232,6 +232,10 @@ struct pfc_ctx {
   float4 *pos = nullptr, *vel = nullptr, *frc = nullptr;
   float* E = nullptr;
   cudaStream_t stream = nullptr, cap_stream = nullptr;
+  // pfc_run_host*: the new positions go back to the host on a side stream while the forces are evaluated
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_drift = nullptr, ev_copied = nullptr;
+  float4* early_pos_dst = nullptr;   // HOST destination of that copy for the step being enqueued, or NULL
   bool bound = false, forces_stale = true;
   float cur_dt = -1.0f;
   // graphs of the bound state: forces; one Verlet / Langevin step; steps_per_graph of them
@@ -1071,6 +1075,13 @@ static int run_steps(pfc_ctx* c, int32_t n_steps, float dt_fs, bool langevin) {
   // launch.  Then the last half kick and the per-system energies of the final state (the step graphs
   // leave the energy sum out: E cannot be read between the steps of one call).
   if (langevin) enqueue_langevin<1>(c, st); else enqueue_verlet<1>(c, st);
+  if (n_steps == 1 && c->early_pos_dst) {            // x_1 is final: its copy to the host overlaps the force evaluation
+    if (cudaEventRecord(c->ev_drift, st) != cudaSuccess || cudaStreamWaitEvent(c->copy_stream, c->ev_drift, 0) != cudaSuccess ||
+        cudaMemcpyAsync(c->early_pos_dst, c->pos, sizeof(float4) * (size_t)c->sz.n_atoms, cudaMemcpyDeviceToHost,
+                        c->copy_stream) != cudaSuccess ||
+        cudaEventRecord(c->ev_copied, c->copy_stream) != cudaSuccess)
+      return PFC_ERR_CUDA;
+  }
   if (cudaGraphLaunch(c->g_forces, st) != cudaSuccess) return PFC_ERR_CUDA;
   if ((rc = maybe_store_frame(c, st)) != PFC_OK) return rc;
   int left = n_steps - 1;
@@ -1140,8 +1151,21 @@ static int run_host_impl(pfc_t* c, float* pos_h, float* vel_h, int32_t n_steps, 
   int rc = pfc_set_state(c, (float*)b.h_pos, (float*)b.h_vel, b.h_E, (float*)b.h_frc, stream);
   if (rc != PFC_OK) return rc;
   if (forces_in) c->forces_stale = false;          // the caller vouches: F_h = forces at pos_h
-  if ((rc = pfc_step(c, n_steps, dt_fs)) != PFC_OK) return rc;
-  if (cudaMemcpyAsync(pos_h, b.h_pos, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
+  // one step with known forces: the new positions are final after the first kernel -- copy them back meanwhile
+  const bool early = forces_in && n_steps == 1;
+  if (early && !c->copy_stream) {
+    if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_drift, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming) != cudaSuccess)
+      return PFC_ERR_CUDA;
+  }
+  c->early_pos_dst = early ? (float4*)pos_h : nullptr;
+  rc = pfc_step(c, n_steps, dt_fs);
+  c->early_pos_dst = nullptr;
+  if (rc != PFC_OK) return rc;
+  if (early) {
+    if (cudaStreamWaitEvent(st, c->ev_copied, 0) != cudaSuccess) return PFC_ERR_CUDA;
+  } else if (cudaMemcpyAsync(pos_h, b.h_pos, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpyAsync(vel_h, b.h_vel, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
   if (F_h && cudaMemcpyAsync(F_h, b.h_frc, nb, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PFC_ERR_CUDA;
   if (cudaMemcpyAsync(E_h, b.h_E, sizeof(float) * c->sz.n_systems, cudaMemcpyDeviceToHost, st) != cudaSuccess)
@@ -1256,6 +1280,9 @@ int pfc_destroy(pfc_t* c) {
   for (EfGraph& g : c->ef)
     if (g.exec) cudaGraphExecDestroy(g.exec);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->ev_drift) cudaEventDestroy(c->ev_drift);
+  if (c->ev_copied) cudaEventDestroy(c->ev_copied);
   delete c;
   return PFC_OK;
 }
