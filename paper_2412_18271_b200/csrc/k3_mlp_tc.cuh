@@ -21,12 +21,11 @@
 //              SWIZZLE_64B) from the previous accumulator in TMEM (bias, CELU, CELU', Hadamard), and
 //              drain g;
 //   warp 8     TMA: streams the pre-packed, pre-swizzled weight chunks (hi | lo) of the schedule
-//              from L2 into a 4-slot ring with cp.async.bulk + mbarrier -- and the A operand of
-//              phase 0, which K2 writes in exactly the chunk image the tensor core reads (AEV times 8,
-//              fp16 hi | lo, SWIZZLE_64B; one contiguous 16 KB block per tile and chunk), into ring A;
+//              from L2 into a 4-slot ring with cp.async.bulk + mbarrier;
 //   warp 9     walks the MMA schedule; one elected lane issues tcgen05.mma and commits to the ring / phase barriers;
-//   warp 10    TMA: the first GEMM's A operand chunks into ring A (its own thread: no head-of-line blocking behind
-//              the weight stream).
+//   warp 10    TMA: the A operand of phase 0, which K2 writes in exactly the chunk image the tensor core reads
+//              (AEV times 8, fp16 hi | lo, SWIZZLE_64B; one contiguous 16 KB block per tile and chunk), into the
+//              3-slot ring A (its own thread: no head-of-line blocking behind the weight stream).
 // Schedule.  The eight phases of a tile are a serial chain (each needs the previous
 // accumulator), except at its two ends: the first GEMM (AEV x W1) depends only on global
 // memory and the three g passes (delta1 x W1^T) only on delta1.  So consecutive tiles are
