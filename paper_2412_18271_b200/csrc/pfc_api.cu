@@ -10,11 +10,13 @@
 
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 #include <new>
 #include <vector>
 
 #include "../../include/pfc.h"
 #include "../../include/pfc_debug.h"
+#include "../../include/pfc_noalloc.h"
 #include "k0_units.cuh"
 #include "k1_neighbors.cuh"
 #include "k2_aev.cuh"
@@ -1205,6 +1207,47 @@ int pfc_get_neighbors(pfc_t* c, const int32_t** r_off, const int32_t** r_idx, co
   return PFC_OK;
 }
 
+// ---- the entry point with static scratch (include/pfc_noalloc.h) ----------------------------------
+// Block totals of the reduce-then-scan over cnt: one int2 per SCAN_BLOCK atoms.  A file-scope device
+// array: resident on every GPU that loads the library; shared by all calls (they race if they overlap).
+constexpr int NOALLOC_MAX_BLOCKS = PFC_NOALLOC_MAX_ATOMS / SCAN_BLOCK;
+static_assert(NOALLOC_MAX_BLOCKS * SCAN_BLOCK == PFC_NOALLOC_MAX_ATOMS && NOALLOC_MAX_BLOCKS == 512, "static scratch size");
+static __device__ __align__(256) int2 g_noalloc_block_tot[NOALLOC_MAX_BLOCKS];
+
+// In host code the array's name is a stand-in, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static int2* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+static std::mutex g_noalloc_mutex;
+
+static int noalloc_scratch(int device, int2** out) {
+  if (device < 0 || device >= NOALLOC_MAX_DEVICES) return PFC_ERR_STATE;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[device]) {
+    int2* p = nullptr;
+    if (cudaGetSymbolAddress((void**)&p, g_noalloc_block_tot) != cudaSuccess || !p) { cudaGetLastError(); return PFC_ERR_CUDA; }
+    g_noalloc_ptr[device] = p;
+  }
+  *out = g_noalloc_ptr[device];
+  return PFC_OK;
+}
+
+int pfc_neighbor_offsets_noalloc(pfc_t* c, int32_t* r_off, int32_t* a_off, void* stream) {
+  if (!c || !r_off || !a_off) return PFC_ERR_ARG;
+  if (!on_device(c)) return PFC_ERR_STATE;            // (so the symbol address below belongs to the handle's device)
+  if (c->sz.n_atoms > PFC_NOALLOC_MAX_ATOMS) return PFC_ERR_TOO_LARGE;
+  int2* tot = nullptr;
+  const int rc = noalloc_scratch(c->device, &tot);
+  if (rc != PFC_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int n = c->sz.n_atoms, nb = cdiv(n, SCAN_BLOCK);
+  // the same two kernels as the export of pfc_get_neighbors, their block totals in the static array
+  // (block q's total is written by the first kernel before the second reads totals 0 .. q-1)
+  if (nb > 1) k1_scan_totals_kernel<<<nb, SCAN_THREADS, 0, st>>>(n, c->b.cnt, tot);
+  k1_scan_kernel<<<nb, SCAN_THREADS, 0, st>>>(n, c->b.cnt, tot, r_off, a_off);
+  return cudaGetLastError() == cudaSuccess ? PFC_OK : PFC_ERR_CUDA;
+}
+
 int pfc_get_intermediates(pfc_t* c, const float** aev, const float** g, const int32_t** row_of_atom,
                           int32_t* n_rows) {
   if (!c) return PFC_ERR_ARG;
@@ -1296,6 +1339,7 @@ const char* pfc_error_string(int code) {
     case PFC_ERR_CUDA: return "CUDA runtime error";
     case PFC_ERR_CAPTURE: return "CUDA graph capture failed";
     case PFC_ERR_STATE: return "no MD state bound (pfc_set_state), or the handle's CUDA device is not current";
+    case PFC_ERR_TOO_LARGE: return "the handle has more atoms than the static scratch of the no-allocation entry point holds (PFC_NOALLOC_MAX_ATOMS)";
     default: return "unknown pfc error";
   }
 }

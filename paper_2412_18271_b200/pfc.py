@@ -40,6 +40,11 @@ EXPORTS = ("pfc_workspace_bytes", "pfc_create", "pfc_energy_forces", "pfc_energy
 DEBUG_EXPORTS = ("pfc_profile_stages", "pfc_work_counts", "pfc_k3_timeline", "pfc_copy_to_host", "pfc_mlp_path", "pfc_launch_counts", "pfc_tc_calibration", "pfc_tc_chain_probe")
 
 
+NOALLOC_EXPORTS = ("pfc_neighbor_offsets_noalloc",)        # include/pfc_noalloc.h
+NOALLOC_MAX_ATOMS = 1048576
+ERR_TOO_LARGE = -7
+
+
 class PfcError(RuntimeError):
     pass
 
@@ -97,6 +102,8 @@ def load_library() -> ctypes.CDLL:
     lib.pfc_tc_chain_probe.argtypes = [c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
     lib.pfc_launch_counts.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32)]
     lib.pfc_destroy.argtypes = [c_void_p]
+    lib.pfc_neighbor_offsets_noalloc.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p]
+    lib.pfc_neighbor_offsets_noalloc.restype = c_int
     lib.pfc_error_string.argtypes = [c_int]
     lib.pfc_error_string.restype = c_char_p
     for name in EXPORTS + DEBUG_EXPORTS:
@@ -344,6 +351,23 @@ class Pfc:
         r_idx = self._copy(p[1], int(r_off[-1]), np.int32)
         a_idx = self._copy(p[3], int(a_off[-1]), np.int32)
         return r_off, r_idx, a_off, a_idx
+
+    @_on_device
+    def neighbor_offsets_noalloc(self, r_off=None, a_off=None, stream=None):
+        """pfc_neighbor_offsets_noalloc (include/pfc_noalloc.h): r_off / a_off of the last evaluation into
+        caller-owned cuda int32 tensors [n_atoms + 1] (made here if not given); the library's scratch for it is a
+        static device array.  Enqueues only."""
+        import torch
+        if r_off is None:
+            r_off = torch.empty(self.n_atoms + 1, dtype=torch.int32, device=self.device)
+        if a_off is None:
+            a_off = torch.empty(self.n_atoms + 1, dtype=torch.int32, device=self.device)
+        for t in (r_off, a_off):
+            if not (t.is_cuda and t.dtype == torch.int32 and t.numel() == self.n_atoms + 1 and t.is_contiguous()):
+                raise PfcError("expected contiguous cuda int32 tensors of n_atoms + 1 elements")
+        _check(self._lib.pfc_neighbor_offsets_noalloc(self._h, r_off.data_ptr(), a_off.data_ptr(), _stream_ptr(stream)),
+               "pfc_neighbor_offsets_noalloc")
+        return r_off, a_off
 
     @_on_device
     def intermediates(self):

@@ -18,12 +18,14 @@ def test_library_exports_every_declared_symbol():
     from paper_2412_18271_b200 import build, pfc
     build.build_libpfc()
     lib = ctypes.CDLL(pfc.LIB_PATH)
-    names, debug = _declared("pfc.h"), _declared("pfc_debug.h")
+    names, debug, noalloc = _declared("pfc.h"), _declared("pfc_debug.h"), _declared("pfc_noalloc.h")
     assert {"pfc_create", "pfc_energy_forces", "pfc_step", "pfc_destroy"} <= names      # the north_star four
-    missing = [n for n in sorted(names | debug) if not hasattr(lib, n)]
+    missing = [n for n in sorted(names | debug | noalloc) if not hasattr(lib, n)]
     assert not missing, missing
     assert set(pfc.EXPORTS) == names
     assert set(pfc.DEBUG_EXPORTS) == debug
+    assert set(pfc.NOALLOC_EXPORTS) == noalloc
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["pfc.h", "pfc_debug.h", "pfc_noalloc.h"]
     assert len(names) <= 16                                    # "keep them few"
 
 
