@@ -38,11 +38,11 @@ constexpr int SCAN_THREADS = 256, SCAN_ITEMS = 8, SCAN_BLOCK = SCAN_THREADS * SC
 // Also writes the packed copies every later kernel reads: xs[i] = {x, y, z, bitcast(species)} and
 // xsl[i], the low words of the two-float positions (S15): the list predicate sees only the fp32
 // positions, the AEV geometry sees the two-float difference.
-__global__ void __launch_bounds__(K1_WARPS * 32)
+__global__ void __launch_bounds__(K1_WARPS * 32, 6)
 k1_brute_kernel(const int4* __restrict__ items, const float4* __restrict__ pos, const int* __restrict__ species,
                 const float4* __restrict__ xlo, float4* __restrict__ xs, float4* __restrict__ xsl,
                 const int* __restrict__ row_beg, uint32_t* __restrict__ nbr, int2* __restrict__ cnt,
-                uint32_t* __restrict__ status) {
+                const int4* __restrict__ rank_info, int2* __restrict__ rank_tab, uint32_t* __restrict__ status) {
   extern __shared__ float4 k1_sp[];              // the system's positions, species bits in .w
   const int4 it = items[blockIdx.x];
   const int nsys = it.y - it.x;
@@ -61,6 +61,11 @@ k1_brute_kernel(const int4* __restrict__ items, const float4* __restrict__ pos, 
       xsl[i] = xlo ? xlo[i] : make_float4(0.f, 0.f, 0.f, 0.f);
     }
     const int beg = row_beg[i], cap = row_beg[i + 1] - beg;
+    // rank table (read by K4a): per 32-candidate chunk of my scan the ballot and the entries before it, so that
+    // "the position of atom k in row i" is  n_before + popc(ballot & bits below k)  -- one 8-byte load
+    // Every lane keeps the word of "its" chunk (chunk index mod 32) in registers; one coalesced store per 32 chunks.
+    int2* rtab = rank_tab + rank_info[i].x;
+    int2 my_word = make_int2(0, 0);
     int nr = 0, na = 0;
     for (int j0 = 0; j0 < nsys; j0 += 32) {
       const int jl = j0 + (int)lane;
@@ -72,6 +77,8 @@ k1_brute_kernel(const int4* __restrict__ items, const float4* __restrict__ pos, 
         sp = __float_as_int(pj.w);
       }
       const uint32_t mr = __ballot_sync(0xffffffffu, d2 < RC2_R);
+      if ((uint32_t)(j0 >> 5 & 31) == lane) my_word = make_int2((int)mr, nr);
+      if ((j0 >> 5 & 31) == 31) rtab[(j0 >> 5 & ~31) + (int)lane] = my_word;   // warp-uniform: 32 words are full (systems > 992 atoms)
       if (mr == 0u) continue;                    // warp-uniform
       const int slot = nr + __popc(mr & lt);
       const bool stored = d2 < RC2_R && slot < cap;     // capacity overflow is flagged below; never write out of the row
@@ -79,6 +86,10 @@ k1_brute_kernel(const int4* __restrict__ items, const float4* __restrict__ pos, 
       if (stored) nbr[beg + slot] = (uint32_t)(it.x + jl) | ((uint32_t)sp << 29) | (ang ? 0x80000000u : 0u);
       na += __popc(__ballot_sync(0xffffffffu, stored && ang));
       nr += __popc(mr);
+    }
+    {                                            // the last (partial) group of rank words
+      const int n_words = (nsys + 31) >> 5, w = (n_words & ~31) + (int)lane;
+      if (w < n_words) rtab[w] = my_word;
     }
     if (lane == 0) {
       if (nr > cap) atomicOr(status, ST_RADIAL_OVERFLOW);

@@ -2,9 +2,14 @@
 // fixed-order accumulation (O7; "forces by backprop").
 //
 // K4a (centre-owned, one warp per atom i): recomputes the pair/triple geometry
-// and writes, for every entry e = (i -> j) of atom i's neighbour row,
-//      edge[e] = P_e = sum_a g_i[a] * dAEV_i[a]/dx_j        (gradient, not force)
+// and computes, for every entry e = (i -> j) of atom i's neighbour row,
+//      P_e = sum_a g_i[a] * dAEV_i[a]/dx_j        (gradient, not force)
 // plus self[i] = sum_e P_e.  By translation invariance dE_i/dx_i = -self[i].
+// Brute-force systems: P_e is written where atom j will read it, edge[rev(e)], rev(i -> j) = the position of i in
+// row j (rows are symmetric and sorted), found with ONE load from K1's rank table (ballot + running count per
+// 32-candidate chunk of j's scan; row and table of j follow from my own by arithmetic, a system's atoms share
+// capacity and stride); K4b then reads its row contiguously.  Cell-list systems have no such table: P_e stays in
+// my own slot edge[e] and K4b finds rev(e) by binary search in row j.
 //   radial : lane <-> entry, 16 shells.
 //   angular: the m(m-1)/2 triples of the m angular neighbours (table in row order) are
 //            enumerated in round-robin (circulant) order: slot q = (d-1) m + a is the pair
@@ -16,10 +21,10 @@
 //            phase 2, lane <-> angular neighbour n: for every round d of the chunk it meets
 //            its partners (n+d) mod m and (n-d) mod m in that fixed order:
 //               grad_n = (sum_k C u_k - (sum_k C cos(phi)) u_n)/r_n + (sum_k R) u_n.
-// K4b (gather, one warp per atom a):
-//      F_a = self[a] - sum_{e in row(a), ascending} edge[rev(e)]
-// where rev(a->j) is the position of a in row j (binary search; rows are
-// symmetric and sorted).  No float atomics anywhere.
+// K4b (one warp per atom a):
+//      F_a = self[a] - sum_{k < cnt(a), ascending} P_(j_k -> a),   j_k = k-th neighbour of a,
+// read from slot k of a's own row (brute-force systems) or from edge[rev(a -> j_k)] (cell-list systems).
+// Every slot has exactly one writer and the summation order is fixed.  No float atomics anywhere.
 #pragma once
 #include "aev_common.cuh"
 
@@ -44,7 +49,8 @@ struct AevBwdSmem {
 __global__ void __launch_bounds__(AEV_WARPS * 32, PFC_K4A_MINB)
 k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __restrict__ xsl,
                    const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr, const int2* __restrict__ cnt,
-                   const int* __restrict__ row_of_atom,
+                   const int* __restrict__ row_of_atom, const int4* __restrict__ rank_info,
+                   const int2* __restrict__ rank_tab,
                    const float* __restrict__ g, float4* __restrict__ edge, float4* __restrict__ self) {
   __shared__ __align__(16) AevBwdSmem sm[AEV_WARPS];
   const int warp = threadIdx.x >> 5;
@@ -69,16 +75,31 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
   const float4 xi = xs[i], li = xsl[i];
   const int rb = row_beg[i];
   const int re = rb + cnt[i].x;
+  // Atoms of one brute-force system share the row capacity and the rank-table stride, so neighbour j's row and
+  // table follow from my own by arithmetic: the lookup is ONE load.  Cell-list systems (no table): tab_i < 0.
+  const int4 ri = rank_info[i];                  // {my first table word or -1, first atom of my system, words per atom, -}
+  const int rel_i = i - ri.y;                    // my index inside my system
+  const int tab_i = ri.x, words_i = ri.z;
+  const int cap_i = row_beg[i + 1] - rb;
   int m = 0;
   float sx = 0.f, sy = 0.f, sz = 0.f;            // this lane's share of self[i]
   for (int c0 = rb; c0 < re; c0 += 32) {
-    const int e = c0 + (int)lane;
+    int e = c0 + (int)lane;                      // my entry; from the lookup below on: the slot its gradient goes to
+    const bool live = e < re;
     NbrGeom ng;
     ng.ang = false; ng.sp = 0; ng.r = 1.0f; ng.ux = ng.uy = ng.uz = 0.0f;
     float px = 0.f, py = 0.f, pz = 0.f;
     float fc = 0.f, dfc = 0.f;
-    if (e < re) {
-      ng = nbr_geometry(nbr[e], xi, li, xs, xsl);
+    if (live) {
+      const uint32_t w = nbr[e];
+      if (tab_i >= 0) {
+        // rev(e): where neighbour j keeps me in ITS row
+        const int dj = nbr_index(w) - i;
+        const int2 t = rank_tab[tab_i + dj * words_i + (rel_i >> 5)];
+        // (on a row-capacity overflow, flagged by K1, outputs are unspecified -- but the slot stays inside row j)
+        e = rb + dj * cap_i + min(t.y + __popc((uint32_t)t.x & ((1u << (rel_i & 31)) - 1u)), cap_i - 1);
+      }                                          // (cell-list system: the gradient stays in my own slot, K4b searches)
+      ng = nbr_geometry(w, xi, li, xs, xsl);
       float sn, cs;
       __sincosf((PI_F / RC_R) * ng.r, &sn, &cs);
       fc = 0.5f * cs + 0.5f; dfc = -(PI_F / (2.0f * RC_R)) * sn;
@@ -88,7 +109,7 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
       __syncwarp();
       g_pending = false;
     }
-    if (e < re) {
+    if (live) {
       // two shells at a time in packed fp32 pairs (the exponentials stay scalar SFU calls)
       const float2* gs = reinterpret_cast<const float2*>(S.gR + NSHF_R * ng.sp);
       const float2 r2 = make_float2(ng.r, ng.r), m1 = make_float2(-1.0f, -1.0f), fc2 = make_float2(fc, fc),
@@ -119,7 +140,7 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
         in_table = true;
       }
     }
-    if (e < re && !in_table) {                   // purely radial neighbour: final already
+    if (live && !in_table) {                     // purely radial neighbour: final already
       edge[e] = make_float4(px, py, pz, 0.f);
       sx += px; sy += py; sz += pz;
     }
@@ -237,7 +258,8 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
 constexpr int K4B_WARPS = 8;
 __global__ void __launch_bounds__(K4B_WARPS * 32)
 k4b_gather_kernel(int n_atoms, const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr,
-                  const int2* __restrict__ cnt, const float4* __restrict__ edge, const float4* __restrict__ self,
+                  const int2* __restrict__ cnt, const int4* __restrict__ rank_info,
+                  const float4* __restrict__ edge, const float4* __restrict__ self,
                   const int* __restrict__ row_of_atom, const float* __restrict__ e_row,
                   float4* __restrict__ frc) {
   const int a = blockIdx.x * K4B_WARPS + (threadIdx.x >> 5);
@@ -245,24 +267,29 @@ k4b_gather_kernel(int n_atoms, const int* __restrict__ row_beg, const uint32_t* 
   const uint32_t lane = lane_id();
   const int rb = row_beg[a];
   const int re = rb + cnt[a].x;
+  const bool own_row = rank_info[a].x >= 0;         // brute-force system: my neighbours wrote into my row
+  // (requested now, used at the end: they do not wait for the row)
+  const float4 s = self[a];
+  const float ea = e_row[row_of_atom[a]];
   float gx = 0.f, gy = 0.f, gz = 0.f;
   for (int e = rb + (int)lane; e < re; e += 32) {
-    const int j = nbr_index(nbr[e]);
-    // find a in row j (on a row-capacity overflow, flagged by K1, the entry may be missing: outputs
-    // are unspecified then, but the search stays inside row j)
-    int lo = row_beg[j], hi = lo + max(cnt[j].x, 1) - 1;
-    while (lo < hi) {
-      const int mid = (lo + hi) >> 1;
-      if (nbr_index(nbr[mid]) < a) lo = mid + 1; else hi = mid;
+    int slot = e;
+    if (!own_row) {
+      // find a in row j (on a row-capacity overflow, flagged by K1, the entry may be missing: outputs
+      // are unspecified then, but the search stays inside row j)
+      const int j = nbr_index(nbr[e]);
+      int lo = row_beg[j], hi = lo + max(cnt[j].x, 1) - 1;
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (nbr_index(nbr[mid]) < a) lo = mid + 1; else hi = mid;
+      }
+      slot = lo;
     }
-    const float4 p = edge[lo];
+    const float4 p = edge[slot];
     gx += p.x; gy += p.y; gz += p.z;
   }
   gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz);
-  if (lane == 0) {
-    const float4 s = self[a];
-    frc[a] = make_float4(s.x - gx, s.y - gy, s.z - gz, e_row[row_of_atom[a]]);
-  }
+  if (lane == 0) frc[a] = make_float4(s.x - gx, s.y - gy, s.z - gz, ea);
 }
 
 // per-system potential energy: one CTA per system, fixed-order tree, fp64 partials

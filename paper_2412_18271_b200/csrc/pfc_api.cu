@@ -56,6 +56,7 @@ struct Sizes {
   int n_atoms, n_systems, n_rows;
   int cap_r;                                  // neighbour-row entries (sum of the row capacities, worst case)
   int n_items;                                // K1 brute-force work items (worst case)
+  size_t rank_words;                          // rank-table words (worst case: every system BRUTE_MAX atoms)
   int n_scan_blocks;
   int n_cell_sys, n_cell_atoms, cell_slots;   // cell_slots: pooled cell arrays (incl. +1 per system)
 };
@@ -66,6 +67,8 @@ struct Buffers {
   int4* items;                  // K1 brute-force work items
   int* row_beg;                 // [N+1] first entry of every atom's fixed-capacity neighbour row
   uint32_t* nbr;                // [cap_r] entry words (k1_neighbors.cuh)
+  int4* rank_info;              // [N] {first word of the atom's rank table or -1 (cell-list system), first atom of its system, words per atom, 0}
+  int2* rank_tab;               // brute-force systems: per atom ceil(N_sys / 32) words {ballot, entries before} (K1 -> K4a)
   int2 *cnt, *block_tot;
   int *r_off, *a_off, *r_idx, *a_idx;   // CSR export (pfc_get_neighbors only); r_idx | a_idx are one block ...
   uint32_t* cand;               // ... which between exports holds the cell-list systems' candidate rows (skin list)
@@ -107,6 +110,8 @@ size_t carve(const Sizes& s, void* base, Buffers* b) {
   t.items = c.take<int4>((size_t)s.n_items);
   t.row_beg = c.take<int>(N + 1);
   t.nbr = c.take<uint32_t>((size_t)s.cap_r);
+  t.rank_info = c.take<int4>(N);
+  t.rank_tab = c.take<int2>(s.rank_words + 1);
   t.cnt = c.take<int2>(N);
   t.block_tot = c.take<int2>((size_t)s.n_scan_blocks);
   t.r_off = c.take<int>(N + 1);
@@ -180,6 +185,7 @@ Sizes worst_case_sizes(int n_atoms, int n_systems) {
   long long cr = (long long)n_atoms * (per_r > 1 ? per_r : 1);
   s.cap_r = (int)(cr > 2000000000LL ? 2000000000LL : cr);
   s.n_items = n_atoms / K1_MIN_BLOCK + n_systems + 1;
+  s.rank_words = (size_t)n_atoms * (size_t)(((n_atoms < BRUTE_MAX ? n_atoms : BRUTE_MAX) + 31) / 32);
   s.n_scan_blocks = (n_atoms + SCAN_BLOCK - 1) / SCAN_BLOCK;
   s.n_cell_sys = n_atoms / (BRUTE_MAX + 1) + 1;
   if (s.n_cell_sys > n_systems) s.n_cell_sys = n_systems;
@@ -274,7 +280,7 @@ void enqueue_k1(pfc_ctx* c, const float4* pos, bool with_xlo, cudaStream_t st) {
   const float4* xlo = with_xlo ? b.xlo : nullptr;
   if (c->n_items > 0)
     LAUNCH(c, k1_brute_kernel, c->n_items, K1_WARPS * 32, c->k1_smem, st, b.items, pos, b.species, xlo, b.xs, b.xsl,
-           b.row_beg, b.nbr, b.cnt, b.status);
+           b.row_beg, b.nbr, b.cnt, b.rank_info, b.rank_tab, b.status);
   if (c->n_cell_sys > 0) {
     const int nca = c->n_cell_atoms;
     // skin list on: has any atom moved more than SKIN/2 since the candidate rows were built?  If so the five
@@ -375,10 +381,10 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool wit
   else enqueue_k3_tc(c, st);
   mark(3);
   LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
-         b.row_of_atom, b.g, b.edge, b.self);
+         b.row_of_atom, b.rank_info, b.rank_tab, b.g, b.edge, b.self);
   mark(4);
-  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.row_beg, b.nbr, b.cnt, b.edge, b.self,
-         b.row_of_atom, b.e_row, F);
+  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.row_beg, b.nbr, b.cnt, b.rank_info, b.edge,
+         b.self, b.row_of_atom, b.e_row, F);
   mark(5);
   if (with_esum) enqueue_energy_sum(c, F, E, st);
   mark(6);
@@ -613,6 +619,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   for (int e = 0; e < NSPEC; ++e) row_start[e + 1] = row_start[e] + (count[e] + ROW_PAD - 1) / ROW_PAD * ROW_PAD;
   c->sz.n_rows = row_start[NSPEC];
   std::vector<int> row_of_atom(N), row_beg(N + 1);
+  std::vector<int4> rank_info(N);
   {
     int next[NSPEC];
     for (int e = 0; e < NSPEC; ++e) next[e] = row_start[e];
@@ -631,11 +638,15 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   int k1_block = (int)((n_brute / (4LL * 148) + 7) / 8 * 8);
   k1_block = k1_block < K1_MIN_BLOCK ? K1_MIN_BLOCK : k1_block > K1_MAX_BLOCK ? K1_MAX_BLOCK : k1_block;
   {
-    long long beg = 0;
+    long long beg = 0, rank_off = 0;
     for (int s = 0; s < NS; ++s) {
       const int b0 = d->sys_offsets[s], e0 = d->sys_offsets[s + 1], n = e0 - b0;
       const int cap = n - 1 < ROW_CAP ? (n - 1 > 1 ? n - 1 : 1) : ROW_CAP;
       for (int i = b0; i < e0; ++i) { row_beg[i] = (int)beg; beg += cap; }
+      for (int i = b0; i < e0; ++i) {                       // rank table: (n + 31) / 32 words per atom of a brute-force system
+        rank_info[i] = make_int4(n <= BRUTE_MAX ? (int)rank_off : -1, b0, n <= BRUTE_MAX ? (n + 31) / 32 : 0, 0);
+        if (n <= BRUTE_MAX) rank_off += (n + 31) / 32;
+      }
       if (n > BRUTE_MAX) {
         cell_slot_base.push_back((int)cell_atom_list.size());
         for (int i = b0; i < e0; ++i) { cell_atom_list.push_back(i); atom_cell_sys.push_back((int)cell_sys.size()); }
@@ -811,6 +822,7 @@ int pfc_create(const pfc_desc_t* d, pfc_t** out) {
   up(b.species, d->species, sizeof(int) * N);
   up(b.sp, &sp0, sizeof(sp0));
   up(b.row_beg, row_beg.data(), sizeof(int) * (N + 1));
+  up(b.rank_info, rank_info.data(), sizeof(int4) * N);
   up(b.items, items.data(), sizeof(int4) * items.size());
   up(b.sys_off, d->sys_offsets, sizeof(int) * (NS + 1));
   up(b.row_of_atom, row_of_atom.data(), sizeof(int) * N);
