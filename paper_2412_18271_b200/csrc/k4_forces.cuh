@@ -254,25 +254,33 @@ k4a_aev_bwd_kernel(int n_atoms, const float4* __restrict__ xs, const float4* __r
   if (lane == 0) self[i] = make_float4(sx, sy, sz, 0.f);
 }
 
-// K4b: gather.  frc[a] = {F_a, e_a}.
-constexpr int K4B_WARPS = 8;
+// K4b: gather.  frc[a] = {F_a, e_a}.  EIGHT lanes per atom, four atoms per warp: a row has 27 entries on
+// average and the kernel is a short chain of dependent loads per atom -- four atoms per warp put four times as
+// many chains in flight (64 -> 43 us on config 4 against one warp per atom).
+constexpr int K4B_WARPS = 8, K4B_LANES = 8, K4B_ATOMS = K4B_WARPS * 32 / K4B_LANES;
 __global__ void __launch_bounds__(K4B_WARPS * 32)
 k4b_gather_kernel(int n_atoms, const int* __restrict__ row_beg, const uint32_t* __restrict__ nbr,
                   const int2* __restrict__ cnt, const int4* __restrict__ rank_info,
                   const float4* __restrict__ edge, const float4* __restrict__ self,
                   const int* __restrict__ row_of_atom, const float* __restrict__ e_row,
                   float4* __restrict__ frc) {
-  const int a = blockIdx.x * K4B_WARPS + (threadIdx.x >> 5);
-  if (a >= n_atoms) return;
-  const uint32_t lane = lane_id();
-  const int rb = row_beg[a];
-  const int re = rb + cnt[a].x;
-  const bool own_row = rank_info[a].x >= 0;         // brute-force system: my neighbours wrote into my row
-  // (requested now, used at the end: they do not wait for the row)
-  const float4 s = self[a];
-  const float ea = e_row[row_of_atom[a]];
+  const int a = blockIdx.x * K4B_ATOMS + (int)(threadIdx.x / K4B_LANES);
+  const int sub = (int)(threadIdx.x % K4B_LANES);
+  const bool have = a < n_atoms;                    // (no early return: the shuffles below take the whole warp)
+  int rb = 0, re = 0;
+  bool own_row = true;
+  float4 s = make_float4(0.f, 0.f, 0.f, 0.f);
+  float ea = 0.f;
+  if (have) {
+    rb = row_beg[a];
+    re = rb + cnt[a].x;
+    own_row = rank_info[a].x >= 0;                  // brute-force system: my neighbours wrote into my row
+    // (requested now, used at the end: they do not wait for the row)
+    s = self[a];
+    ea = e_row[row_of_atom[a]];
+  }
   float gx = 0.f, gy = 0.f, gz = 0.f;
-  for (int e = rb + (int)lane; e < re; e += 32) {
+  for (int e = rb + sub; e < re; e += K4B_LANES) {
     int slot = e;
     if (!own_row) {
       // find a in row j (on a row-capacity overflow, flagged by K1, the entry may be missing: outputs
@@ -288,8 +296,13 @@ k4b_gather_kernel(int n_atoms, const int* __restrict__ row_beg, const uint32_t* 
     const float4 p = edge[slot];
     gx += p.x; gy += p.y; gz += p.z;
   }
-  gx = warp_sum(gx); gy = warp_sum(gy); gz = warp_sum(gz);
-  if (lane == 0) frc[a] = make_float4(s.x - gx, s.y - gy, s.z - gz, ea);
+#pragma unroll
+  for (int o = K4B_LANES / 2; o > 0; o >>= 1) {     // fixed xor tree inside the atom's eight lanes: deterministic
+    gx += __shfl_xor_sync(0xffffffffu, gx, o);
+    gy += __shfl_xor_sync(0xffffffffu, gy, o);
+    gz += __shfl_xor_sync(0xffffffffu, gz, o);
+  }
+  if (have && sub == 0) frc[a] = make_float4(s.x - gx, s.y - gy, s.z - gz, ea);
 }
 
 // per-system potential energy: one CTA per system, fixed-order tree, fp64 partials

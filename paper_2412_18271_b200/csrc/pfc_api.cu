@@ -383,7 +383,7 @@ void enqueue_forces(pfc_ctx* c, const float4* pos, float* E, float4* F, bool wit
   LAUNCH(c, k4a_aev_bwd_kernel, cdiv(N, AEV_WARPS), AEV_WARPS * 32, 0, st, N, b.xs, b.xsl, b.row_beg, b.nbr, b.cnt,
          b.row_of_atom, b.rank_info, b.rank_tab, b.g, b.edge, b.self);
   mark(4);
-  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_WARPS), K4B_WARPS * 32, 0, st, N, b.row_beg, b.nbr, b.cnt, b.rank_info, b.edge,
+  LAUNCH(c, k4b_gather_kernel, cdiv(N, K4B_ATOMS), K4B_WARPS * 32, 0, st, N, b.row_beg, b.nbr, b.cnt, b.rank_info, b.edge,
          b.self, b.row_of_atom, b.e_row, F);
   mark(5);
   if (with_esum) enqueue_energy_sum(c, F, E, st);
