@@ -16,14 +16,16 @@
 // N_TERMS = 1 is plain FP16 operands, kept only to produce the evidence that a single 16-bit
 // term misses the tolerance.
 //
-// One persistent CTA per SM, 352 threads, 128-row tiles of ONE element each:
-//   warps 0-7  workers: make the A operand of phases 1-7 in 32-wide K chunks (hi | lo, K-major,
+// One persistent CTA per SM, 608 threads, 128-row tiles of ONE element each:
+//   warps 0-15 workers (warp = TMEM lane quarter + 4 x column group; a thread makes 8 columns of a chunk: the
+//              epilogues are latency chains -- TMEM read, ex2, conversions -- and four warps per scheduler hide them
+//              better than two: K3 321 -> 312 us on config 4): make the A operand of phases 1-7 in 32-wide K chunks (hi | lo, K-major,
 //              SWIZZLE_64B) from the previous accumulator in TMEM (bias, CELU, CELU', Hadamard), and
 //              drain g;
-//   warp 8     TMA: streams the pre-packed, pre-swizzled weight chunks (hi | lo) of the schedule
+//   warp 16    TMA: streams the pre-packed, pre-swizzled weight chunks (hi | lo) of the schedule
 //              from L2 into a 4-slot ring with cp.async.bulk + mbarrier;
-//   warp 9     walks the MMA schedule; one elected lane issues tcgen05.mma and commits to the ring / phase barriers;
-//   warp 10    TMA: the A operand of phase 0, which K2 writes in exactly the chunk image the tensor core reads
+//   warp 17    walks the MMA schedule; one elected lane issues tcgen05.mma and commits to the ring / phase barriers;
+//   warp 18    TMA: the A operand of phase 0, which K2 writes in exactly the chunk image the tensor core reads
 //              (AEV times 8, fp16 hi | lo, SWIZZLE_64B; one contiguous 16 KB block per tile and chunk), into the
 //              3-slot ring A (its own thread: no head-of-line blocking behind the weight stream).
 // Schedule.  The eight phases of a tile are a serial chain (each needs the previous
@@ -50,8 +52,10 @@
 namespace pfc {
 
 constexpr int TC_TM = 128;                       // rows per tile == ROW_PAD
-constexpr int TC_THREADS = 352;
-constexpr int TC_WORKERS = 256;                  // warps 0-7
+constexpr int TC_CW = 8;                         // columns of a 32-wide chunk one worker thread makes (8 or 16)
+constexpr int TC_NWW = 4 * (32 / TC_CW);         // worker warps: 4 TMEM lane quarters x column groups
+constexpr int TC_WORKERS = 32 * TC_NWW;          // warps 0 .. TC_NWW-1
+constexpr int TC_THREADS = TC_WORKERS + 96;      // + weight TMA warp, MMA warp, A-operand TMA warp
 constexpr int TC_KC = 32;                        // k per chunk: one 64-byte SWIZZLE_64B row of fp16
 constexpr int TC_NA = 3, TC_NB = 4;              // ring depths: A operand chunks, weight chunks
 constexpr int TC_A_HALF = TC_TM * 64;            // 8,192 B: one part (hi or lo) of an A chunk
@@ -112,7 +116,6 @@ struct TcSmem {                                   // after the 1024-aligned oper
   uint64_t dd_full;                               // the four delta2 chunks are written to the resident region (256)
   uint64_t p5_done;                               // the delta1 producers have finished reading TMEM (256)
   uint32_t tmem_base;
-  float epart[2][TC_TM];
   float4 stage[4][32 * 8];                        // per drain warp: 32 rows x 32 columns of g, 16-byte units XOR-swizzled by row
 };
 constexpr size_t TC_SMEM_BYTES = 1024 + (size_t)TC_ND1 * TC_A_SLOT + (size_t)TC_NA * TC_A_SLOT +
@@ -209,24 +212,26 @@ __device__ __forceinline__ float2 celu_h2(float2 x, float2 d) {
   return pk_fma(make_float2(fmaxf(x.x, 0.0f), fmaxf(x.y, 0.0f)), make_float2(1.0f, 1.0f), t);
 }
 
-// 16 consecutive floats of a 64-byte aligned table (biases, w4) through the read-only path, four 16-byte loads
-__device__ __forceinline__ void tc_ld16(const float* p, float (&v)[16]) {
+// TC_CW consecutive floats of an aligned table (biases, w4) through the read-only path, 16-byte loads
+__device__ __forceinline__ void tc_ldw(const float* p, float (&v)[TC_CW]) {
 #pragma unroll
-  for (int j = 0; j < 4; ++j) {
+  for (int j = 0; j < TC_CW / 4; ++j) {
     const float4 t = __ldg(reinterpret_cast<const float4*>(p) + j);
     v[4 * j] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
   }
 }
-
-// store 16 consecutive K values (columns 16*hf .. 16*hf+15 of a 32-wide chunk) of row r as hi | lo
-__device__ __forceinline__ void tc_store_a16(uint8_t* slot, int r, int hf, const float (&v)[16]) {
-  uint32_t hi[8], lo[8];
+// my accumulator columns TMEM -> registers (8 or 16 per thread)
+__device__ __forceinline__ void tc_tmem_ldw(uint32_t taddr, float (&v)[16]) { tc::tmem_ld16(taddr, v); }
+__device__ __forceinline__ void tc_tmem_ldw(uint32_t taddr, float (&v)[8]) { tc::tmem_ld8(taddr, v); }
+// store TC_CW consecutive K values (columns TC_CW*hf .. of a 32-wide chunk) of row r as hi | lo
+__device__ __forceinline__ void tc_store_aw(uint8_t* slot, int r, int hf, const float (&v)[TC_CW]) {
+  uint32_t hi[TC_CW / 2], lo[TC_CW / 2];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) tc_split2(v[2 * j], v[2 * j + 1], hi[j], lo[j]);
+  for (int j = 0; j < TC_CW / 2; ++j) tc_split2(v[2 * j], v[2 * j + 1], hi[j], lo[j]);
   const uint32_t row = (uint32_t)(r >> 3) * 512u + (uint32_t)(r & 7) * 64u, sw = (uint32_t)(r >> 1) & 3u;
 #pragma unroll
-  for (int u = 0; u < 2; ++u) {
-    const uint32_t off = row + ((((uint32_t)(2 * hf + u)) ^ sw) << 4);
+  for (int u = 0; u < TC_CW / 8; ++u) {
+    const uint32_t off = row + ((((uint32_t)((TC_CW / 8) * hf + u)) ^ sw) << 4);
     *reinterpret_cast<uint4*>(slot + off) = make_uint4(hi[4 * u], hi[4 * u + 1], hi[4 * u + 2], hi[4 * u + 3]);
     *reinterpret_cast<uint4*>(slot + TC_A_HALF + off) = make_uint4(lo[4 * u], lo[4 * u + 1], lo[4 * u + 2], lo[4 * u + 3]);
   }
@@ -263,14 +268,14 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
     for (int i = 0; i < TC_NB; ++i) { tc::mbar_init(&S.b_full[i], 1); tc::mbar_init(&S.b_empty[i], 1); }
     for (int i = 0; i < 5; ++i) tc::mbar_init(&S.z_full[i], 1);
     tc::mbar_init(&S.g_full[0], 1); tc::mbar_init(&S.g_full[1], 1);
-    tc::mbar_init(&S.g_free, TC_WORKERS / 2);
+    tc::mbar_init(&S.g_free, 128);
     for (int i = 0; i < TC_ND1; ++i) tc::mbar_init(&S.d1_full[i], TC_WORKERS);
     tc::mbar_init(&S.d1_free, 1);
     tc::mbar_init(&S.dd_full, TC_WORKERS);
     tc::mbar_init(&S.p5_done, TC_WORKERS);
     tc::mbar_fence_init();
   }
-  if (warp == 9) tc::tmem_alloc<512>(&S.tmem_base);
+  if (warp == TC_NWW + 1) tc::tmem_alloc<512>(&S.tmem_base);
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
@@ -286,7 +291,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
     return el;
   };
 
-  if (warp < 8) {
+  if (warp < TC_NWW) {
     // =========================== workers ===========================
     const int q = warp & 3, hf = warp >> 2;
     const int r = 32 * q + lane;                               // tile row == TMEM lane
@@ -358,7 +363,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
           }
         }
       }
-      if (have_cur) ia += D0 / TC_KC;                          // the twelve first-GEMM chunks come by bulk copy (warp 10)
+      if (have_cur) ia += D0 / TC_KC;                          // the twelve first-GEMM chunks come by bulk copy (warp 18)
       if (!have_cur) break;
       // ------------------------------ chain of the current tile ------------------------------
       const int row0 = tile_of(it) * TC_TM;
@@ -376,19 +381,19 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       if (tid == 0) TC_TRACE(36);
 #pragma unroll 1
       for (int c = 0; c < D1 / TC_KC; ++c) {
-        float z[16], h[16];
-        tc::tmem_ld16(tlane + TC_COL_Z1 + 32 * c + 16 * hf, z);
+        float z[TC_CW], h[TC_CW];
+        tc_tmem_ldw(tlane + TC_COL_Z1 + 32 * c + TC_CW * hf, z);
         tc::tmem_ld_wait();
-        float bb[16];
-        tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
+        float bb[TC_CW];
+        tc_ldw(bias + TC_BIAS_B1 + 32 * c + TC_CW * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; k += 2) {
+        for (int k = 0; k < TC_CW; k += 2) {
           const float2 x = tc_affine2(z[k], z[k + 1], ks0, kb0, bb[k], bb[k + 1]);
           const float2 hh = celu_h2(x, celu_d2(x));
           h[k] = hh.x; h[k + 1] = hh.y;
         }
         uint8_t* slot = acquire();
-        tc_store_a16(slot, r, hf, h);
+        tc_store_aw(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
         ++ia;
       }
@@ -399,19 +404,19 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       if (tid == 0) TC_TRACE(38);
 #pragma unroll 1
       for (int c = 0; c < D2 / TC_KC; ++c) {
-        float z[16], h[16];
-        tc::tmem_ld16(tlane + TC_COL_Z2 + 32 * c + 16 * hf, z);
+        float z[TC_CW], h[TC_CW];
+        tc_tmem_ldw(tlane + TC_COL_Z2 + 32 * c + TC_CW * hf, z);
         tc::tmem_ld_wait();
-        float bb[16];
-        tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
+        float bb[TC_CW];
+        tc_ldw(bias + TC_BIAS_B2 + 32 * c + TC_CW * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; k += 2) {
+        for (int k = 0; k < TC_CW; k += 2) {
           const float2 x = tc_affine2(z[k], z[k + 1], ks1, kb1, bb[k], bb[k + 1]);
           const float2 hh = celu_h2(x, celu_d2(x));
           h[k] = hh.x; h[k + 1] = hh.y;
         }
         uint8_t* slot = acquire();
-        tc_store_a16(slot, r, hf, h);
+        tc_store_aw(slot, r, hf, h);
         publish(&S.a_full[ia % TC_NA]);
         ++ia;
       }
@@ -424,15 +429,15 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         float2 epart2 = make_float2(0.0f, 0.0f);            // even / odd columns, added at the end
 #pragma unroll 1
         for (int c = 0; c < D3 / TC_KC; ++c) {
-          float z[16], dl[16];
-          tc::tmem_ld16(tlane + TC_COL_Z3 + 32 * c + 16 * hf, z);
+          float z[TC_CW], dl[TC_CW];
+          tc_tmem_ldw(tlane + TC_COL_Z3 + 32 * c + TC_CW * hf, z);
           tc::tmem_ld_wait();
-          float bb[16], w4[16], w4s[16];
-          tc_ld16(bias + TC_BIAS_B3 + 32 * c + 16 * hf, bb);
-          tc_ld16(bias + TC_BIAS_W4 + 32 * c + 16 * hf, w4);
-          tc_ld16(bias + TC_BIAS_W4S + 32 * c + 16 * hf, w4s);
+          float bb[TC_CW], w4[TC_CW], w4s[TC_CW];
+          tc_ldw(bias + TC_BIAS_B3 + 32 * c + TC_CW * hf, bb);
+          tc_ldw(bias + TC_BIAS_W4 + 32 * c + TC_CW * hf, w4);
+          tc_ldw(bias + TC_BIAS_W4S + 32 * c + TC_CW * hf, w4s);
 #pragma unroll
-          for (int k = 0; k < 16; k += 2) {
+          for (int k = 0; k < TC_CW; k += 2) {
             const float2 x = tc_affine2(z[k], z[k + 1], ks2, kb2, bb[k], bb[k + 1]);
             const float2 d = celu_d2(x);
             epart2 = pk_fma(make_float2(w4[k], w4[k + 1]), celu_h2(x, d), epart2);
@@ -440,13 +445,21 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
             dl[k] = dd.x; dl[k + 1] = dd.y;
           }
           uint8_t* slot = acquire();
-          tc_store_a16(slot, r, hf, dl);
+          tc_store_aw(slot, r, hf, dl);
           publish(&S.a_full[ia % TC_NA]);
           ++ia;
         }
-        S.epart[hf][r] = epart2.x + epart2.y;
+        // (energy partials share the drain's staging block: every drain of the previous tile is over before z3 exists,
+        // and the next drain starts behind the barrier below)
+        float (*epart)[TC_TM] = reinterpret_cast<float (*)[TC_TM]>(&S.stage[0][0]);
+        epart[hf][r] = epart2.x + epart2.y;
         asm volatile("bar.sync 1, %0;" ::"n"(TC_WORKERS) : "memory");
-        if (hf == 0) e_row[row0 + r] = (S.epart[0][r] + S.epart[1][r]) + __ldg(bias + TC_BIAS_B4);
+        if (hf == 0) {
+          float es = epart[0][r];
+#pragma unroll
+          for (int k = 1; k < 32 / TC_CW; ++k) es += epart[k][r];
+          e_row[row0 + r] = es + __ldg(bias + TC_BIAS_B4);
+        }
       }
       if (tid == 0) TC_TRACE(41);
       // ---- delta2 = d2pre * CELU'(z2 + b2): operand of phase 4 ----
@@ -459,19 +472,19 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       if (have_prev) tc::mbar_wait(&S.d1_free, par_prev);      // the previous tile's g passes have read the region
 #pragma unroll 1
       for (int c = 0; c < D2 / TC_KC; ++c) {
-        float z[16], p[16];
-        tc::tmem_ld16(tlane + TC_COL_Z2 + 32 * c + 16 * hf, z);
-        tc::tmem_ld16(tlane + TC_COL_D2 + 32 * c + 16 * hf, p);
+        float z[TC_CW], p[TC_CW];
+        tc_tmem_ldw(tlane + TC_COL_Z2 + 32 * c + TC_CW * hf, z);
+        tc_tmem_ldw(tlane + TC_COL_D2 + 32 * c + TC_CW * hf, p);
         tc::tmem_ld_wait();
-        float bb[16];
-        tc_ld16(bias + TC_BIAS_B2 + 32 * c + 16 * hf, bb);
+        float bb[TC_CW];
+        tc_ldw(bias + TC_BIAS_B2 + 32 * c + TC_CW * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; k += 2) {
+        for (int k = 0; k < TC_CW; k += 2) {
           const float2 pp = make_float2(p[k], p[k + 1]);
           const float2 t = pk_mul(pk_fma(pp, kb3, pk_mul(pp, ks3)), celu_d2(tc_affine2(z[k], z[k + 1], ks1, kb1, bb[k], bb[k + 1])));
           p[k] = t.x; p[k + 1] = t.y;
         }
-        tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
+        tc_store_aw(resD1 + c * TC_A_SLOT, r, hf, p);
       }
       publish(&S.dd_full);
       if (tid == 0) TC_TRACE(43);
@@ -481,26 +494,26 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
       if (tid == 0) TC_TRACE(44);
 #pragma unroll 1
       for (int c = 0; c < TC_ND1; ++c) {
-        float z[16], p[16];
-        tc::tmem_ld16(tlane + TC_COL_Z1 + 32 * c + 16 * hf, z);
-        tc::tmem_ld16(tlane + TC_COL_D1 + 32 * c + 16 * hf, p);
+        float z[TC_CW], p[TC_CW];
+        tc_tmem_ldw(tlane + TC_COL_Z1 + 32 * c + TC_CW * hf, z);
+        tc_tmem_ldw(tlane + TC_COL_D1 + 32 * c + TC_CW * hf, p);
         tc::tmem_ld_wait();
-        float bb[16];
-        tc_ld16(bias + TC_BIAS_B1 + 32 * c + 16 * hf, bb);
+        float bb[TC_CW];
+        tc_ldw(bias + TC_BIAS_B1 + 32 * c + TC_CW * hf, bb);
 #pragma unroll
-        for (int k = 0; k < 16; k += 2) {
+        for (int k = 0; k < TC_CW; k += 2) {
           const float2 pp = make_float2(p[k], p[k + 1]);
           const float2 t = pk_mul(pk_fma(pp, kb4, pk_mul(pp, ks4)), celu_d2(tc_affine2(z[k], z[k + 1], ks0, kb0, bb[k], bb[k + 1])));
           p[k] = t.x; p[k + 1] = t.y;
         }
-        tc_store_a16(resD1 + c * TC_A_SLOT, r, hf, p);
+        tc_store_aw(resD1 + c * TC_A_SLOT, r, hf, p);
         publish(&S.d1_full[c]);
       }
       tc::tc_fence_before();
       tc::mbar_arrive(&S.p5_done);
       if (tid == 0) TC_TRACE(45);
     }
-  } else if (warp == 8) {
+  } else if (warp == TC_NWW) {
     // =========================== TMA: weight chunks ===========================
     if (lane == 0) {
       uint32_t ib = 0;
@@ -533,7 +546,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
         }
       }
     }
-  } else if (warp == 10) {
+  } else if (warp == TC_NWW + 2) {
     // =========================== TMA: the first GEMM's A operand ===========================
     // its own thread, so that a chunk is requested the moment a ring-A slot frees (up to three chunks ahead, and
     // already during the previous tile's last epilogues) instead of when the weight stream's walk reaches it
@@ -654,7 +667,7 @@ k3_mlp_tc_kernel(const __grid_constant__ TcParams P, const uint8_t* __restrict__
   }
   tc::tc_fence_before();
   __syncthreads();
-  if (warp == 9) tc::tmem_dealloc<512>(tbase);
+  if (warp == TC_NWW + 1) tc::tmem_dealloc<512>(tbase);
 }
 
 }  // namespace pfc
