@@ -34,7 +34,7 @@
 // software-pipelined: while the tensor pipe runs the g passes of tile t (delta1 kept RESIDENT in
 // shared memory, produced once) it also runs the first GEMM of tile t+1 (the "overlapped
 // block"); meanwhile warps 0-3 drain g of tile t (TMEM -> global, two accumulator buffers).  Then all
-// eight warps walk the chain z1 -> h1 -> z2 -> h2 -> z3 -> delta3 -> d2pre -> delta2 -> d1pre -> delta1.
+// sixteen worker warps walk the chain z1 -> h1 -> z2 -> h2 -> z3 -> delta3 -> d2pre -> delta2 -> d1pre -> delta1.
 // TMEM (512 columns):  z1 [0,160)   z2 [160,288)   z3 [288,384)   d2pre [384,512)
 //                      d1pre [160,320)   g buffer A [384,512)   g buffer B [160,288)
 // The accumulate step of the tensor core rounds toward zero -- the running sum once per MMA
